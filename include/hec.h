@@ -1,0 +1,168 @@
+/*
+ * hec.h -- C ABI of libhec: batched naive Hasse-Weil point counts of hyperelliptic
+ * curves y^2 = f(x) over small finite fields in Zech-logarithm representation
+ * (arXiv 1805.11991, M. Raum; citations are /root/reference/PAPER.md:<line>).
+ *
+ * Conventions shared by every call
+ *   - extern "C", plain pointers and sizes, no exceptions or aborts cross the ABI.
+ *   - Every int-returning call returns HEC_OK (0) or a negative hec_status;
+ *     hec_last_error() returns a thread-local, NUL-terminated description of the
+ *     last failure on the calling thread (valid until the next failing call).
+ *   - "host or device" pointers are classified with cudaPointerGetAttributes.  All
+ *     array arguments of one call must live on the same side.  Device work is
+ *     enqueued on the stream given to hec_set_stream (default: the legacy default
+ *     stream) and the call returns after that work has completed (it synchronises
+ *     the stream, because the status code depends on device-side validation).
+ *   - The caller owns every buffer it passes in; the library owns hec_field handles
+ *     and its internal per-(q,g) device plans (released by hec_shutdown).
+ *   - An F_q element (q = p^r, p an odd prime) is the integer sum a_i p^i, which
+ *     stands for sum a_i T^i in F_p[T]/(R_q) (little-endian base-p digits,
+ *     PAPER.md:199); R_q is the lexicographically smallest monic primitive
+ *     polynomial of degree r over F_p, ordering the tuple (a_{r-1}, ..., a_0)
+ *     (reading G7).  For prime q this is the plain residue.
+ */
+#ifndef HEC_H
+#define HEC_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum hec_status {
+    HEC_OK = 0,
+    HEC_ERR_INVALID_FIELD = -1,   /* p not an odd prime, r or k < 1, q^k above HEC_MAX_FIELD_SIZE */
+    HEC_ERR_INVALID_ARG = -2,     /* NULL pointer, g < 1, g above HEC_MAX_GENUS, mixed host/device pointers */
+    HEC_ERR_COEFF_RANGE = -3,     /* some coefficient >= q; hec_last_error_index() = first offending row */
+    HEC_ERR_DEGREE = -4,          /* some row has c[2g+2] = c[2g+1] = 0 (degree < 2g+1) */
+    HEC_ERR_CAPACITY = -5,        /* hec_histogram: cap < number of distinct tuples (*out_m is still set) */
+    HEC_ERR_UNSUPPORTED = -6,     /* hec_histogram: the tuple does not pack into 64 bits */
+    HEC_ERR_CUDA = -7,            /* a CUDA runtime call failed, or no device is present */
+    HEC_ERR_NOMEM = -8
+} hec_status;
+
+#define HEC_MAX_FIELD_SIZE (1u << 26)   /* largest supported q^k */
+#define HEC_MAX_GENUS 5u
+
+const char *hec_last_error(void);
+/* Row index attached to the last HEC_ERR_COEFF_RANGE / HEC_ERR_DEGREE on this thread, else (size_t)-1. */
+size_t hec_last_error_index(void);
+
+/* ------------------------------------------------------------------------------------------------
+ * hec_build_field -- section 2.3 and 3.1-3.2.
+ *
+ * Builds F_{q^k}, q = p^r, entirely on the host (no CUDA call): picks the lexicographically
+ * smallest monic primitive polynomial P of degree n = r*k over F_p (reading G7), takes alpha = t as
+ * the generator g_q of PAPER.md:203, and tabulates
+ *   antilog[i] = encoding of alpha^i                       0 <= i <= Q-2
+ *   log[e]     = i with antilog[i] = e, log[0] = Q-1        0 <= e <= Q-1     (encoding (3.1))
+ *   zech[i]    = m(i) with alpha^m(i) = 1 + alpha^i, or Q-1 if 1 + alpha^i = 0   (table (3.2))
+ *   embed[c]   = log of the image in F_{q^k} of the F_q element encoded c, embed[0] = Q-1
+ *                (F_q -> F_{q^k} sends T to rho = alpha^(s (Q-1)/(q-1)), s the smallest unit mod q-1
+ *                 with R_q(rho) = 0; reading G6: NOT simply c's log times (Q-1)/(q-1))
+ * Returns NULL on failure (hec_last_error says why).  The handle is immutable and may be shared
+ * between threads; release it with hec_free_field.
+ */
+typedef struct hec_field hec_field;
+hec_field *hec_build_field(uint32_t p, uint32_t r, uint32_t k);
+void hec_free_field(hec_field *F);
+
+/* Read-only accessors (paper's conventions: logs in [0, Q-2], zero <-> Q-1).  The out arrays are HOST
+ * arrays owned by the caller with the stated number of elements.  A NULL field returns 0 / does nothing. */
+uint32_t hec_field_p(const hec_field *F);
+uint32_t hec_field_degree(const hec_field *F);                 /* n = r*k */
+uint32_t hec_field_q(const hec_field *F);                      /* size of the base field */
+uint32_t hec_field_Q(const hec_field *F);                      /* size of the field, q^k */
+uint32_t hec_field_embed_unit(const hec_field *F);             /* s above (1 when k = 1) */
+void hec_field_modulus(const hec_field *F, uint32_t *out);     /* n+1 coefficients a_0..a_{n-1}, 1 */
+void hec_field_antilog(const hec_field *F, uint32_t *out);     /* Q-1 entries */
+void hec_field_log(const hec_field *F, uint32_t *out);         /* Q entries */
+void hec_field_zech(const hec_field *F, uint32_t *out);        /* Q-1 entries */
+void hec_field_embed(const hec_field *F, uint32_t *out);       /* q entries */
+
+/* ------------------------------------------------------------------------------------------------
+ * hec_count -- Algorithm 1 lines 6-14 for a whole batch of curves, plus the
+ * points at infinity and x = 0 and the squarefree filter.
+ *
+ *   coeffs[n][2g+3]   row-major uint16, coeffs[i][j] = coefficient of X^j of curve i (F_q encoding above)
+ *   out_counts[n][g]  uint32, row i = (N_1 .. N_g), N_k = #C_f(F_{q^k})
+ *                       = #{x: f(x)=0} + 2 #{x: f(x) a nonzero square} + (1 if c_{2g+2}=0;
+ *                         2 if c_{2g+2} a nonzero square in F_{q^k}; else 0)
+ *   out_squarefree[n] uint8 in {0,1}: deg gcd(f, f') = 0 over F_q; may be NULL
+ * N_k is computed by the same formula whether or not f is squarefree (reading G12).
+ * Pointers: all host or all device.  Host pointers: the library stages the batch through its own
+ * device buffers (H2D, kernels, D2H) on the current stream.  n = 0 is a no-op.
+ * Errors: HEC_ERR_INVALID_FIELD (q not an odd prime power below 65536, q^g too large),
+ * HEC_ERR_INVALID_ARG, HEC_ERR_COEFF_RANGE, HEC_ERR_DEGREE (outputs are unspecified after these
+ * two), HEC_ERR_CUDA, HEC_ERR_NOMEM.
+ */
+int hec_count(uint32_t q, uint32_t g, const uint16_t *coeffs, size_t n,
+              uint32_t *out_counts, uint8_t *out_squarefree);
+
+/* ------------------------------------------------------------------------------------------------
+ * hec_histogram -- the multiplicity map of eq. (1.2) / Algorithm 1 line 20
+ * in its reduced form: unweighted, keyed by the tuple (N_1..N_g) only.
+ *
+ *   counts[n][g]      uint32 rows (typically hec_count's output)
+ *   mask[n]           uint8 or NULL; rows with mask 0 are skipped (the paper counts squarefree f only)
+ *   out_tuples[cap][g], out_mult[cap]   distinct rows in ASCENDING LEXICOGRAPHIC order + multiplicities
+ *   *out_m            number of distinct rows (HOST pointer, always written on HEC_OK / HEC_ERR_CAPACITY)
+ * Two-call pattern: if cap < *out_m nothing is written to out_tuples/out_mult and HEC_ERR_CAPACITY is
+ * returned; out_tuples/out_mult may be NULL when cap = 0.  counts/mask/out_tuples/out_mult: all host or
+ * all device.  Sum of out_mult = number of unmasked rows.  HEC_ERR_UNSUPPORTED if the per-column
+ * ranges (max - min) need more than 64 bits in total.
+ */
+int hec_histogram(const uint32_t *counts, const uint8_t *mask, size_t n, uint32_t g,
+                  uint32_t *out_tuples, uint64_t *out_mult, size_t cap, size_t *out_m);
+
+/* ------------------------------------------------------------------------------------------------
+ * Execution control and instrumentation (used by the tests, bench.py and the ncu runs).
+ */
+/* cudaStream_t (as void*) on which later calls enqueue their device work; NULL = default stream. */
+int hec_set_stream(void *cuda_stream);
+
+typedef enum hec_regime {
+    HEC_REGIME_AUTO = 0,    /* shared-memory table when the extended Zech table of F_{q^k} fits, else L2 */
+    HEC_REGIME_SMEM = 1,    /* force shared memory (fails with HEC_ERR_INVALID_ARG when it cannot fit) */
+    HEC_REGIME_L2 = 2       /* force the L2-resident (global memory, 32-bit entries) table for the largest field */
+} hec_regime;
+int hec_set_regime(int regime);
+
+/* Statistics of the last hec_count on this thread's library state: device time of the count kernel and
+ * of the squarefree kernel (CUDA events on the launch stream, ms), number of kernel launches, the regime
+ * used for the largest field (hec_regime), dynamic shared memory bytes per CTA, grid and block size. */
+typedef struct hec_count_stats {
+    float count_kernel_ms;
+    float squarefree_kernel_ms;
+    uint32_t launches;
+    uint32_t regime;
+    uint32_t smem_bytes;
+    uint32_t grid;
+    uint32_t block;
+    uint32_t chains_per_lane;
+} hec_count_stats;
+int hec_last_count_stats(hec_count_stats *out);
+
+/* Total number of kernels launched by this library since load (bench.py's gpu_launches). */
+uint64_t hec_launch_count(void);
+
+/*
+ * Gather micro-benchmark for the lookup ceilings: every lane follows a dependent chain
+ * idx <- table[idx] + lane-dependent offset through a table of `entries` uniformly random entries of
+ * `entry_bytes` (2 or 4) bytes.  where = 0: shared memory; 1: global memory through L1 (ld.global.nc);
+ * 2: global memory bypassing L1 (ld.global.cg).  Runs `lookups_per_lane` dependent lookups on each of
+ * `chains` independent chains per lane with one CTA of `block` threads per SM times `ctas_per_sm`,
+ * and writes lookups per second and the kernel time.  Table contents are seeded.
+ */
+int hec_gather_bench(int where, uint32_t entries, uint32_t entry_bytes, uint32_t block, uint32_t ctas_per_sm,
+                     uint32_t chains, uint32_t lookups_per_lane, double *out_lookups_per_s, float *out_ms);
+
+/* Release cached fields, device plans and staging buffers. */
+void hec_shutdown(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* HEC_H */

@@ -1,0 +1,230 @@
+"""Thin ctypes binding of libhec.so (include/hec.h): argument marshalling only.
+
+Every step of the path runs in the library's CUDA kernels.  There is no CPU fallback: if
+libhec.so is missing the first call raises, and on a box without a GPU `count`,
+`histogram` and `gather_bench` raise HecError(HEC_ERR_CUDA) (only `build_field`, which is
+host code by design, works without a device).  Arrays may be numpy arrays (host pointers)
+or torch CUDA tensors (device pointers, passed as data_ptr()); results come back the
+same way.
+"""
+from __future__ import annotations
+
+import ctypes
+from pathlib import Path
+
+import numpy as np
+
+_PKG = Path(__file__).resolve().parent
+LIB_PATH = _PKG / "libhec.so"
+_lib = None
+
+HEC_OK = 0
+HEC_ERR_INVALID_FIELD, HEC_ERR_INVALID_ARG, HEC_ERR_COEFF_RANGE, HEC_ERR_DEGREE = -1, -2, -3, -4
+HEC_ERR_CAPACITY, HEC_ERR_UNSUPPORTED, HEC_ERR_CUDA, HEC_ERR_NOMEM = -5, -6, -7, -8
+REGIME_AUTO, REGIME_SMEM, REGIME_L2 = 0, 1, 2
+MAX_GENUS = 5
+
+# every symbol include/hec.h declares (tests check the library exports all of them)
+SYMBOLS = [
+    "hec_last_error", "hec_last_error_index", "hec_build_field", "hec_free_field", "hec_field_p",
+    "hec_field_degree", "hec_field_q", "hec_field_Q", "hec_field_embed_unit", "hec_field_modulus",
+    "hec_field_antilog", "hec_field_log", "hec_field_zech", "hec_field_embed", "hec_count", "hec_histogram",
+    "hec_set_stream", "hec_set_regime", "hec_last_count_stats", "hec_launch_count", "hec_gather_bench",
+    "hec_shutdown",
+]
+
+
+class HecError(RuntimeError):
+    def __init__(self, code: int, msg: str, index: int | None = None):
+        super().__init__(f"libhec error {code}: {msg}" + (f" (row {index})" if index is not None else ""))
+        self.code, self.index = code, index
+
+
+class CountStats(ctypes.Structure):
+    _fields_ = [("count_kernel_ms", ctypes.c_float), ("squarefree_kernel_ms", ctypes.c_float),
+                ("launches", ctypes.c_uint32), ("regime", ctypes.c_uint32), ("smem_bytes", ctypes.c_uint32),
+                ("grid", ctypes.c_uint32), ("block", ctypes.c_uint32), ("chains_per_lane", ctypes.c_uint32)]
+
+
+def lib():
+    """Load libhec.so (built in-tree by paper_1805_11991_b200/build.py); fail loudly if absent."""
+    global _lib
+    if _lib is None:
+        if not LIB_PATH.exists():
+            raise ImportError(f"{LIB_PATH} is missing: run `python -c 'import __graft_entry__ as g; g.build()'` "
+                              "(nvcc, sm_100a). libhec has no CPU fallback.")
+        L = ctypes.CDLL(str(LIB_PATH))
+        u32, vp, sz = ctypes.c_uint32, ctypes.c_void_p, ctypes.c_size_t
+        L.hec_last_error.restype = ctypes.c_char_p
+        L.hec_last_error_index.restype = sz
+        L.hec_build_field.restype = vp
+        L.hec_build_field.argtypes = [u32, u32, u32]
+        L.hec_free_field.argtypes = [vp]
+        for name in ("p", "degree", "q", "Q", "embed_unit"):
+            f = getattr(L, f"hec_field_{name}")
+            f.restype, f.argtypes = u32, [vp]
+        for name in ("modulus", "antilog", "log", "zech", "embed"):
+            f = getattr(L, f"hec_field_{name}")
+            f.restype, f.argtypes = None, [vp, vp]
+        L.hec_count.argtypes = [u32, u32, vp, sz, vp, vp]
+        L.hec_histogram.argtypes = [vp, vp, sz, u32, vp, vp, sz, ctypes.POINTER(sz)]
+        L.hec_set_stream.argtypes = [vp]
+        L.hec_set_regime.argtypes = [ctypes.c_int]
+        L.hec_last_count_stats.argtypes = [ctypes.POINTER(CountStats)]
+        L.hec_launch_count.restype = ctypes.c_uint64
+        L.hec_gather_bench.argtypes = [ctypes.c_int, u32, u32, u32, u32, u32, u32,
+                                       ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_float)]
+        L.hec_shutdown.restype = None
+        _lib = L
+    return _lib
+
+
+def _check(rc: int):
+    if rc != HEC_OK:
+        L = lib()
+        idx = L.hec_last_error_index()
+        raise HecError(rc, L.hec_last_error().decode(), None if idx == ctypes.c_size_t(-1).value else idx)
+
+
+def _is_torch(x) -> bool:
+    return type(x).__module__.startswith("torch")
+
+
+def _ptr(x):
+    if x is None:
+        return None
+    return x.data_ptr() if _is_torch(x) else x.ctypes.data
+
+
+class Field:
+    """hec_build_field handle with the read-only accessors of hec.h (paper's conventions)."""
+
+    def __init__(self, p: int, r: int, k: int):
+        L = lib()
+        self._h = L.hec_build_field(p, r, k)
+        if not self._h:
+            raise HecError(HEC_ERR_INVALID_FIELD, L.hec_last_error().decode())
+        self.p, self.r, self.k = p, r, k
+        self.n = L.hec_field_degree(self._h)
+        self.q = L.hec_field_q(self._h)
+        self.Q = L.hec_field_Q(self._h)
+        self.embed_unit = L.hec_field_embed_unit(self._h)
+
+    def _arr(self, name: str, size: int) -> np.ndarray:
+        out = np.empty(size, dtype=np.uint32)
+        getattr(lib(), f"hec_field_{name}")(self._h, out.ctypes.data)
+        return out
+
+    @property
+    def modulus(self):
+        return self._arr("modulus", self.n + 1).tolist()
+
+    @property
+    def antilog(self):
+        return self._arr("antilog", self.Q - 1)
+
+    @property
+    def log(self):
+        return self._arr("log", self.Q)
+
+    @property
+    def zech(self):
+        return self._arr("zech", self.Q - 1)
+
+    @property
+    def embed(self):
+        return self._arr("embed", self.q)
+
+    def close(self):
+        if self._h:
+            lib().hec_free_field(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+def build_field(p: int, r: int, k: int) -> Field:
+    return Field(p, r, k)
+
+
+def set_stream(cuda_stream: int | None):
+    """cuda_stream: a cudaStream_t as an integer (e.g. torch.cuda.current_stream().cuda_stream) or None."""
+    _check(lib().hec_set_stream(ctypes.c_void_p(cuda_stream or 0)))
+
+
+def set_regime(regime: int):
+    _check(lib().hec_set_regime(regime))
+
+
+def count(q: int, g: int, coeffs, out_counts=None, out_squarefree=None, want_squarefree: bool = True):
+    """hec_count.  coeffs: uint16 [n][2g+3], numpy (host) or torch CUDA tensor (device).
+    Returns (counts uint32-valued [n][g], squarefree uint8 [n] or None) of the same kind as coeffs
+    (torch has no uint32 arithmetic: device counts come back as an int32 tensor holding the same bits)."""
+    n = int(coeffs.shape[0])
+    if tuple(coeffs.shape[1:]) != (2 * g + 3,):
+        raise ValueError("coeffs must be [n][2g+3]")
+    if _is_torch(coeffs):
+        import torch
+        if coeffs.dtype not in (torch.uint16, torch.int16) or not coeffs.is_contiguous():
+            raise ValueError("device coeffs must be a contiguous uint16/int16 tensor")
+        if out_counts is None:
+            out_counts = torch.empty((n, g), dtype=torch.int32, device=coeffs.device)
+        if out_squarefree is None and want_squarefree:
+            out_squarefree = torch.empty((n,), dtype=torch.uint8, device=coeffs.device)
+    else:
+        coeffs = np.ascontiguousarray(coeffs, dtype=np.uint16)
+        if out_counts is None:
+            out_counts = np.empty((n, g), dtype=np.uint32)
+        if out_squarefree is None and want_squarefree:
+            out_squarefree = np.empty((n,), dtype=np.uint8)
+    _check(lib().hec_count(q, g, _ptr(coeffs), n, _ptr(out_counts), _ptr(out_squarefree)))
+    return out_counts, out_squarefree
+
+
+def histogram(counts, mask=None):
+    """hec_histogram with the two-call pattern.  Returns (tuples [m][g], multiplicities [m])."""
+    n, g = int(counts.shape[0]), int(counts.shape[1])
+    L = lib()
+    m = ctypes.c_size_t(0)
+    rc = L.hec_histogram(_ptr(counts), _ptr(mask), n, g, None, None, 0, ctypes.byref(m))
+    if rc not in (HEC_OK, HEC_ERR_CAPACITY):
+        _check(rc)
+    cap = m.value
+    if _is_torch(counts):
+        import torch
+        tup = torch.empty((cap, g), dtype=torch.int32, device=counts.device)
+        mult = torch.empty((cap,), dtype=torch.int64, device=counts.device)
+    else:
+        counts = np.ascontiguousarray(counts, dtype=np.uint32)
+        tup = np.empty((cap, g), dtype=np.uint32)
+        mult = np.empty((cap,), dtype=np.uint64)
+    if cap:
+        _check(L.hec_histogram(_ptr(counts), _ptr(mask), n, g, _ptr(tup), _ptr(mult), cap, ctypes.byref(m)))
+    return tup, mult
+
+
+def last_count_stats() -> dict:
+    s = CountStats()
+    _check(lib().hec_last_count_stats(ctypes.byref(s)))
+    return {name: getattr(s, name) for name, _ in s._fields_}
+
+
+def launch_count() -> int:
+    return int(lib().hec_launch_count())
+
+
+def gather_bench(where: int, entries: int, entry_bytes: int, block: int = 1024, ctas_per_sm: int = 1,
+                 chains: int = 4, lookups_per_lane: int = 4096) -> tuple[float, float]:
+    """Returns (lookups per second, kernel ms) of the dependent random-gather micro-benchmark."""
+    rate, ms = ctypes.c_double(0), ctypes.c_float(0)
+    _check(lib().hec_gather_bench(where, entries, entry_bytes, block, ctas_per_sm, chains, lookups_per_lane,
+                                  ctypes.byref(rate), ctypes.byref(ms)))
+    return rate.value, ms.value
+
+
+def shutdown():
+    lib().hec_shutdown()

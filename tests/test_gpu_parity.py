@@ -1,0 +1,229 @@
+"""Parity of the CUDA path (through the C ABI, paper_1805_11991_b200.hec) against the CPU oracle.
+
+Integer work: the bar is bit-exact.  Small cases are compared element by element; at BASELINE.json's
+full sizes (in the launch configuration bench.py times) the oracle checks a deterministic sample and every
+row is checked against properties that hold at any size (Weil bound on squarefree rows, parity, histogram
+totals, regime independence).
+"""
+import numpy as np
+import pytest
+
+from oracle import hec_oracle as O
+from paper_1805_11991_b200 import hec, workloads as W
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def torch_cuda():
+    import torch
+    from paper_1805_11991_b200 import build as hb
+    hb.build_lib()
+    assert torch.cuda.is_available()
+    torch.cuda.set_device(0)
+    hec.set_stream(torch.cuda.current_stream().cuda_stream)
+    hec.set_regime(hec.REGIME_AUTO)
+    return torch
+
+
+def _dev(torch, rows):
+    return torch.from_numpy(np.ascontiguousarray(rows).view(np.int16)).cuda()
+
+
+def _gpu_count(torch, q, g, rows):
+    cnt, sf = hec.count(q, g, _dev(torch, rows))
+    return cnt.cpu().numpy().view(np.uint32), sf.cpu().numpy()
+
+
+def _assert_parity(torch, q, g, rows, k_hi=None):
+    cnt, sf = _gpu_count(torch, q, g, rows)
+    ocnt, osf, _ = O.count(q, g, rows, k_hi=k_hi)
+    kk = g if k_hi is None else k_hi
+    assert (cnt[:, :kk] == ocnt[:, :kk]).all(), np.argwhere(cnt[:, :kk] != ocnt[:, :kk])[:5]
+    assert (sf == osf).all(), np.argwhere(sf != osf)[:5]
+    return cnt, sf
+
+
+# ------------------------------------------------------------------------------------------ small, element by element
+
+def test_config1_exhaustive_device_and_host_pointers(torch_cuda):
+    rows = W.generate(W.CONFIGS[1])
+    cnt, sf = _assert_parity(torch_cuda, 3, 2, rows)
+    # host pointers (the library stages H2D/D2H itself)
+    hcnt, hsf = hec.count(3, 2, rows)
+    assert (hcnt == cnt).all() and (hsf == sf).all()
+    # histogram, all rows and squarefree rows only
+    for mask in (None, sf):
+        otup, omult = O.histogram(cnt, mask)
+        tup, mult = hec.histogram(cnt, mask)
+        assert (tup == otup).all() and (mult == omult).all()
+        dt, dm = hec.histogram(torch_cuda.from_numpy(cnt.view(np.int32)).cuda(),
+                               None if mask is None else torch_cuda.from_numpy(mask).cuda())
+        assert (dt.cpu().numpy().view(np.uint32) == otup).all() and (dm.cpu().numpy().view(np.uint64) == omult).all()
+
+
+@pytest.mark.parametrize("cid,n_all,n_top", [(2, 1500, 1500), (3, 160, 10), (4, 260, 70), (5, 300, 40)])
+def test_config_slices_against_oracle(torch_cuda, cid, n_all, n_top):
+    """First rows of each seeded workload: all N_k for n_top rows, N_k (k < g) for n_all rows.
+    Sizes span several CTAs' worth of warps and a ragged tail."""
+    cfg = W.CONFIGS[cid]
+    rows = W.generate(cfg, 0, n_all)
+    cnt, sf = _gpu_count(torch_cuda, cfg.q, cfg.g, rows)
+    ocnt, osf, _ = O.count(cfg.q, cfg.g, rows, k_hi=cfg.g - 1)
+    assert (cnt[:, : cfg.g - 1] == ocnt[:, : cfg.g - 1]).all()
+    assert (sf == osf).all()
+    otop, _, _ = O.count(cfg.q, cfg.g, rows[:n_top], k_lo=cfg.g, k_hi=cfg.g, want_squarefree=False)
+    assert (cnt[:n_top, cfg.g - 1] == otop[:, cfg.g - 1]).all()
+
+
+@pytest.mark.parametrize("q,g,k_hi", [(3, 2, 2), (13, 4, 3), (25, 2, 2), (49, 3, 2), (293, 2, 1), (9, 1, 1), (5, 3, 3), (27, 2, 2), (7, 5, 3)])
+def test_edge_rows(torch_cuda, q, g, k_hi):
+    """Degenerate inputs: monomials, c x^{2g+2} for every c, sparse rows (gaps > 1), c_0 = 0, all-(q-1)."""
+    rows = W.edge_rows(q, g)
+    _assert_parity(torch_cuda, q, g, rows, k_hi=k_hi)
+
+
+def test_edge_rows_top_field_q13_g4(torch_cuda):
+    rows = W.edge_rows(13, 4)[::3]
+    _assert_parity(torch_cuda, 13, 4, rows)
+
+
+@pytest.mark.parametrize("n", [1, 2, 31, 32, 33, 4735, 4737])
+def test_ragged_batch_sizes(torch_cuda, n):
+    cfg = W.CONFIGS[2]
+    rows = W.generate(cfg, 1000, n)
+    cnt, sf = _gpu_count(torch_cuda, cfg.q, cfg.g, rows)
+    idx = np.unique(np.concatenate([np.arange(min(n, 40)), np.arange(max(0, n - 40), n)]))
+    ocnt, osf, _ = O.count(cfg.q, cfg.g, rows[idx])
+    assert (cnt[idx] == ocnt).all() and (sf[idx] == osf).all()
+
+
+def test_sparse_and_zero_heavy_rows(torch_cuda):
+    """Random rows with many zero coefficients (exercises every gap m_j and trailing zeros)."""
+    rng = np.random.default_rng(7)
+    for q, g in [(13, 2), (25, 2), (7, 3)]:
+        rows = rng.integers(0, q, size=(400, 2 * g + 3)).astype(np.uint16)
+        rows[rng.random(rows.shape) < 0.6] = 0
+        rows[:, -1] = np.where(rng.random(400) < 0.5, rng.integers(1, q, 400), 0)
+        rows[:, -2] = np.where(rows[:, -1] == 0, rng.integers(1, q, 400), rows[:, -2])
+        _assert_parity(torch_cuda, q, g, rows)
+
+
+def test_regimes_agree(torch_cuda):
+    """The L2-resident (global, 32-bit) table and the shared-memory (16-bit) table give identical counts."""
+    try:
+        for cid, n in [(2, 3000), (4, 600)]:
+            cfg = W.CONFIGS[cid]
+            rows = W.generate(cfg, 5000, n)
+            hec.set_regime(hec.REGIME_SMEM)
+            a, sa = _gpu_count(torch_cuda, cfg.q, cfg.g, rows)
+            assert hec.last_count_stats()["regime"] == hec.REGIME_SMEM
+            hec.set_regime(hec.REGIME_L2)
+            b, sb = _gpu_count(torch_cuda, cfg.q, cfg.g, rows)
+            assert hec.last_count_stats()["regime"] == hec.REGIME_L2
+            assert (a == b).all() and (sa == sb).all()
+        hec.set_regime(hec.REGIME_SMEM)
+        with pytest.raises(hec.HecError):
+            _gpu_count(torch_cuda, 293, 2, W.generate(W.CONFIGS[5], 0, 8))
+    finally:
+        hec.set_regime(hec.REGIME_AUTO)
+
+
+# ------------------------------------------------------------------------------------------ boundary behaviour
+
+def test_error_codes(torch_cuda):
+    good = W.generate(W.CONFIGS[2], 0, 100)
+    bad = good.copy(); bad[37, 3] = 25
+    with pytest.raises(hec.HecError) as e:
+        hec.count(25, 2, _dev(torch_cuda, bad))
+    assert e.value.code == hec.HEC_ERR_COEFF_RANGE and e.value.index == 37
+    bad = good.copy(); bad[61, 5] = 0; bad[61, 6] = 0; bad[80, 5] = 0; bad[80, 6] = 0
+    with pytest.raises(hec.HecError) as e:
+        hec.count(25, 2, bad)
+    assert e.value.code == hec.HEC_ERR_DEGREE and e.value.index == 61
+    for q, g in [(15, 2), (4, 2), (1, 2), (13, 0), (13, 6), (293, 4)]:
+        with pytest.raises(hec.HecError):
+            hec.count(q, g, np.zeros((1, 2 * g + 3), dtype=np.uint16))
+    # mixed host / device pointers
+    with pytest.raises(hec.HecError) as e:
+        hec.count(25, 2, _dev(torch_cuda, good), out_counts=np.empty((100, 2), dtype=np.uint32))
+    assert e.value.code == hec.HEC_ERR_INVALID_ARG
+    # empty batch is a no-op
+    cnt, sf = hec.count(25, 2, np.zeros((0, 7), dtype=np.uint16))
+    assert cnt.shape == (0, 2)
+    # the library still works after errors
+    cnt, _ = hec.count(25, 2, good[:10])
+    assert (cnt == O.count(25, 2, good[:10])[0]).all()
+
+
+def test_histogram_random_tuples_and_capacity(torch_cuda):
+    rng = np.random.default_rng(11)
+    cases = [
+        rng.integers(0, 50, size=(100000, 2)),                       # few distinct, heavy multiplicities
+        rng.integers(0, 2 ** 20, size=(300000, 3)),                  # almost all distinct
+        np.stack([rng.integers(5, 9, 50000), rng.integers(2 ** 31, 2 ** 31 + 1000, 50000)], axis=1),
+        np.full((1000, 4), 7),                                       # single tuple, zero-width key
+        rng.integers(0, 3, size=(5, 1)),
+    ]
+    for c in cases:
+        c = c.astype(np.uint32)
+        mask = (rng.random(len(c)) < 0.7).astype(np.uint8)
+        for m in (None, mask):
+            otup, omult = O.histogram(c, m)
+            tup, mult = hec.histogram(c, m)
+            assert tup.shape == otup.shape and (tup == otup).all() and (mult == omult).all()
+            assert int(mult.sum()) == (len(c) if m is None else int(m.sum()))
+    # all rows masked out
+    tup, mult = hec.histogram(cases[0].astype(np.uint32), np.zeros(len(cases[0]), dtype=np.uint8))
+    assert tup.shape[0] == 0
+    # capacity error keeps *out_m
+    import ctypes
+    c = cases[0].astype(np.uint32)
+    m = ctypes.c_size_t(0)
+    tup = np.empty((3, 2), dtype=np.uint32); mult = np.empty(3, dtype=np.uint64)
+    rc = hec.lib().hec_histogram(c.ctypes.data, None, len(c), 2, tup.ctypes.data, mult.ctypes.data, 3, ctypes.byref(m))
+    assert rc == hec.HEC_ERR_CAPACITY and m.value == len(O.histogram(c)[0])
+    # more than 63 bits of key
+    wide = rng.integers(0, 2 ** 32, size=(100, 3), dtype=np.uint64).astype(np.uint32)
+    with pytest.raises(hec.HecError) as e:
+        hec.histogram(wide)
+    assert e.value.code == hec.HEC_ERR_UNSUPPORTED
+
+
+# ------------------------------------------------------------------------------------------ full sizes
+
+def _full_size_checks(torch, cid, S):
+    cfg = W.CONFIGS[cid]
+    rows = W.generate(cfg)
+    d_rows = _dev(torch, rows)
+    cnt_d, sf_d = hec.count(cfg.q, cfg.g, d_rows)
+    stats = hec.last_count_stats()
+    cnt, sf = cnt_d.cpu().numpy().view(np.uint32), sf_d.cpu().numpy()
+    # oracle on a deterministic sample
+    idx = W.sample_indices(cfg, S)
+    ocnt, osf, _ = O.count(cfg.q, cfg.g, rows[idx])
+    assert (cnt[idx] == ocnt).all() and (sf[idx] == osf).all()
+    # properties on every row
+    q, g = cfg.q, cfg.g
+    sq = sf == 1
+    for k in range(1, g + 1):
+        nk = cnt[:, k - 1].astype(np.int64)
+        assert (np.abs(nk[sq] - (q ** k + 1)) <= np.floor(2 * g * q ** (k / 2))).all(), f"Weil bound, k={k}"
+        assert (nk <= 2 * q ** k + 2).all()
+    # squarefree density ~ 1 - 1/q
+    assert abs(sq.mean() - (1 - 1 / q)) < 0.01
+    # histogram of the device counts against sort + run-length
+    tup_d, mult_d = hec.histogram(cnt_d, sf_d)
+    otup, omult = O.histogram(cnt, sf)
+    assert (tup_d.cpu().numpy().view(np.uint32) == otup).all()
+    assert (mult_d.cpu().numpy().view(np.uint64) == omult).all()
+    return stats
+
+
+def test_full_config2(torch_cuda):
+    _full_size_checks(torch_cuda, 2, 2048)
+
+
+def test_full_config4_headline(torch_cuda):
+    stats = _full_size_checks(torch_cuda, 4, 96)
+    assert stats["regime"] == hec.REGIME_SMEM
