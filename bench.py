@@ -1,0 +1,335 @@
+#!/usr/bin/env python
+"""bench.py -- whole hot path of arXiv 1805.11991 on B200 (driver contract in the task statement).
+
+One "step" = one pass of the whole hot path over one batch of synthetic curves:
+    hec_count (embed + Horner at every x of F_{q^k}, k = 1..g, + classify/reduce + x = 0 and infinity
+    + squarefree flag)  ->  hec_histogram (multiplicities of the squarefree tuples)
+    [N > 1: + all-gather of the partial histograms and hec_histogram_merge]
+Default workload: BASELINE.json's headline config, q = 13, g = 4, 2^24 curves (degree 9/10), which fits one
+GPU.  `--config {1,2,3,5}` runs the other seeded workloads (parity-test cases, not bench lines).
+
+  python bench.py [--gpus N --steps K --warmup W] [--config C] [--impl reference]
+  python -m torch.distributed.run --nnodes=1 --nproc-per-node N --master-addr 127.0.0.1 --master-port P \
+         bench.py --gpus N --steps K --warmup W
+
+`--impl reference` times the CPU oracle (oracle/, as it stands) on a bounded sample of the same workload.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+from pathlib import Path
+
+import numpy as np
+
+ROOT = Path(__file__).resolve().parent
+if str(ROOT) not in sys.path:
+    sys.path.insert(0, str(ROOT))
+
+from paper_1805_11991_b200 import workloads as W  # noqa: E402
+
+EXPECTED_WAVEFRONTS = 3.53      # E[max bank load], 32 uniformly random 2-byte lookups in 32 banks
+
+
+# ------------------------------------------------------------------------------------------------ helpers
+
+def workload_rows(cfg: W.Workload, rank: int) -> np.ndarray:
+    """Weak scaling: rank r takes rows [r n, (r+1) n) of the counter-based generator (exhaustive config: all)."""
+    if cfg.degree_mode == "exhaustive":
+        return W.generate(cfg, 0, cfg.n)
+    return W.generate(cfg, rank * cfg.n, cfg.n)
+
+
+def algorithmic_lookups(cfg: W.Workload, rows: np.ndarray) -> int:
+    """One Zech lookup per Horner step with a nonzero coefficient, at every nonzero x of every F_{q^k}
+    (SURVEY.md 8(d)): sum over curves of (#nonzero coefficients - 1) * sum_k (q^k - 1)."""
+    steps = (rows != 0).sum(axis=1).astype(np.int64) - 1
+    nx = sum(cfg.q ** k - 1 for k in range(1, cfg.g + 1))
+    return int(steps.sum()) * nx
+
+
+class ClockSampler:
+    """Samples SM clock and throttle reasons during the timed region (pynvml, 100 ms period)."""
+    REASONS = {0x4: "sw_power_cap", 0x8: "hw_slowdown", 0x20: "sw_thermal_slowdown", 0x40: "hw_thermal_slowdown",
+               0x80: "hw_power_brake_slowdown", 0x2: "applications_clocks_setting", 0x10: "sync_boost"}
+
+    def __init__(self, index: int):
+        self.samples, self.reasons, self.max_mhz = [], set(), None
+        self._stop = threading.Event()
+        self._thread = None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self._nv = pynvml
+            visible = os.environ.get("CUDA_VISIBLE_DEVICES")
+            phys = int(visible.split(",")[index]) if visible and visible.split(",")[index].isdigit() else index
+            self._h = pynvml.nvmlDeviceGetHandleByIndex(phys)
+            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self._h, pynvml.NVML_CLOCK_SM)
+        except Exception:
+            self._nv = None
+
+    def _run(self):
+        nv = self._nv
+        while not self._stop.is_set():
+            try:
+                self.samples.append(nv.nvmlDeviceGetClockInfo(self._h, nv.NVML_CLOCK_SM))
+                mask = nv.nvmlDeviceGetCurrentClocksEventReasons(self._h)
+                for bit, name in self.REASONS.items():
+                    if mask & bit:
+                        self.reasons.add(name)
+            except Exception:
+                pass
+            self._stop.wait(0.1)
+
+    def __enter__(self):
+        if self._nv:
+            self._thread = threading.Thread(target=self._run, daemon=True)
+            self._thread.start()
+        return self
+
+    def __exit__(self, *exc):
+        self._stop.set()
+        if self._thread:
+            self._thread.join()
+
+    def summary(self) -> dict:
+        if not self.samples:
+            return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": ["unavailable"]}
+        return {"sm_mhz": float(np.median(self.samples)), "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons)}
+
+
+def oracle_sample_run(cfg: W.Workload, target_s: float):
+    """Times the oracle, as it stands, on a bounded deterministic sample of the workload (all host cores)."""
+    from oracle import hec_oracle as O
+    cores = os.cpu_count() or 1
+    probe = W.rows_by_index(cfg, W.sample_indices(cfg, max(2, min(cores, cfg.n)), edge=0))
+    t0 = time.perf_counter()
+    O.count(cfg.q, cfg.g, probe)
+    per_curve_core = (time.perf_counter() - t0) * min(cores, len(probe)) / len(probe)
+    S = int(max(len(probe), min(cfg.n, target_s * cores / max(per_curve_core, 1e-9))))
+    idx = W.sample_indices(cfg, S, edge=0)
+    rows = W.rows_by_index(cfg, idx)
+    t0 = time.perf_counter()
+    cnt, sf, used = O.count(cfg.q, cfg.g, rows)
+    O.histogram(cnt, sf)
+    dt = time.perf_counter() - t0
+    return len(rows), dt, used, rows, cnt, sf
+
+
+# ------------------------------------------------------------------------------------------------ reference arm
+
+def run_reference(args, cfg):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    from oracle import hec_oracle as O
+    cores = os.cpu_count() or 1
+    S0, dt0, used, *_ = oracle_sample_run(cfg, 4.0)
+    per_curve = dt0 / S0
+    S = int(max(1, min(cfg.n, 6.0 / per_curve)))            # ~6 s of CPU work per step
+    idx = W.sample_indices(cfg, S, edge=0)
+    rows = W.rows_by_index(cfg, idx)
+    for _ in range(args.warmup):
+        cnt, sf, used = O.count(cfg.q, cfg.g, rows[: max(1, len(rows) // 8)])
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        cnt, sf, used = O.count(cfg.q, cfg.g, rows)
+        O.histogram(cnt, sf)
+    dt = time.perf_counter() - t0
+    value = len(rows) * args.steps / dt
+    sample = f"{len(rows)} curves per step: every {cfg.n // max(1, S)}-th row of {cfg.name} (n = {cfg.n})"
+    line = {
+        "impl": "reference", "metric": "curves_per_s", "value": value, "unit": "curves/s", "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt / args.steps * 1e3, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "u32", "data": "synthetic",
+        "config": {"workload": cfg.name, "q": cfg.q, "g": cfg.g, "n_curves": cfg.n, "sample": sample},
+        "xevals_per_s": value * cfg.xevals_per_curve,
+        "cpu_baseline": {"value": value, "unit": "curves/s", "cores": used, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": "curves/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0, "host_cores": cores,
+    }
+    print(json.dumps(line), flush=True)
+
+
+# ------------------------------------------------------------------------------------------------ our arm
+
+def run_ours(args, cfg):
+    import torch
+    from paper_1805_11991_b200 import build as hb, distributed as D, hec
+
+    rank, local_rank, world = D.init_from_env()
+    if world != args.gpus:
+        raise SystemExit(f"--gpus {args.gpus} but WORLD_SIZE={world}: launch with torch.distributed.run")
+    torch.cuda.set_device(local_rank)
+    dist = torch.distributed
+    if rank == 0:
+        hb.build_lib()
+    if world > 1:
+        dist.barrier()
+    stream = torch.cuda.current_stream()
+    hec.set_stream(stream.cuda_stream)
+    hec.set_regime({"auto": hec.REGIME_AUTO, "smem": hec.REGIME_SMEM, "l2": hec.REGIME_L2}[args.regime])
+
+    rows = workload_rows(cfg, rank)
+    n, g, q = rows.shape[0], cfg.g, cfg.q
+    lookups = algorithmic_lookups(cfg, rows)
+    d_rows = torch.from_numpy(rows.view(np.int16)).cuda()
+    d_cnt = torch.empty((n, g), dtype=torch.int32, device="cuda")
+    d_sf = torch.empty((n,), dtype=torch.uint8, device="cuda")
+
+    def step():
+        hec.count(q, g, d_rows, d_cnt, d_sf)
+        st = hec.last_count_stats()
+        tup, mult = D.global_histogram(d_cnt, d_sf)
+        return st, tup, mult
+
+    def sync_all():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        stats, tup, mult = step()
+    # measured lookup ceiling at the same footprint and entry width as the largest field's table
+    regime = stats["regime"]
+    Mtop = q ** g - 1
+    ceil_entries = 3 * Mtop + 2 * min(32 * stats["chains_per_lane"], Mtop) * (2 * g + 2)
+    where = 0 if regime == hec.REGIME_SMEM else 1
+    gather_rate, _ = hec.gather_bench(where, max(ceil_entries, 1024), 2 if where == 0 else 4, 1024, 1, 4,
+                                      8192 if where == 0 else 1024)
+
+    sync_all()
+    launches0 = hec.launch_count()
+    kernel_ms, sq_ms = [], []
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    with ClockSampler(local_rank) as clocks:
+        ev0.record(stream)
+        for _ in range(args.steps):
+            stats, tup, mult = step()
+            kernel_ms.append(stats["count_kernel_ms"])
+            sq_ms.append(stats["squarefree_kernel_ms"])
+        ev1.record(stream)
+        sync_all()
+    launches = hec.launch_count() - launches0
+    elapsed_ms = ev0.elapsed_time(ev1)
+    t = torch.tensor([elapsed_ms], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    elapsed_ms = float(t.item())
+
+    # ---- end to end through the C ABI with HOST buffers (pinned), copies inside the timed region
+    h_rows = torch.from_numpy(rows.view(np.int16)).pin_memory()
+    h_cnt = torch.empty((n, g), dtype=torch.int32).pin_memory()
+    h_sf = torch.empty((n,), dtype=torch.uint8).pin_memory()
+    np_rows, np_cnt, np_sf = h_rows.numpy().view(np.uint16), h_cnt.numpy().view(np.uint32), h_sf.numpy()
+
+    def e2e_step():
+        hec.count(q, g, np_rows, np_cnt, np_sf)
+        return hec.histogram(np_cnt, np_sf)
+
+    e2e_step()
+    sync_all()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        e_tup, e_mult = e2e_step()
+    sync_all()
+    e2e_s = time.perf_counter() - t0
+    t = torch.tensor([e2e_s], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    e2e_s = float(t.item())
+    h2d = np_rows.nbytes + np_cnt.nbytes + np_sf.nbytes            # rows for hec_count; counts + mask for hec_histogram
+    d2h = np_cnt.nbytes + np_sf.nbytes + e_tup.nbytes + e_mult.nbytes
+
+    if rank != 0:
+        return
+    total_curves = n * world
+    value = total_curves * args.steps / (elapsed_ms * 1e-3)
+    k_ms = float(np.mean(kernel_ms))
+    achieved = lookups / (k_ms * 1e-3)
+    clk = clocks.summary()
+    sms = torch.cuda.get_device_properties(local_rank).multi_processor_count
+    mhz = clk["sm_mhz"] or clk["sm_max_mhz"] or 1965.0
+    conflict_free = sms * mhz * 1e6 * 32
+    peaks_file = ROOT / "MEASURED_PEAKS.json"
+    hbm_peak = json.loads(peaks_file.read_text())["hbm_gbs"] if peaks_file.exists() else 6650.0
+    hbm_bytes = rows.nbytes + n * g * 4 + n
+    roofline = {
+        "bound": "smem" if regime == hec.REGIME_SMEM else "l1/l2",
+        "kernel": "hec_count_kernel",
+        "achieved": achieved / 1e9, "peak": gather_rate / 1e9, "unit": "Glookups/s", "frac": achieved / gather_rate,
+        "peak_source": "measured in this run: hec_gather_bench, dependent random gathers, same footprint and entry width",
+        "peak_model": conflict_free / EXPECTED_WAVEFRONTS / 1e9 if regime == hec.REGIME_SMEM else None,
+        "peak_conflict_free": conflict_free / 1e9, "frac_conflict_free": achieved / conflict_free,
+        "lookups_per_launch": lookups, "kernel_ms": k_ms, "squarefree_kernel_ms": float(np.mean(sq_ms)),
+        "kernel_share_of_step": k_ms * args.steps / elapsed_ms,
+        "hbm": {"achieved_gbs": hbm_bytes / (k_ms * 1e-3) / 1e9, "peak_gbs": hbm_peak,
+                "frac": hbm_bytes / (k_ms * 1e-3) / 1e9 / hbm_peak, "algorithmic_bytes_per_launch": hbm_bytes},
+        "traffic": None,
+    }
+    line = {
+        "metric": "curves_per_s", "value": value, "unit": "curves/s", "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": elapsed_ms / args.steps, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "u32", "data": "synthetic",
+        "config": {"workload": cfg.name, "q": q, "g": g, "n_curves_per_gpu": n, "regime": {1: "smem", 2: "l2"}[regime],
+                   "grid": stats["grid"], "block": stats["block"], "smem_bytes": stats["smem_bytes"],
+                   "chains_per_lane": stats["chains_per_lane"], "parallelism": f"curve-sharded x{world}",
+                   "l2": f"inputs+outputs {hbm_bytes / 1e6:.0f} MB per step vs 126 MB L2: larger than L2"
+                         if hbm_bytes > 126e6 else "working set below L2 size; tables are on-chip by design"},
+        "xevals_per_s": value * cfg.xevals_per_curve,
+        "lookups_per_s": lookups * world * args.steps / (elapsed_ms * 1e-3),
+        "distinct_tuples": int(tup.shape[0]),
+        "clocks": clk,
+        "e2e": {"value": total_curves * args.steps / e2e_s, "unit": "curves/s", "h2d_bytes_per_step": h2d,
+                "d2h_bytes_per_step": d2h},
+        "gpu_launches": int(launches),
+        "roofline": roofline,
+    }
+    if world == 1 and not args.no_cpu_baseline:
+        S, dt, used, o_rows, o_cnt, o_sf = oracle_sample_run(cfg, args.cpu_seconds)
+        line["cpu_baseline"] = {"value": S / dt, "unit": "curves/s", "cores": used, "kind": "oracle",
+                                "sample": f"{S} curves: every {cfg.n // max(1, S)}-th row of {cfg.name}, {dt:.1f} s",
+                                "xevals_per_s": S / dt * cfg.xevals_per_curve}
+        # the sample doubles as a parity spot check of the timed configuration
+        idx = W.sample_indices(cfg, S, edge=0)
+        line["cpu_baseline"]["parity_rows_checked"] = int(len(idx))
+        line["cpu_baseline"]["parity_ok"] = bool(
+            (np_cnt[idx] == o_cnt).all() and (np_sf[idx] == o_sf).all())
+    print(json.dumps(line), flush=True)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=4, choices=sorted(W.CONFIGS))
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--regime", default="auto", choices=["auto", "smem", "l2"])
+    ap.add_argument("--cpu-seconds", type=float, default=15.0, help="CPU work of the cpu_baseline sample")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--curves", type=int, default=0,
+                    help="profiling only: first N curves of the workload (the line is then marked reduced and is not a bench value)")
+    args = ap.parse_args()
+    cfg = W.CONFIGS[args.config]
+    if args.curves:
+        import dataclasses
+        cfg = dataclasses.replace(cfg, n=min(args.curves, cfg.n), name=cfg.name + f"_REDUCED_first{args.curves}")
+    if args.impl == "reference":
+        run_reference(args, cfg)
+    else:
+        run_ours(args, cfg)
+    try:
+        import torch.distributed as dist
+        if dist.is_available() and dist.is_initialized():
+            dist.destroy_process_group()
+    except Exception:
+        pass
+
+
+if __name__ == "__main__":
+    main()

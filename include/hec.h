@@ -117,6 +117,16 @@ int hec_count(uint32_t q, uint32_t g, const uint16_t *coeffs, size_t n,
 int hec_histogram(const uint32_t *counts, const uint8_t *mask, size_t n, uint32_t g,
                   uint32_t *out_tuples, uint64_t *out_mult, size_t cap, size_t *out_m);
 
+/*
+ * hec_histogram_merge -- the one exchange step of the multi-GPU path: merges partial
+ * histograms.  in_tuples[n][g] with multiplicities in_mult[n] (tuples may repeat, e.g. the concatenation of
+ * several ranks' hec_histogram outputs; entries with multiplicity 0 are ignored) -> distinct tuples in
+ * ascending lexicographic order with summed multiplicities.  Same pointer, capacity and error rules as
+ * hec_histogram.
+ */
+int hec_histogram_merge(const uint32_t *in_tuples, const uint64_t *in_mult, size_t n, uint32_t g,
+                        uint32_t *out_tuples, uint64_t *out_mult, size_t cap, size_t *out_m);
+
 /* ------------------------------------------------------------------------------------------------
  * Execution control and instrumentation (used by the tests, bench.py and the ncu runs).
  */
@@ -150,8 +160,9 @@ uint64_t hec_launch_count(void);
 
 /*
  * Gather micro-benchmark for the lookup ceilings: every lane follows a dependent chain
- * idx <- table[idx] + lane-dependent offset through a table of `entries` uniformly random entries of
- * `entry_bytes` (2 or 4) bytes.  where = 0: shared memory; 1: global memory through L1 (ld.global.nc);
+ * idx <- table[idx] + warp-uniform offset + lane term (the count kernel's inner step) through a table of
+ * `entries` uniformly random entries of `entry_bytes` (2 or 4) bytes; with 2-byte entries and more than
+ * 65536 + 256 entries the uniform offset rotates so that the whole footprint is touched.  where = 0: shared memory; 1: global memory through L1 (ld.global.nc);
  * 2: global memory bypassing L1 (ld.global.cg).  Runs `lookups_per_lane` dependent lookups on each of
  * `chains` independent chains per lane with one CTA of `block` threads per SM times `ctas_per_sm`,
  * and writes lookups per second and the kernel time.  Table contents are seeded.

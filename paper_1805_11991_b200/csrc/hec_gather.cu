@@ -25,7 +25,7 @@ __device__ __forceinline__ uint32_t gather_load(const T *t, uint32_t idx) {
 }
 
 template <typename T, int WHERE, int U>
-__global__ void __launch_bounds__(1024) gather_kernel(const T *table, uint32_t entries, uint32_t steps, uint32_t *sink) {
+__global__ void __launch_bounds__(1024) gather_kernel(const T *table, uint32_t entries, uint32_t maxval, uint32_t steps, uint32_t *sink) {
     extern __shared__ uint4 gsm[];
     const T *tab = table;
     if constexpr (WHERE == 0) {
@@ -38,10 +38,15 @@ __global__ void __launch_bounds__(1024) gather_kernel(const T *table, uint32_t e
     const uint32_t lane = threadIdx.x & 31u;
     uint32_t v[U], l[U];
 #pragma unroll
-    for (int u = 0; u < U; u++) { l[u] = lane + 32u * u; v[u] = (threadIdx.x * 2654435761u + blockIdx.x * 40503u + u * 977u) % (entries - 256u); }
+    for (int u = 0; u < U; u++) { l[u] = lane + 32u * u; v[u] = (threadIdx.x * 2654435761u + blockIdx.x * 40503u + u * 977u) % maxval; }
+    // like the count kernel: index = looked-up value + warp-uniform offset + lane term
+    const uint32_t lim = entries - 256u - maxval + 1u;
+    uint32_t ub = 0;
     for (uint32_t s = 0; s < steps; s++) {
 #pragma unroll
-        for (int u = 0; u < U; u++) v[u] = gather_load<T, WHERE>(tab, v[u] + l[u]);
+        for (int u = 0; u < U; u++) v[u] = gather_load<T, WHERE>(tab, v[u] + ub + l[u]);
+        ub += 7919u;
+        if (ub >= lim) ub %= lim;
     }
     uint32_t acc = 0;
 #pragma unroll
@@ -50,11 +55,11 @@ __global__ void __launch_bounds__(1024) gather_kernel(const T *table, uint32_t e
 }
 
 template <typename T, int WHERE>
-int run_gather(const T *d_table, uint32_t entries, uint32_t block, uint32_t grid, uint32_t chains, uint32_t steps,
+int run_gather(const T *d_table, uint32_t entries, uint32_t maxval, uint32_t block, uint32_t grid, uint32_t chains, uint32_t steps,
                size_t smem, uint32_t *d_sink, cudaStream_t st) {
     auto launch = [&](auto kern) -> int {
         if (smem) HEC_CUDA_OK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        kern<<<grid, block, smem, st>>>(d_table, entries, steps, d_sink);
+        kern<<<grid, block, smem, st>>>(d_table, entries, maxval, steps, d_sink);
         hec_launch_counter::value++;
         HEC_CUDA_OK(cudaGetLastError());
         return HEC_OK;
@@ -75,7 +80,8 @@ int gather_typed(int where, uint32_t entries, uint32_t block, uint32_t ctas_per_
     int rc = hec_ensure_device(&sms, &optin);
     if (rc) return rc;
     cudaStream_t st = hec_current_stream();
-    // seeded table: values uniform in [0, entries - 256) so that value + lane term stays in range
+    // seeded table: values uniform in [0, maxval) so that value + uniform offset + lane term stays in range
+    const uint32_t maxval = (uint32_t)std::min<uint64_t>(entries - 256u, sizeof(T) == 2 ? 65536u : 0xFFFFFFFFu);
     std::vector<T> host(entries);
     uint64_t s = 0x1805119900000000ull + entries;
     for (uint32_t i = 0; i < entries; i++) {
@@ -84,7 +90,7 @@ int gather_typed(int where, uint32_t entries, uint32_t block, uint32_t ctas_per_
         z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9ull;
         z = (z ^ (z >> 27)) * 0x94D049BB133111EBull;
         z ^= z >> 31;
-        host[i] = (T)(((z >> 32) * (uint64_t)(entries - 256u)) >> 32);
+        host[i] = (T)(((z >> 32) * (uint64_t)maxval) >> 32);
     }
     const size_t bytes = ((size_t)entries * sizeof(T) + 15) & ~(size_t)15;
     size_t smem = 0;
@@ -103,9 +109,9 @@ int gather_typed(int where, uint32_t entries, uint32_t block, uint32_t ctas_per_
     HEC_CUDA_OK(cudaEventCreate(&e1));
     for (int rep = 0; rep < 2 && rc == HEC_OK; rep++) {         // rep 0 warms up
         HEC_CUDA_OK(cudaEventRecord(e0, st));
-        if (where == 0) rc = run_gather<T, 0>(d_table, entries, block, grid, chains, steps, smem, d_sink, st);
-        else if (where == 1) rc = run_gather<T, 1>(d_table, entries, block, grid, chains, steps, 0, d_sink, st);
-        else rc = run_gather<T, 2>(d_table, entries, block, grid, chains, steps, 0, d_sink, st);
+        if (where == 0) rc = run_gather<T, 0>(d_table, entries, maxval, block, grid, chains, steps, smem, d_sink, st);
+        else if (where == 1) rc = run_gather<T, 1>(d_table, entries, maxval, block, grid, chains, steps, 0, d_sink, st);
+        else rc = run_gather<T, 2>(d_table, entries, maxval, block, grid, chains, steps, 0, d_sink, st);
         HEC_CUDA_OK(cudaEventRecord(e1, st));
         HEC_CUDA_OK(cudaStreamSynchronize(st));
     }
@@ -130,7 +136,6 @@ extern "C" int hec_gather_bench(int where, uint32_t entries, uint32_t entry_byte
     if (block < 32 || block > 1024 || block % 32) HEC_FAIL(HEC_ERR_INVALID_ARG, "block must be a multiple of 32 in [32, 1024]");
     if (ctas_per_sm < 1 || ctas_per_sm > 32) HEC_FAIL(HEC_ERR_INVALID_ARG, "ctas_per_sm must be in [1, 32]");
     if (entry_bytes == 2) {
-        if (entries > 65536) HEC_FAIL(HEC_ERR_INVALID_ARG, "16-bit entries address at most 65536 entries");
         return gather_typed<uint16_t>(where, entries, block, ctas_per_sm, chains, lookups_per_lane, out_lookups_per_s, out_ms);
     }
     if (entry_bytes == 4)

@@ -15,7 +15,7 @@ bool hec_is_device_pointer(const void *p);
 namespace {
 
 constexpr unsigned long long kEmpty = ~0ull;
-constexpr int kSharedSlots = 4096;          // per-CTA table: 4096 x (8 B key + 4 B count) = 48 KB
+constexpr int kSharedSlots = 2048;          // per-CTA table: 2048 x (8 B key + 8 B count) = 32 KB
 constexpr int kSharedProbes = 8;
 
 struct PackSpec {
@@ -25,14 +25,15 @@ struct PackSpec {
     uint32_t bits[HEC_MAX_GENUS];
 };
 
-__global__ void hist_minmax_kernel(const uint32_t *counts, const uint8_t *mask, unsigned long long n, uint32_t g,
-                                   uint32_t *mn, uint32_t *mx, unsigned long long *rows) {
+__global__ void hist_minmax_kernel(const uint32_t *counts, const uint8_t *mask, const unsigned long long *weights,
+                                   unsigned long long n, uint32_t g, uint32_t *mn, uint32_t *mx, unsigned long long *rows) {
     uint32_t lmn[HEC_MAX_GENUS], lmx[HEC_MAX_GENUS];
     for (uint32_t k = 0; k < g; k++) { lmn[k] = 0xFFFFFFFFu; lmx[k] = 0; }
     unsigned long long cnt = 0;
     for (unsigned long long i = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; i < n;
          i += (unsigned long long)gridDim.x * blockDim.x) {
         if (mask && !mask[i]) continue;
+        if (weights && weights[i] == 0) continue;
         cnt++;
         for (uint32_t k = 0; k < g; k++) {
             const uint32_t v = counts[i * g + k];
@@ -64,26 +65,28 @@ __device__ __forceinline__ void global_insert(unsigned long long *gkeys, unsigne
     }
 }
 
-__global__ void __launch_bounds__(512) hist_insert_kernel(const uint32_t *counts, const uint8_t *mask, unsigned long long n,
-                                                          PackSpec S, unsigned long long *gkeys, unsigned long long *gcnt,
-                                                          unsigned long long capmask) {
+__global__ void __launch_bounds__(512) hist_insert_kernel(const uint32_t *counts, const uint8_t *mask, const unsigned long long *weights,
+                                                          unsigned long long n, PackSpec S, unsigned long long *gkeys,
+                                                          unsigned long long *gcnt, unsigned long long capmask) {
     __shared__ unsigned long long skeys[kSharedSlots];
-    __shared__ unsigned int scnt[kSharedSlots];
+    __shared__ unsigned long long scnt[kSharedSlots];
     for (int i = threadIdx.x; i < kSharedSlots; i += blockDim.x) { skeys[i] = kEmpty; scnt[i] = 0; }
     __syncthreads();
     for (unsigned long long i = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; i < n;
          i += (unsigned long long)gridDim.x * blockDim.x) {
         if (mask && !mask[i]) continue;
+        const unsigned long long w = weights ? weights[i] : 1ull;
+        if (w == 0) continue;
         unsigned long long key = 0;
         for (uint32_t k = 0; k < S.g; k++) key |= (unsigned long long)(counts[i * S.g + k] - S.mn[k]) << S.shift[k];
         uint32_t slot = (uint32_t)hash64(key) & (kSharedSlots - 1);
         bool done = false;
         for (int probe = 0; probe < kSharedProbes && !done; probe++) {
             const unsigned long long prev = atomicCAS(&skeys[slot], kEmpty, key);
-            if (prev == kEmpty || prev == key) { atomicAdd(&scnt[slot], 1u); done = true; }
+            if (prev == kEmpty || prev == key) { atomicAdd(&scnt[slot], w); done = true; }
             slot = (slot + 1) & (kSharedSlots - 1);
         }
-        if (!done) global_insert(gkeys, gcnt, capmask, key, 1ull);
+        if (!done) global_insert(gkeys, gcnt, capmask, key, w);
     }
     __syncthreads();
     for (int i = threadIdx.x; i < kSharedSlots; i += blockDim.x)
@@ -220,8 +223,8 @@ struct DeviceBuf {
 
 }  // namespace
 
-extern "C" int hec_histogram(const uint32_t *counts, const uint8_t *mask, size_t n, uint32_t g, uint32_t *out_tuples,
-                             uint64_t *out_mult, size_t cap, size_t *out_m) {
+static int histogram_impl(const uint32_t *counts, const uint8_t *mask, const uint64_t *weights, size_t n, uint32_t g,
+                          uint32_t *out_tuples, uint64_t *out_mult, size_t cap, size_t *out_m) {
     if (g < 1 || g > HEC_MAX_GENUS) HEC_FAIL(HEC_ERR_INVALID_ARG, "g must be in [1, HEC_MAX_GENUS]");
     if (!out_m) HEC_FAIL(HEC_ERR_INVALID_ARG, "out_m must not be NULL");
     *out_m = 0;
@@ -233,12 +236,13 @@ extern "C" int hec_histogram(const uint32_t *counts, const uint8_t *mask, size_t
     if (rc) return rc;
     cudaStream_t st = hec_current_stream();
     const bool dev = hec_is_device_pointer(counts);
-    if ((mask && hec_is_device_pointer(mask) != dev) || (cap > 0 && (hec_is_device_pointer(out_tuples) != dev || hec_is_device_pointer(out_mult) != dev)))
+    if ((mask && hec_is_device_pointer(mask) != dev) || (weights && hec_is_device_pointer(weights) != dev) || (cap > 0 && (hec_is_device_pointer(out_tuples) != dev || hec_is_device_pointer(out_mult) != dev)))
         HEC_FAIL(HEC_ERR_INVALID_ARG, "counts/mask/out_tuples/out_mult must all be host or all device pointers");
 
-    DeviceBuf in_counts, in_mask;
+    DeviceBuf in_counts, in_mask, in_w;
     const uint32_t *d_counts = counts;
     const uint8_t *d_mask = mask;
+    const unsigned long long *d_w = reinterpret_cast<const unsigned long long *>(weights);
     if (!dev) {
         if ((rc = in_counts.alloc(n * g * sizeof(uint32_t)))) return rc;
         HEC_CUDA_OK(cudaMemcpyAsync(in_counts.p, counts, n * g * sizeof(uint32_t), cudaMemcpyHostToDevice, st));
@@ -247,6 +251,11 @@ extern "C" int hec_histogram(const uint32_t *counts, const uint8_t *mask, size_t
             if ((rc = in_mask.alloc(n))) return rc;
             HEC_CUDA_OK(cudaMemcpyAsync(in_mask.p, mask, n, cudaMemcpyHostToDevice, st));
             d_mask = static_cast<const uint8_t *>(in_mask.p);
+        }
+        if (weights) {
+            if ((rc = in_w.alloc(n * 8))) return rc;
+            HEC_CUDA_OK(cudaMemcpyAsync(in_w.p, weights, n * 8, cudaMemcpyHostToDevice, st));
+            d_w = static_cast<const unsigned long long *>(in_w.p);
         }
     }
 
@@ -261,7 +270,7 @@ extern "C" int hec_histogram(const uint32_t *counts, const uint8_t *mask, size_t
     HEC_CUDA_OK(cudaMemcpyAsync(d_mn, h_init, sizeof h_init, cudaMemcpyHostToDevice, st));
     HEC_CUDA_OK(cudaMemcpyAsync(d_rows, h_zero, sizeof h_zero, cudaMemcpyHostToDevice, st));
     const unsigned grid = (unsigned)std::min<unsigned long long>((n + 511) / 512, (unsigned long long)sms * 4);
-    hist_minmax_kernel<<<grid, 512, 0, st>>>(d_counts, d_mask, n, g, d_mn, d_mx, d_rows);
+    hist_minmax_kernel<<<grid, 512, 0, st>>>(d_counts, d_mask, d_w, n, g, d_mn, d_mx, d_rows);
     hec_launch_counter::value++;
     uint32_t h_mm[16];
     unsigned long long h_rows = 0;
@@ -294,7 +303,7 @@ extern "C" int hec_histogram(const uint32_t *counts, const uint8_t *mask, size_t
     HEC_CUDA_OK(cudaMemsetAsync(gkeys.p, 0xFF, capslots * 8, st));
     HEC_CUDA_OK(cudaMemsetAsync(gcnt.p, 0, capslots * 8, st));
     hist_insert_kernel<<<(unsigned)std::min<unsigned long long>((n + 511) / 512, (unsigned long long)sms * 2), 512, 0, st>>>(
-        d_counts, d_mask, n, S, static_cast<unsigned long long *>(gkeys.p), static_cast<unsigned long long *>(gcnt.p), capslots - 1);
+        d_counts, d_mask, d_w, n, S, static_cast<unsigned long long *>(gkeys.p), static_cast<unsigned long long *>(gcnt.p), capslots - 1);
     hec_launch_counter::value++;
     HEC_CUDA_OK(cudaGetLastError());
 
@@ -349,4 +358,15 @@ extern "C" int hec_histogram(const uint32_t *counts, const uint8_t *mask, size_t
     }
     HEC_CUDA_OK(cudaStreamSynchronize(st));
     return HEC_OK;
+}
+
+extern "C" int hec_histogram(const uint32_t *counts, const uint8_t *mask, size_t n, uint32_t g, uint32_t *out_tuples,
+                             uint64_t *out_mult, size_t cap, size_t *out_m) {
+    return histogram_impl(counts, mask, nullptr, n, g, out_tuples, out_mult, cap, out_m);
+}
+
+extern "C" int hec_histogram_merge(const uint32_t *in_tuples, const uint64_t *in_mult, size_t n, uint32_t g,
+                                   uint32_t *out_tuples, uint64_t *out_mult, size_t cap, size_t *out_m) {
+    if (n > 0 && !in_mult) HEC_FAIL(HEC_ERR_INVALID_ARG, "in_mult must not be NULL");
+    return histogram_impl(in_tuples, nullptr, in_mult, n, g, out_tuples, out_mult, cap, out_m);
 }

@@ -29,6 +29,7 @@ SYMBOLS = [
     "hec_last_error", "hec_last_error_index", "hec_build_field", "hec_free_field", "hec_field_p",
     "hec_field_degree", "hec_field_q", "hec_field_Q", "hec_field_embed_unit", "hec_field_modulus",
     "hec_field_antilog", "hec_field_log", "hec_field_zech", "hec_field_embed", "hec_count", "hec_histogram",
+    "hec_histogram_merge",
     "hec_set_stream", "hec_set_regime", "hec_last_count_stats", "hec_launch_count", "hec_gather_bench",
     "hec_shutdown",
 ]
@@ -68,6 +69,7 @@ def lib():
             f.restype, f.argtypes = None, [vp, vp]
         L.hec_count.argtypes = [u32, u32, vp, sz, vp, vp]
         L.hec_histogram.argtypes = [vp, vp, sz, u32, vp, vp, sz, ctypes.POINTER(sz)]
+        L.hec_histogram_merge.argtypes = [vp, vp, sz, u32, vp, vp, sz, ctypes.POINTER(sz)]
         L.hec_set_stream.argtypes = [vp]
         L.hec_set_regime.argtypes = [ctypes.c_int]
         L.hec_last_count_stats.argtypes = [ctypes.POINTER(CountStats)]
@@ -185,12 +187,20 @@ def count(q: int, g: int, coeffs, out_counts=None, out_squarefree=None, want_squ
     return out_counts, out_squarefree
 
 
-def histogram(counts, mask=None):
+def histogram(counts, mask=None, _weights=None):
     """hec_histogram with the two-call pattern.  Returns (tuples [m][g], multiplicities [m])."""
     n, g = int(counts.shape[0]), int(counts.shape[1])
     L = lib()
     m = ctypes.c_size_t(0)
-    rc = L.hec_histogram(_ptr(counts), _ptr(mask), n, g, None, None, 0, ctypes.byref(m))
+    if not _is_torch(counts):
+        counts = np.ascontiguousarray(counts, dtype=np.uint32)
+    if _weights is not None:
+        def call(*a):
+            return L.hec_histogram_merge(_ptr(counts), _ptr(_weights), n, g, *a)
+    else:
+        def call(*a):
+            return L.hec_histogram(_ptr(counts), _ptr(mask), n, g, *a)
+    rc = call(None, None, 0, ctypes.byref(m))
     if rc not in (HEC_OK, HEC_ERR_CAPACITY):
         _check(rc)
     cap = m.value
@@ -199,12 +209,18 @@ def histogram(counts, mask=None):
         tup = torch.empty((cap, g), dtype=torch.int32, device=counts.device)
         mult = torch.empty((cap,), dtype=torch.int64, device=counts.device)
     else:
-        counts = np.ascontiguousarray(counts, dtype=np.uint32)
         tup = np.empty((cap, g), dtype=np.uint32)
         mult = np.empty((cap,), dtype=np.uint64)
     if cap:
-        _check(L.hec_histogram(_ptr(counts), _ptr(mask), n, g, _ptr(tup), _ptr(mult), cap, ctypes.byref(m)))
+        _check(call(_ptr(tup), _ptr(mult), cap, ctypes.byref(m)))
     return tup, mult
+
+
+def histogram_merge(tuples, mult):
+    """hec_histogram_merge: (tuples [n][g], mult [n]) with repeats -> sorted distinct tuples, summed mult."""
+    if not _is_torch(mult):
+        mult = np.ascontiguousarray(mult, dtype=np.uint64)
+    return histogram(tuples, None, _weights=mult)
 
 
 def last_count_stats() -> dict:
