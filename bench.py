@@ -172,7 +172,7 @@ def run_ours(args, cfg):
         dist.barrier()
     stream = torch.cuda.current_stream()
     hec.set_stream(stream.cuda_stream)
-    hec.set_regime({"auto": hec.REGIME_AUTO, "smem": hec.REGIME_SMEM, "l2": hec.REGIME_L2}[args.regime])
+    hec.set_regime({"auto": hec.REGIME_AUTO, "smem": hec.REGIME_SMEM, "l2": hec.REGIME_L2, "half": hec.REGIME_SMEM_HALF}[args.regime])
 
     rows = workload_rows(cfg, rank)
     n, g, q = rows.shape[0], cfg.g, cfg.q
@@ -195,12 +195,15 @@ def run_ours(args, cfg):
     for _ in range(args.warmup):
         stats, tup, mult = step()
     # measured lookup ceiling at the same footprint and entry width as the largest field's table
-    regime = stats["regime"]
+    regime, mode = stats["regime"], stats["table_mode"]
     Mtop = q ** g - 1
-    ceil_entries = 3 * Mtop + 2 * min(32 * stats["chains_per_lane"], Mtop) * (2 * g + 2)
-    where = 0 if regime == hec.REGIME_SMEM else 1
-    gather_rate, _ = hec.gather_bench(where, max(ceil_entries, 1024), 2 if where == 0 else 4, 1024, 1, 4,
+    ext_entries = 3 * Mtop + 2 * min(32 * stats["chains_per_lane"], Mtop) * (2 * g + 2)
+    # (where, entries, entry bytes) of the gather micro-benchmark that matches the largest field's table
+    where, ceil_entries, ceil_bytes = {0: (1, ext_entries, 4), 1: (0, ext_entries, 2),
+                                       2: (0, Mtop // 2 + 2, 4), 3: (0, Mtop // 2 + 2, 2)}[mode]
+    gather_rate, _ = hec.gather_bench(where, max(ceil_entries, 1024), ceil_bytes, 1024, 1, 4,
                                       8192 if where == 0 else 1024)
+    loads_per_lookup = 2 if mode == 3 else 1           # 16+8-bit planes: two shared-memory loads per Zech lookup
 
     sync_all()
     launches0 = hec.launch_count()
@@ -259,11 +262,12 @@ def run_ours(args, cfg):
     hbm_peak = json.loads(peaks_file.read_text())["hbm_gbs"] if peaks_file.exists() else 6650.0
     hbm_bytes = rows.nbytes + n * g * 4 + n
     roofline = {
-        "bound": "smem" if regime == hec.REGIME_SMEM else "l1/l2",
+        "bound": "smem" if mode != 0 else "l1/l2",
+        "table_layout": hec.TABLE_MODES[mode], "smem_loads_per_lookup": loads_per_lookup,
         "kernel": "hec_count_kernel",
         "achieved": achieved / 1e9, "peak": gather_rate / 1e9, "unit": "Glookups/s", "frac": achieved / gather_rate,
         "peak_source": "measured in this run: hec_gather_bench, dependent random gathers, same footprint and entry width",
-        "peak_model": conflict_free / EXPECTED_WAVEFRONTS / 1e9 if regime == hec.REGIME_SMEM else None,
+        "peak_model": conflict_free / EXPECTED_WAVEFRONTS / 1e9 if mode != 0 else None,
         "peak_conflict_free": conflict_free / 1e9, "frac_conflict_free": achieved / conflict_free,
         "lookups_per_launch": lookups, "kernel_ms": k_ms, "squarefree_kernel_ms": float(np.mean(sq_ms)),
         "kernel_share_of_step": k_ms * args.steps / elapsed_ms,
@@ -275,7 +279,8 @@ def run_ours(args, cfg):
         "metric": "curves_per_s", "value": value, "unit": "curves/s", "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": elapsed_ms / args.steps, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "u32", "data": "synthetic",
-        "config": {"workload": cfg.name, "q": q, "g": g, "n_curves_per_gpu": n, "regime": {1: "smem", 2: "l2"}[regime],
+        "config": {"workload": cfg.name, "q": q, "g": g, "n_curves_per_gpu": n, "regime": {1: "smem", 2: "l2", 3: "smem-half"}[regime],
+                   "table_layout": hec.TABLE_MODES[mode], "count_launches": stats["launches"] - 1,
                    "grid": stats["grid"], "block": stats["block"], "smem_bytes": stats["smem_bytes"],
                    "chains_per_lane": stats["chains_per_lane"], "parallelism": f"curve-sharded x{world}",
                    "l2": f"inputs+outputs {hbm_bytes / 1e6:.0f} MB per step vs 126 MB L2: larger than L2"
@@ -309,7 +314,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", type=int, default=4, choices=sorted(W.CONFIGS))
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--regime", default="auto", choices=["auto", "smem", "l2"])
+    ap.add_argument("--regime", default="auto", choices=["auto", "smem", "l2", "half"])
     ap.add_argument("--cpu-seconds", type=float, default=15.0, help="CPU work of the cpu_baseline sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--curves", type=int, default=0,

@@ -134,15 +134,23 @@ int hec_histogram_merge(const uint32_t *in_tuples, const uint64_t *in_mult, size
 int hec_set_stream(void *cuda_stream);
 
 typedef enum hec_regime {
-    HEC_REGIME_AUTO = 0,    /* shared-memory table when the extended Zech table of F_{q^k} fits, else L2 */
-    HEC_REGIME_SMEM = 1,    /* force shared memory (fails with HEC_ERR_INVALID_ARG when it cannot fit) */
-    HEC_REGIME_L2 = 2       /* force the L2-resident (global memory, 32-bit entries) table for the largest field */
+    HEC_REGIME_AUTO = 0,       /* per field: extended 16-bit table in shared memory if it fits, else a half table
+                                  (Z(-n) = Z(n) - n; 32-bit, else 16+8-bit planes) in shared memory if it fits,
+                                  else the L2-resident table */
+    HEC_REGIME_SMEM = 1,       /* force the extended shared-memory table for the largest field (HEC_ERR_INVALID_ARG
+                                  when it cannot fit) */
+    HEC_REGIME_L2 = 2,         /* force the L2-resident (global memory, 32-bit entries) table for the largest field */
+    HEC_REGIME_SMEM_HALF = 3   /* force the shared-memory half table for the largest field (HEC_ERR_INVALID_ARG when
+                                  it cannot fit or the field has fewer than 2^13 elements) */
 } hec_regime;
 int hec_set_regime(int regime);
 
-/* Statistics of the last hec_count on this thread's library state: device time of the count kernel and
- * of the squarefree kernel (CUDA events on the launch stream, ms), number of kernel launches, the regime
- * used for the largest field (hec_regime), dynamic shared memory bytes per CTA, grid and block size. */
+/* Statistics of the last hec_count on this thread's library state: device time of the count kernel(s) and
+ * of the squarefree kernel (CUDA events on the launch stream, ms), number of kernel launches (one count
+ * launch per group of fields whose tables share one shared-memory image, plus the squarefree kernel), the
+ * regime used for the largest field (hec_regime) and its table layout (0 global 32-bit extended, 1 shared
+ * 16-bit extended, 2 shared 32-bit half, 3 shared 16+8-bit half), the largest dynamic shared memory per
+ * CTA, grid and block size of the last count launch. */
 typedef struct hec_count_stats {
     float count_kernel_ms;
     float squarefree_kernel_ms;
@@ -152,6 +160,7 @@ typedef struct hec_count_stats {
     uint32_t grid;
     uint32_t block;
     uint32_t chains_per_lane;
+    uint32_t table_mode;
 } hec_count_stats;
 int hec_last_count_stats(hec_count_stats *out);
 

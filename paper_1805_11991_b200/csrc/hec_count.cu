@@ -24,62 +24,126 @@ namespace {
 constexpr int kThreads = 1024;
 constexpr int kWarps = kThreads / 32;
 
-struct SmemTable16 {
-    const uint16_t *t;
-    __device__ __forceinline__ uint32_t operator()(uint32_t idx) const { return t[idx]; }
-};
-struct GlobalTable32 {
-    const uint32_t *t;
-    __device__ __forceinline__ uint32_t operator()(uint32_t idx) const { return __ldg(t + idx); }
-};
-
 __device__ __forceinline__ uint32_t mod_once(uint32_t x, uint32_t M, uint32_t rcp) {
     // x mod M for any 32-bit x: the quotient estimate is at most one too small
     uint32_t r = x - __umulhi(x, rcp) * M;
     return r >= M ? r - M : r;
 }
 
-// All x in F_{q^k}^x for one curve: returns in (r0, rsq) this lane's share of
-//   r0 = #{x != 0 : f(x) = 0},  rsq = #{x != 0 : f(x) a nonzero square}        (reading G3)
+// ---------------------------------------------------------------------------------------------------------
+// Table policies.  A policy turns the chain state v and the per-lane offset u (= uniform part + lane term,
+// both in units of SC) into the next state with ONE pass through the Zech table; DESIGN.md "Table layouts".
+//
+// Extended tables (EXT16 in shared memory, GLOBAL32 in global memory): the state is the stored table value
+// (0 = "the element is zero", else OFF + W), the table is tabulated over idx in [0, 2 LMAX + M) so that
+// v + u never needs a reduction modulo M and the zero state maps to OFF (= log 1) by itself.
+template <typename T, bool kGlobal>
+struct ExtTable {
+    static constexpr uint32_t SC = 1;
+    const T *t;
+    uint32_t M, OFF;
+    __device__ __forceinline__ uint32_t init() const { return OFF; }                       // W_1 = log 1 = 0
+    __device__ __forceinline__ uint32_t ub_init(uint32_t delta) const { return delta; }    // delta in [0, M)
+    __device__ __forceinline__ uint32_t ub_next(uint32_t ub, uint32_t inc) const {
+        const uint32_t nx = ub + inc;
+        return nx >= M ? nx - M : nx;
+    }
+    __device__ __forceinline__ uint32_t step(uint32_t v, uint32_t u) const {
+        if constexpr (kGlobal) return (uint32_t)__ldg(t + (v + u));
+        else return (uint32_t)t[v + u];
+    }
+    __device__ __forceinline__ bool zero(uint32_t v) const { return v == 0u; }
+    __device__ __forceinline__ uint32_t odd(uint32_t v) const { return v & 1u; }           // OFF is even
+};
+
+// Half tables in shared memory, for fields whose extended table does not fit.  With h = M/2 and
+// Z(-n) = Z(n) - n (mod M) only Z(0..h) is stored.  All quantities are byte offsets (units of SC):
+//   x = v + u  is congruent to  n + h  with n the Zech argument;  v in [-hs, Ms), u in [-hs, hs + pad)
+//   y = x mod Ms        three candidates x + Ms, x, x - Ms, unsigned minimum (fused add+min, VIADDMNMX)
+//   b = min(y, Ms - y)  = SC (h - |d|), d = y/SC - h the signed residue of n nearest to 0; clamped to lims
+//   table[b] = SC (Z(h - b/SC) - h);   v' = table[b] + min(y, hs) = SC (Z(|d|) + min(d, 0)) = SC Z(n)
+// Zero handling without a branch: Z(h) (b = 0) is stored as a huge sentinel; a sentinel
+// state makes x, y and Ms - y huge, so b clamps to lims, whose entry -hs gives v' = -hs + hs = 0 = log 1.
+template <int BYTES>
+struct HalfTable {
+    static constexpr uint32_t SC = BYTES == 4 ? 4u : 2u;
+    const char *lo, *hi;
+    uint32_t M, Ms, hs, lims;
+    __device__ __forceinline__ uint32_t init() const { return 0u; }
+    __device__ __forceinline__ uint32_t ub_init(uint32_t delta) const {                    // (delta + h) mod M in [-h, h)
+        const uint32_t h = M >> 1;
+        uint32_t e = delta + h;
+        e = e >= M ? e - M : e;
+        const int32_t r = e >= h ? (int32_t)e - (int32_t)M : (int32_t)e;
+        return (uint32_t)(r * (int32_t)SC);
+    }
+    __device__ __forceinline__ uint32_t ub_next(uint32_t ub, uint32_t inc) const {
+        const int32_t nx = (int32_t)ub + (int32_t)inc;
+        return (uint32_t)(nx >= (int32_t)hs ? nx - (int32_t)Ms : nx);
+    }
+    __device__ __forceinline__ uint32_t step(uint32_t v, uint32_t u) const {
+        const uint32_t x = v + u;
+        const uint32_t y = min(min(x + Ms, x), x - Ms);
+        const uint32_t b = min(min(y, Ms - y), lims);
+        const uint32_t mn = min(y, hs);
+        if constexpr (BYTES == 4) {
+            return *reinterpret_cast<const uint32_t *>(lo + b) + mn;
+        } else {
+            const uint32_t l = *reinterpret_cast<const uint16_t *>(lo + b);
+            const int32_t h8 = *reinterpret_cast<const int8_t *>(hi + (b >> 1));
+            return l * 2u + mn + (uint32_t)(h8 * 131072);
+        }
+    }
+    __device__ __forceinline__ bool zero(uint32_t v) const { return (int32_t)v < -(1 << 22); }
+    __device__ __forceinline__ uint32_t odd(uint32_t v) const { return (v / SC) & 1u; }    // M is even
+};
+
+// All x in F_{q^k}^x for one curve: returns this lane's share of
+//   n_zero = #{x != 0 : f(x) = 0},  n_odd = #{x != 0 : f(x) != 0 and W_T odd}         (reading G3)
 // Per-term uniform state: ub[i] = (delta_i + m_i * base) mod M, advanced by inc[i] per batch of 32*U points.
-template <int D, int U, typename Table>
-__device__ __forceinline__ void horner_all_x(const Table tab, const uint32_t M, const uint32_t OFF,
-                                             const uint32_t lane, const uint32_t lane_cap,
-                                             uint32_t nzmask, uint32_t (&ub)[D], const uint32_t (&inc)[D],
+template <int D, int U, typename Pol>
+__device__ __forceinline__ void horner_all_x(const Pol pol, const uint32_t M, const uint32_t lane, const uint32_t lane_cap,
+                                             const uint32_t nzmask, const uint32_t (&delta)[D], const uint32_t (&incr)[D],
                                              const uint32_t (&gap)[D], uint32_t &n_odd, uint32_t &n_zero) {
-    uint32_t lterm[U];
+    uint32_t lterm[U], ub[D], inc[D];
 #pragma unroll
     for (int u = 0; u < U; u++) {
-        uint32_t l = lane + 32u * u;
-        lterm[u] = l < lane_cap ? l : 0u;
+        const uint32_t l = lane + 32u * u;
+        lterm[u] = (l < lane_cap ? l : 0u) * Pol::SC;
+    }
+#pragma unroll
+    for (int i = 0; i < D; i++) {
+        ub[i] = pol.ub_init(delta[i]);
+        inc[i] = incr[i] * Pol::SC;
     }
     n_odd = 0;
     n_zero = 0;
     for (uint32_t base = 0; base < M; base += 32u * U) {
         uint32_t v[U];
 #pragma unroll
-        for (int u = 0; u < U; u++) v[u] = OFF;                  // W_1 = log 1 = 0
+        for (int u = 0; u < U; u++) v[u] = pol.init();
 #pragma unroll
         for (int i = D - 1; i >= 0; i--) {
             if (nzmask & (1u << i)) {                             // warp-uniform: c_i != 0
                 const uint32_t ubi = ub[i];
                 const uint32_t m = gap[i];
 #pragma unroll
-                for (int u = 0; u < U; u++) v[u] = tab(v[u] + ubi + m * lterm[u]);
-                uint32_t nx = ubi + inc[i];
-                ub[i] = nx >= M ? nx - M : nx;
+                for (int u = 0; u < U; u++) v[u] = pol.step(v[u], ubi + m * lterm[u]);
+                ub[i] = pol.ub_next(ubi, inc[i]);
             }
         }
 #pragma unroll
         for (int u = 0; u < U; u++) {
             const bool valid = base + lane + 32u * u < M;
-            n_odd += valid ? (v[u] & 1u) : 0u;
-            n_zero += (valid && v[u] == 0u) ? 1u : 0u;
+            const bool z = pol.zero(v[u]);
+            n_odd += (valid && !z) ? pol.odd(v[u]) : 0u;
+            n_zero += (valid && z) ? 1u : 0u;
         }
     }
 }
 
-template <int G, int U>
+// One launch computes N_k for k_lo <= k <= k_hi.  Fields below k_hi use EXT16 tables; field k_hi uses TOP.
+template <int G, int U, int TOP>
 __global__ void __launch_bounds__(kThreads, 1) hec_count_kernel(const __grid_constant__ HecCountParams P) {
     constexpr int D = 2 * G + 2;          // largest degree; coefficient slots 0..D
     constexpr int NC = D + 1;
@@ -91,6 +155,7 @@ __global__ void __launch_bounds__(kThreads, 1) hec_count_kernel(const __grid_con
     const uint32_t lane = threadIdx.x & 31u;
     const uint32_t warp = threadIdx.x >> 5;
     const unsigned long long stride = (unsigned long long)gridDim.x * kWarps;
+    const char *smem = reinterpret_cast<const char *>(smem_blob);
 
     for (unsigned long long curve = (unsigned long long)blockIdx.x * kWarps + warp; curve < P.n; curve += stride) {
         // ---- a2: coefficient load (lane j holds c_j) and boundary checks (readings G13, hec.h)
@@ -98,9 +163,10 @@ __global__ void __launch_bounds__(kThreads, 1) hec_count_kernel(const __grid_con
         if (lane < NC) cj = P.coeffs[curve * NC + lane];
         const bool bad_range = __any_sync(0xffffffffu, cj >= P.q);
         const uint32_t top2 = __shfl_sync(0xffffffffu, cj, D) | __shfl_sync(0xffffffffu, cj, D - 1);
+        const bool mine = lane + 1 >= P.k_lo && lane + 1 <= P.k_hi;
         if (bad_range || top2 == 0) {
             if (lane == 0) atomicMin(&P.err[bad_range ? 0 : 1], curve);
-            if (lane < G) P.out[curve * G + lane] = 0;
+            if (mine) P.out[curve * G + lane] = 0;
             continue;
         }
         uint32_t c[NC];
@@ -109,24 +175,24 @@ __global__ void __launch_bounds__(kThreads, 1) hec_count_kernel(const __grid_con
 
         uint32_t my_count = 0;   // lane k-1 keeps N_k
 #pragma unroll 1
-        for (int k = 1; k <= G; k++) {
+        for (uint32_t k = P.k_lo; k <= P.k_hi; k++) {
             const HecFieldDev &F = P.f[k - 1];
-            const uint32_t M = F.M, OFF = F.off;
+            const uint32_t M = F.M;
             // embed: log of c_j in F_{q^k} (reading G6)
             const uint32_t lcj = (lane < NC && cj != 0) ? __ldg(F.emb + cj) : HEC_LOG_ZERO;
-            uint32_t ub[D], inc[D], gap[D];
+            uint32_t delta[D], incr[D], gap[D];
             uint32_t nzmask = 0, prev_lc = 0, prev_e = 0;
             bool started = false;
 #pragma unroll
             for (int i = D; i >= 0; i--) {
                 const uint32_t lci = __shfl_sync(0xffffffffu, lcj, i);
-                if (i < D) { ub[i] = 0; inc[i] = 0; gap[i] = 0; }
+                if (i < D) { delta[i] = 0; incr[i] = 0; gap[i] = 0; }
                 if (c[i] != 0) {
                     if (started && i < D) {
                         const uint32_t m = prev_e - (uint32_t)i;
                         gap[i] = m;
-                        ub[i] = prev_lc >= lci ? prev_lc - lci : prev_lc + M - lci;     // delta_i
-                        inc[i] = mod_once(m * (32u * U), M, F.rcpM);
+                        delta[i] = prev_lc >= lci ? prev_lc - lci : prev_lc + M - lci;
+                        incr[i] = mod_once(m * (32u * U), M, F.rcpM);
                         nzmask |= 1u << i;
                     }
                     started = true;
@@ -136,15 +202,21 @@ __global__ void __launch_bounds__(kThreads, 1) hec_count_kernel(const __grid_con
             }
             // ---- a3 + a4: Horner at every x != 0, classify, per-lane partial sums
             uint32_t n_odd, n_zero;
-            if (F.in_smem) {
-                SmemTable16 tab{reinterpret_cast<const uint16_t *>(reinterpret_cast<const char *>(smem_blob) + F.smem_off)};
-                horner_all_x<D, U>(tab, M, OFF, lane, F.lane_cap, nzmask, ub, inc, gap, n_odd, n_zero);
-            } else {
-                GlobalTable32 tab{F.gtab};
-                horner_all_x<D, U>(tab, M, OFF, lane, F.lane_cap, nzmask, ub, inc, gap, n_odd, n_zero);
+            if (TOP == HEC_TAB_EXT16 || k < P.k_hi) {
+                const ExtTable<uint16_t, false> pol{reinterpret_cast<const uint16_t *>(smem + F.smem_off), M, F.off};
+                horner_all_x<D, U>(pol, M, lane, F.lane_cap, nzmask, delta, incr, gap, n_odd, n_zero);
+            } else if constexpr (TOP == HEC_TAB_GLOBAL32) {
+                const ExtTable<uint32_t, true> pol{F.gtab, M, F.off};
+                horner_all_x<D, U>(pol, M, lane, F.lane_cap, nzmask, delta, incr, gap, n_odd, n_zero);
+            } else if constexpr (TOP == HEC_TAB_HALF32) {
+                const HalfTable<4> pol{smem + F.smem_off, nullptr, M, 4u * M, 2u * M, 4u * ((M >> 1) + 1u)};
+                horner_all_x<D, U>(pol, M, lane, F.lane_cap, nzmask, delta, incr, gap, n_odd, n_zero);
+            } else if constexpr (TOP == HEC_TAB_HALF24) {
+                const HalfTable<3> pol{smem + F.smem_off, smem + F.smem_off2, M, 2u * M, M, 2u * ((M >> 1) + 1u)};
+                horner_all_x<D, U>(pol, M, lane, F.lane_cap, nzmask, delta, incr, gap, n_odd, n_zero);
             }
             // f(x) = A_T x^{e_T}; log f = log c_{e_T} + W_T + e_T log x; a nonzero value is a square iff its log
-            // is even (reading G4; M and OFF are even).  log x = base + lane + 32u has the parity of the lane.
+            // is even (reading G4; M is even).  log x = base + lane + 32u has the parity of the lane.
             const uint32_t n_valid = (M + 31u - lane) >> 5;
             const uint32_t flip = (prev_lc ^ (prev_e & lane)) & 1u;
             const uint32_t rsq_lane = flip ? n_odd : n_valid - n_zero - n_odd;
@@ -156,9 +228,9 @@ __global__ void __launch_bounds__(kThreads, 1) hec_count_kernel(const __grid_con
             const uint32_t x0 = c[0] == 0 ? 1u : ((lc0 & 1u) ? 0u : 2u);
             const uint32_t inf = c[D] == 0 ? 1u : ((lcD & 1u) ? 0u : 2u);
             const uint32_t Nk = r0 + 2u * rsq + x0 + inf;
-            if ((int)lane == k - 1) my_count = Nk;
+            if (lane + 1 == k) my_count = Nk;
         }
-        if (lane < G) P.out[curve * G + lane] = my_count;
+        if (mine) P.out[curve * G + lane] = my_count;
     }
 }
 
@@ -239,15 +311,21 @@ __global__ void __launch_bounds__(256) hec_squarefree_kernel(const HecSquarefree
 // --------------------------------------------------------------------------------------------
 // host side: per-(q, g) device plan
 // --------------------------------------------------------------------------------------------
+struct LaunchPlan {
+    uint32_t k_lo = 1, k_hi = 1;
+    int top_mode = HEC_TAB_EXT16;
+    const uint4 *blob = nullptr;      // device image of this launch's shared-memory tables
+    uint32_t blob_bytes = 0;          // multiple of 16
+    uint32_t smem_bytes = 16;
+};
+
 struct DevicePlan {
     uint32_t q = 0, g = 0, p = 0, r = 0;
-    int regime = 0;               // regime actually used for the largest field
+    int top_mode = HEC_TAB_EXT16;     // table mode of the largest field
     int U = 4;
-    uint32_t smem_bytes = 0;
-    void *d_blob = nullptr;       // all device tables in one allocation
+    void *d_blob = nullptr;           // all device tables in one allocation
     HecFieldDev f[HEC_MAX_GENUS];
-    const uint4 *blob = nullptr;
-    uint32_t blob_bytes = 0;
+    std::vector<LaunchPlan> launches;
     // squarefree
     const uint32_t *sq_zech = nullptr, *sq_emb = nullptr;
     unsigned long long *d_err = nullptr;
@@ -311,6 +389,31 @@ void fill_extended(const hec_field &F, const hec_table_geom &t, T *out) {
     }
 }
 
+// Half table (kernel comment "Half tables"): entry b in [0, h] holds Z(h - b) - h, entry h + 1 holds -h
+// ("the accumulator was zero": the new relative log is log 1 = 0); Z(h) = "1 + alpha^h = 0" is the sentinel.
+uint32_t half_entries(uint32_t M) { return (M >> 1) + 2u; }
+void fill_half32(const hec_field &F, uint32_t M, int32_t *out) {
+    const uint32_t h = M >> 1;
+    for (uint32_t b = 0; b <= h; b++) {
+        const uint32_t z = F.zech[h - b];
+        out[b] = z == M ? INT32_MIN : 4 * ((int32_t)z - (int32_t)h);
+    }
+    out[h + 1] = -4 * (int32_t)h;
+}
+void fill_half24(const hec_field &F, uint32_t M, uint16_t *lo, int8_t *hi) {
+    const uint32_t h = M >> 1;
+    for (uint32_t b = 0; b <= h + 1; b++) {
+        const uint32_t z = b <= h ? F.zech[h - b] : 0u;
+        const int32_t w = (int32_t)z - (int32_t)h;
+        lo[b] = z == M ? 0 : (uint16_t)((uint32_t)w & 0xFFFFu);
+        hi[b] = z == M ? (int8_t)-128 : (int8_t)(w >> 16);
+    }
+}
+
+// Smallest field for which the half-table step is valid: the lane term must stay below h (kernel comment).
+constexpr uint32_t kHalfMinM = 1u << 13;
+constexpr uint32_t kHalf24MaxM = 1u << 22;      // |Z - h| < 127 * 65536
+
 int build_plan(LibState &S, uint32_t q, uint32_t g, int regime, DevicePlan **out) {
     auto key = std::make_tuple(q, g, regime);
     auto it = S.plans.find(key);
@@ -334,38 +437,100 @@ int build_plan(LibState &S, uint32_t q, uint32_t g, int regime, DevicePlan **out
         if (!fields[k - 1]) return HEC_ERR_INVALID_FIELD;
         geom[k - 1] = table_geom(fields[k - 1]->Q - 1, D, U);
     }
-    // which tables live in shared memory (16-bit stored values must fit)
-    std::vector<int> in_smem(g, 0);
-    uint32_t smem_used = 0;
-    for (uint32_t k = 1; k <= g; k++) {
+    // ---- table mode of every field and the grouping into launches (one shared-memory image per launch)
+    auto ext16_bytes = [&](uint32_t k) -> uint32_t {
         const hec_table_geom &t = geom[k - 1];
-        const bool fits16 = (uint64_t)t.lmax + t.M <= 65536u;
-        const uint32_t bytes = align16(t.entries * 2u);
-        const bool force_l2 = regime == HEC_REGIME_L2 && k == g;
-        if (fits16 && !force_l2 && smem_used + bytes <= budget) { in_smem[k - 1] = 1; smem_used += bytes; }
-    }
-    if (regime == HEC_REGIME_SMEM && !in_smem[g - 1])
-        HEC_FAIL(HEC_ERR_INVALID_ARG, "HEC_REGIME_SMEM: the extended Zech table of the largest field does not fit shared memory");
-    plan->regime = in_smem[g - 1] ? HEC_REGIME_SMEM : HEC_REGIME_L2;
-
-    // one device allocation: [smem blob][global 32-bit tables][embed tables][squarefree tables]
-    std::vector<uint8_t> host;
-    auto reserve = [&](size_t bytes) { size_t o = host.size(); host.resize(o + ((bytes + 255) & ~(size_t)255)); return o; };
-    const size_t blob_off = reserve(std::max<uint32_t>(smem_used, 16u));
-    std::vector<size_t> gtab_off(g, 0), emb_off(g, 0);
-    uint32_t so = 0;
+        if ((uint64_t)t.lmax + t.M > 65536u) return 0;               // stored values must fit 16 bits
+        const uint64_t b = (uint64_t)t.entries * 2u;
+        return b <= budget ? align16((uint32_t)b) : 0;
+    };
+    auto half_bytes = [&](uint32_t k, int mode) -> uint32_t {
+        const uint32_t M = geom[k - 1].M;
+        if (M < kHalfMinM || (mode == HEC_TAB_HALF24 && M >= kHalf24MaxM)) return 0;
+        const uint64_t e = half_entries(M);
+        const uint64_t b = mode == HEC_TAB_HALF32 ? e * 4u : (uint64_t)align16((uint32_t)(e * 2u)) + e;
+        return b <= budget ? align16((uint32_t)b) : 0;
+    };
+    std::vector<int> mode(g, HEC_TAB_EXT16);
+    std::vector<uint32_t> bytes(g, 0);
     for (uint32_t k = 1; k <= g; k++) {
-        const hec_table_geom &t = geom[k - 1];
-        HecFieldDev &fd = plan->f[k - 1];
-        fd.M = t.M; fd.off = t.lmax; fd.rcpM = (uint32_t)((1ull << 32) / t.M);
-        fd.in_smem = (uint32_t)in_smem[k - 1];
-        fd.lane_cap = std::min<uint32_t>(32u * U, t.M);
-        fd.smem_off = 0;
-        if (in_smem[k - 1]) {
-            fd.smem_off = so;
-            fill_extended<uint16_t>(*fields[k - 1], t, reinterpret_cast<uint16_t *>(host.data() + blob_off + so));
-            so += align16(t.entries * 2u);
+        const bool top = k == g;
+        int m = -1;
+        uint32_t b = 0;
+        auto try_mode = [&](int cand) {
+            if (m >= 0) return;
+            const uint32_t cb = cand == HEC_TAB_EXT16 ? ext16_bytes(k) : cand == HEC_TAB_GLOBAL32 ? 1u : half_bytes(k, cand);
+            if (cb) { m = cand; b = cand == HEC_TAB_GLOBAL32 ? 0u : cb; }
+        };
+        if (top && regime == HEC_REGIME_L2) {
+            try_mode(HEC_TAB_GLOBAL32);
+        } else if (top && regime == HEC_REGIME_SMEM) {
+            try_mode(HEC_TAB_EXT16);
+            if (m < 0) HEC_FAIL(HEC_ERR_INVALID_ARG, "HEC_REGIME_SMEM: the extended Zech table of the largest field does not fit shared memory");
+        } else if (top && regime == HEC_REGIME_SMEM_HALF) {
+            try_mode(HEC_TAB_HALF32);
+            try_mode(HEC_TAB_HALF24);
+            if (m < 0) HEC_FAIL(HEC_ERR_INVALID_ARG, "HEC_REGIME_SMEM_HALF: the half table of the largest field does not fit shared memory (or the field is below 2^13 elements)");
         } else {
+            try_mode(HEC_TAB_EXT16);
+            try_mode(HEC_TAB_HALF32);
+            try_mode(HEC_TAB_HALF24);
+            try_mode(HEC_TAB_GLOBAL32);
+        }
+        mode[k - 1] = m;
+        bytes[k - 1] = b;
+    }
+    plan->top_mode = mode[g - 1];
+    struct Group { uint32_t k_lo, k_hi, smem; };
+    std::vector<Group> groups;
+    {
+        Group cur{1, 0, 0};
+        for (uint32_t k = 1; k <= g; k++) {
+            if (cur.k_hi >= cur.k_lo && cur.smem + bytes[k - 1] > budget) { groups.push_back(cur); cur = Group{k, 0, 0}; }
+            cur.k_hi = k;
+            cur.smem += bytes[k - 1];
+            if (mode[k - 1] != HEC_TAB_EXT16) { groups.push_back(cur); cur = Group{k + 1, 0, 0}; }   // only the top of a launch may differ
+        }
+        if (cur.k_hi >= cur.k_lo) groups.push_back(cur);
+    }
+
+    // ---- one device allocation: [launch blobs][global 32-bit tables][embed tables][squarefree tables]
+    std::vector<uint8_t> host;
+    auto reserve = [&](size_t nbytes) { size_t o = host.size(); host.resize(o + ((nbytes + 255) & ~(size_t)255)); return o; };
+    std::vector<size_t> blob_off(groups.size()), gtab_off(g, 0), emb_off(g, 0);
+    for (size_t gi = 0; gi < groups.size(); gi++) {
+        const Group &G = groups[gi];
+        blob_off[gi] = reserve(std::max<uint32_t>(G.smem, 16u));
+        uint32_t so = 0;
+        for (uint32_t k = G.k_lo; k <= G.k_hi; k++) {
+            const hec_table_geom &t = geom[k - 1];
+            HecFieldDev &fd = plan->f[k - 1];
+            fd.M = t.M; fd.mode = (uint32_t)mode[k - 1]; fd.off = t.lmax; fd.rcpM = (uint32_t)((1ull << 32) / t.M);
+            fd.lane_cap = std::min<uint32_t>(32u * U, t.M);
+            fd.smem_off = so; fd.smem_off2 = 0; fd.pad_ = 0; fd.gtab = nullptr;
+            uint8_t *dst = host.data() + blob_off[gi] + so;
+            switch (mode[k - 1]) {
+                case HEC_TAB_EXT16:
+                    fill_extended<uint16_t>(*fields[k - 1], t, reinterpret_cast<uint16_t *>(dst));
+                    break;
+                case HEC_TAB_HALF32:
+                    fill_half32(*fields[k - 1], t.M, reinterpret_cast<int32_t *>(dst));
+                    break;
+                case HEC_TAB_HALF24: {
+                    const uint32_t lo_bytes = align16(half_entries(t.M) * 2u);
+                    fd.smem_off2 = so + lo_bytes;
+                    fill_half24(*fields[k - 1], t.M, reinterpret_cast<uint16_t *>(dst), reinterpret_cast<int8_t *>(dst + lo_bytes));
+                    break;
+                }
+                default:
+                    break;
+            }
+            so += bytes[k - 1];
+        }
+    }
+    for (uint32_t k = 1; k <= g; k++) {
+        const hec_table_geom &t = geom[k - 1];
+        if (mode[k - 1] == HEC_TAB_GLOBAL32) {
             gtab_off[k - 1] = reserve((size_t)t.entries * 4u);
             fill_extended<uint32_t>(*fields[k - 1], t, reinterpret_cast<uint32_t *>(host.data() + gtab_off[k - 1]));
         }
@@ -380,11 +545,17 @@ int build_plan(LibState &S, uint32_t q, uint32_t g, int regime, DevicePlan **out
     HEC_CUDA_OK(cudaMemcpy(plan->d_blob, host.data(), host.size(), cudaMemcpyHostToDevice));
     HEC_CUDA_OK(cudaMalloc((void **)&plan->d_err, 2 * sizeof(unsigned long long)));
     const uint8_t *base = static_cast<const uint8_t *>(plan->d_blob);
-    plan->blob = reinterpret_cast<const uint4 *>(base + blob_off);
-    plan->blob_bytes = align16(smem_used);
-    plan->smem_bytes = std::max<uint32_t>(align16(smem_used), 16u);
+    for (size_t gi = 0; gi < groups.size(); gi++) {
+        LaunchPlan L;
+        L.k_lo = groups[gi].k_lo; L.k_hi = groups[gi].k_hi;
+        L.top_mode = mode[L.k_hi - 1];
+        L.blob = reinterpret_cast<const uint4 *>(base + blob_off[gi]);
+        L.blob_bytes = align16(groups[gi].smem);
+        L.smem_bytes = std::max<uint32_t>(L.blob_bytes, 16u);
+        plan->launches.push_back(L);
+    }
     for (uint32_t k = 1; k <= g; k++) {
-        plan->f[k - 1].gtab = in_smem[k - 1] ? nullptr : reinterpret_cast<const uint32_t *>(base + gtab_off[k - 1]);
+        plan->f[k - 1].gtab = mode[k - 1] == HEC_TAB_GLOBAL32 ? reinterpret_cast<const uint32_t *>(base + gtab_off[k - 1]) : nullptr;
         plan->f[k - 1].emb = reinterpret_cast<const uint32_t *>(base + emb_off[k - 1]);
     }
     plan->sq_zech = reinterpret_cast<const uint32_t *>(base + sqz_off);
@@ -395,19 +566,36 @@ int build_plan(LibState &S, uint32_t q, uint32_t g, int regime, DevicePlan **out
     return HEC_OK;
 }
 
-template <int G, int U>
-int launch_count(LibState &S, const DevicePlan &plan, const HecCountParams &P) {
-    auto kern = hec_count_kernel<G, U>;
-    HEC_CUDA_OK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)plan.smem_bytes));
-    const unsigned long long warps_needed = (P.n + 0ull);
-    uint32_t grid = (uint32_t)std::min<unsigned long long>((warps_needed + kWarps - 1) / kWarps, (unsigned long long)S.sm_count);
+template <int G, int U, int TOP>
+int launch_one(LibState &S, const LaunchPlan &L, const HecCountParams &P) {
+    auto kern = hec_count_kernel<G, U, TOP>;
+    HEC_CUDA_OK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)L.smem_bytes));
+    uint32_t grid = (uint32_t)std::min<unsigned long long>((P.n + kWarps - 1) / kWarps, (unsigned long long)S.sm_count);
     if (grid == 0) grid = 1;
-    kern<<<grid, kThreads, plan.smem_bytes, S.stream>>>(P);
+    kern<<<grid, kThreads, L.smem_bytes, S.stream>>>(P);
     hec_launch_counter::value++;
     S.stats.grid = grid;
     S.stats.block = kThreads;
     S.stats.chains_per_lane = U;
+    S.stats.smem_bytes = std::max(S.stats.smem_bytes, L.smem_bytes);
+    S.stats.launches++;
     HEC_CUDA_OK(cudaGetLastError());
+    return HEC_OK;
+}
+
+template <int G, int U>
+int launch_count(LibState &S, const DevicePlan &plan, HecCountParams P) {
+    for (const LaunchPlan &L : plan.launches) {
+        P.blob = L.blob; P.blob_bytes = L.blob_bytes; P.k_lo = L.k_lo; P.k_hi = L.k_hi;
+        int rc;
+        switch (L.top_mode) {
+            case HEC_TAB_GLOBAL32: rc = launch_one<G, U, HEC_TAB_GLOBAL32>(S, L, P); break;
+            case HEC_TAB_HALF32: rc = launch_one<G, U, HEC_TAB_HALF32>(S, L, P); break;
+            case HEC_TAB_HALF24: rc = launch_one<G, U, HEC_TAB_HALF24>(S, L, P); break;
+            default: rc = launch_one<G, U, HEC_TAB_EXT16>(S, L, P); break;
+        }
+        if (rc) return rc;
+    }
     return HEC_OK;
 }
 
@@ -440,7 +628,7 @@ int hec_set_stream(void *cuda_stream) {
 }
 
 int hec_set_regime(int regime) {
-    if (regime < HEC_REGIME_AUTO || regime > HEC_REGIME_L2) HEC_FAIL(HEC_ERR_INVALID_ARG, "unknown regime");
+    if (regime < HEC_REGIME_AUTO || regime > HEC_REGIME_SMEM_HALF) HEC_FAIL(HEC_ERR_INVALID_ARG, "unknown regime");
     std::lock_guard<std::mutex> lock(g_state.mu);
     g_state.regime = regime;
     return HEC_OK;
@@ -504,12 +692,12 @@ int hec_count(uint32_t q, uint32_t g, const uint16_t *coeffs, size_t n, uint32_t
 
     HecCountParams P;
     P.coeffs = d_coeffs; P.out = d_counts; P.n = n; P.q = q;
-    P.blob = plan->blob; P.blob_bytes = plan->blob_bytes; P.err = plan->d_err;
+    P.blob = nullptr; P.blob_bytes = 0; P.err = plan->d_err; P.k_lo = 1; P.k_hi = g;
     for (uint32_t k = 0; k < HEC_MAX_GENUS; k++) P.f[k] = plan->f[k < g ? k : 0];
 
     S.stats = hec_count_stats{};
-    S.stats.regime = (uint32_t)plan->regime;
-    S.stats.smem_bytes = plan->smem_bytes;
+    S.stats.table_mode = (uint32_t)plan->top_mode;
+    S.stats.regime = plan->top_mode == HEC_TAB_EXT16 ? HEC_REGIME_SMEM : plan->top_mode == HEC_TAB_GLOBAL32 ? HEC_REGIME_L2 : HEC_REGIME_SMEM_HALF;
     HEC_CUDA_OK(cudaEventRecord(S.ev[0], S.stream));
     switch (g) {
         case 1: rc = launch_count<1, 4>(S, *plan, P); break;
@@ -520,7 +708,6 @@ int hec_count(uint32_t q, uint32_t g, const uint16_t *coeffs, size_t n, uint32_t
     }
     if (rc) return rc;
     HEC_CUDA_OK(cudaEventRecord(S.ev[1], S.stream));
-    S.stats.launches = 1;
     if (d_sf) {
         HecSquarefreeParams Q;
         Q.coeffs = d_coeffs; Q.out = d_sf; Q.n = n; Q.p = p; Q.q = q; Q.M = q - 1; Q.ncoef = (uint32_t)ncoef;
@@ -528,7 +715,7 @@ int hec_count(uint32_t q, uint32_t g, const uint16_t *coeffs, size_t n, uint32_t
         const unsigned long long blocks = (n + 255) / 256;
         hec_squarefree_kernel<<<(unsigned)blocks, 256, 0, S.stream>>>(Q);
         hec_launch_counter::value++;
-        S.stats.launches = 2;
+        S.stats.launches++;
         HEC_CUDA_OK(cudaGetLastError());
     }
     HEC_CUDA_OK(cudaEventRecord(S.ev[2], S.stream));

@@ -17,15 +17,25 @@
 
 constexpr uint32_t HEC_LOG_ZERO = 0xFFFFFFFFu;   // embed table entry of the zero coefficient (device side)
 
-// One field F_{q^k} as the count kernel sees it (DESIGN.md "Table layout").
+// How the Zech table of one field is stored for the count kernel.
+enum HecTableMode : uint32_t {
+    HEC_TAB_GLOBAL32 = 0,   // extended table, 32-bit entries, global memory (L1/L2-resident regime)
+    HEC_TAB_EXT16 = 1,      // extended table, 16-bit entries, shared memory
+    HEC_TAB_HALF32 = 2,     // half table (Z(-n) = Z(n) - n), 32-bit entries, shared memory
+    HEC_TAB_HALF24 = 3      // half table, 16-bit low plane + signed 8-bit high plane, shared memory
+};
+
+// One field F_{q^k} as the count kernel sees it.
 struct HecFieldDev {
     uint32_t M;          // q^k - 1
-    uint32_t off;        // OFF = LMAX = M + PADL (even)
+    uint32_t mode;       // HecTableMode
+    uint32_t off;        // extended tables: OFF = LMAX = M + PADL (even)
     uint32_t rcpM;       // floor(2^32 / M), for x mod M with one correction step
-    uint32_t in_smem;    // 1: 16-bit table in the shared-memory blob at smem_off; 0: 32-bit table gtab
-    uint32_t smem_off;   // byte offset inside the blob (16-byte aligned)
+    uint32_t smem_off;   // byte offset inside the launch's blob (16-byte aligned): table / low plane
+    uint32_t smem_off2;  // HALF24: byte offset of the high plane
     uint32_t lane_cap;   // lanes with lane + 32u >= lane_cap use lane term 0 (they are masked out anyway)
-    const uint32_t *gtab;   // extended table, 32-bit entries, global memory (L2-resident regime)
+    uint32_t pad_;
+    const uint32_t *gtab;   // GLOBAL32: extended table in global memory
     const uint32_t *emb;    // q entries: log in F_{q^k} of the embedded coefficient, HEC_LOG_ZERO for 0
 };
 
@@ -35,8 +45,9 @@ struct HecCountParams {
     unsigned long long n;
     uint32_t q;
     uint32_t blob_bytes;           // multiple of 16
-    const uint4 *blob;             // concatenated shared-memory tables
+    const uint4 *blob;             // this launch's concatenated shared-memory tables
     unsigned long long *err;       // err[0] = first row with a coefficient >= q, err[1] = first row of degree < 2g+1
+    uint32_t k_lo, k_hi;           // this launch computes N_k for k_lo <= k <= k_hi; only field k_hi may be non-EXT16
     HecFieldDev f[HEC_MAX_GENUS];
 };
 

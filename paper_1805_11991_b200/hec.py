@@ -21,7 +21,8 @@ _lib = None
 HEC_OK = 0
 HEC_ERR_INVALID_FIELD, HEC_ERR_INVALID_ARG, HEC_ERR_COEFF_RANGE, HEC_ERR_DEGREE = -1, -2, -3, -4
 HEC_ERR_CAPACITY, HEC_ERR_UNSUPPORTED, HEC_ERR_CUDA, HEC_ERR_NOMEM = -5, -6, -7, -8
-REGIME_AUTO, REGIME_SMEM, REGIME_L2 = 0, 1, 2
+REGIME_AUTO, REGIME_SMEM, REGIME_L2, REGIME_SMEM_HALF = 0, 1, 2, 3
+TABLE_MODES = {0: "global32-extended", 1: "smem16-extended", 2: "smem32-half", 3: "smem16+8-half"}
 MAX_GENUS = 5
 
 # every symbol include/hec.h declares (tests check the library exports all of them)
@@ -44,7 +45,8 @@ class HecError(RuntimeError):
 class CountStats(ctypes.Structure):
     _fields_ = [("count_kernel_ms", ctypes.c_float), ("squarefree_kernel_ms", ctypes.c_float),
                 ("launches", ctypes.c_uint32), ("regime", ctypes.c_uint32), ("smem_bytes", ctypes.c_uint32),
-                ("grid", ctypes.c_uint32), ("block", ctypes.c_uint32), ("chains_per_lane", ctypes.c_uint32)]
+                ("grid", ctypes.c_uint32), ("block", ctypes.c_uint32), ("chains_per_lane", ctypes.c_uint32),
+                ("table_mode", ctypes.c_uint32)]
 
 
 def lib():

@@ -110,23 +110,62 @@ def test_sparse_and_zero_heavy_rows(torch_cuda):
 
 
 def test_regimes_agree(torch_cuda):
-    """The L2-resident (global, 32-bit) table and the shared-memory (16-bit) table give identical counts."""
+    """Every table layout gives identical counts: extended 16-bit shared-memory table, L2-resident 32-bit
+    table, shared-memory half table (32-bit for q=13^4 and 293^2, 16+8-bit planes for 49^3)."""
+    modes = {hec.REGIME_SMEM: 1, hec.REGIME_L2: 0}
     try:
-        for cid, n in [(2, 3000), (4, 600)]:
+        for cid, n, regimes, half_mode in [(2, 3000, (hec.REGIME_SMEM, hec.REGIME_L2), None),
+                                           (4, 600, (hec.REGIME_SMEM, hec.REGIME_L2, hec.REGIME_SMEM_HALF), 2),
+                                           (5, 300, (hec.REGIME_L2, hec.REGIME_SMEM_HALF, hec.REGIME_AUTO), 2),
+                                           (3, 200, (hec.REGIME_L2, hec.REGIME_SMEM_HALF, hec.REGIME_AUTO), 3)]:
             cfg = W.CONFIGS[cid]
-            rows = W.generate(cfg, 5000, n)
-            hec.set_regime(hec.REGIME_SMEM)
-            a, sa = _gpu_count(torch_cuda, cfg.q, cfg.g, rows)
-            assert hec.last_count_stats()["regime"] == hec.REGIME_SMEM
-            hec.set_regime(hec.REGIME_L2)
-            b, sb = _gpu_count(torch_cuda, cfg.q, cfg.g, rows)
-            assert hec.last_count_stats()["regime"] == hec.REGIME_L2
-            assert (a == b).all() and (sa == sb).all()
-        hec.set_regime(hec.REGIME_SMEM)
-        with pytest.raises(hec.HecError):
-            _gpu_count(torch_cuda, 293, 2, W.generate(W.CONFIGS[5], 0, 8))
+            rows = np.concatenate([W.generate(cfg, 5000, n), W.edge_rows(cfg.q, cfg.g)])
+            ref = None
+            for regime in regimes:
+                hec.set_regime(regime)
+                a, sa = _gpu_count(torch_cuda, cfg.q, cfg.g, rows)
+                st = hec.last_count_stats()
+                if regime == hec.REGIME_AUTO:
+                    assert st["regime"] == hec.REGIME_SMEM_HALF and st["table_mode"] == half_mode
+                else:
+                    assert st["regime"] == regime
+                    assert st["table_mode"] == (half_mode if regime == hec.REGIME_SMEM_HALF else modes[regime])
+                if ref is None:
+                    ref = (a, sa)
+                assert (a == ref[0]).all() and (sa == ref[1]).all(), (cid, regime)
+        for regime, cid in [(hec.REGIME_SMEM, 5), (hec.REGIME_SMEM_HALF, 2)]:
+            hec.set_regime(regime)
+            with pytest.raises(hec.HecError):
+                _gpu_count(torch_cuda, W.CONFIGS[cid].q, W.CONFIGS[cid].g, W.generate(W.CONFIGS[cid], 0, 8))
     finally:
         hec.set_regime(hec.REGIME_AUTO)
+
+
+@pytest.mark.parametrize("q,g,mode,min_launches", [(17, 4, 2, 2), (19, 4, 3, 3), (9, 5, 2, 2), (11, 5, 0, 2)])
+def test_mixed_layout_launch_groups(torch_cuda, q, g, mode, min_launches):
+    """Fields that need different layouts in one call (17^4 = 83521 and 9^5 = 59049: 32-bit half table next
+    to the lower fields' extended tables; 19^4 = 130321: 16+8-bit half table in a launch of its own;
+    11^5 = 161051: nothing fits, L2-resident).  Oracle on the fields k <= 3 and on a few rows of k = 4; the
+    forced L2 regime must agree on everything."""
+    rng = np.random.default_rng(q)
+    rows = rng.integers(0, q, size=(70, 2 * g + 3)).astype(np.uint16)
+    rows[:, -1] = np.where(rng.random(70) < 0.5, rng.integers(1, q, 70), 0)
+    rows[:, -2] = np.where(rows[:, -1] == 0, rng.integers(1, q, 70), rows[:, -2])
+    rows = np.concatenate([rows, W.edge_rows(q, g)[:12]])
+    try:
+        hec.set_regime(hec.REGIME_AUTO)
+        a, sa = _gpu_count(torch_cuda, q, g, rows)
+        st = hec.last_count_stats()
+        assert st["launches"] >= min_launches and st["table_mode"] == mode, st
+        hec.set_regime(hec.REGIME_L2)
+        b, sb = _gpu_count(torch_cuda, q, g, rows)
+        assert (a == b).all() and (sa == sb).all()
+    finally:
+        hec.set_regime(hec.REGIME_AUTO)
+    ocnt, osf, _ = O.count(q, g, rows, k_hi=3)
+    assert (a[:, :3] == ocnt[:, :3]).all() and (sa == osf).all()
+    otop, _, _ = O.count(q, g, rows[:3], k_lo=4, k_hi=4, want_squarefree=False)
+    assert (a[:3, 3] == otop[:, 3]).all()
 
 
 # ------------------------------------------------------------------------------------------ boundary behaviour
@@ -227,3 +266,13 @@ def test_full_config2(torch_cuda):
 def test_full_config4_headline(torch_cuda):
     stats = _full_size_checks(torch_cuda, 4, 96)
     assert stats["regime"] == hec.REGIME_SMEM
+
+
+def test_full_config5_half_table(torch_cuda):
+    stats = _full_size_checks(torch_cuda, 5, 64)
+    assert stats["regime"] == hec.REGIME_SMEM_HALF and stats["table_mode"] == 2
+
+
+def test_full_config3_half_planes(torch_cuda):
+    stats = _full_size_checks(torch_cuda, 3, 16)
+    assert stats["regime"] == hec.REGIME_SMEM_HALF and stats["table_mode"] == 3
