@@ -145,12 +145,22 @@ typedef enum hec_regime {
 } hec_regime;
 int hec_set_regime(int regime);
 
+/* Evaluation scheme of hec_count (results are identical; f is evaluated at every x either way). */
+typedef enum hec_eval {
+    HEC_EVAL_AUTO = 0,         /* fields with 4 | q^k - 1 whose table is an extended one: radix-4 split, f(X) = sum_r X^r F_r(X^4):
+                                  the four points x, ix, -x, -ix of a coset share the four Horner chains F_r(x^4) and are
+                                  combined by a butterfly of Zech additions (about 2.5x fewer lookups at degree 10);
+                                  all other fields: HEC_EVAL_HORNER */
+    HEC_EVAL_HORNER = 1        /* the paper's scheme (Algorithm 1 line 8): one Horner chain per x */
+} hec_eval;
+int hec_set_eval(int eval);
+
 /* Statistics of the last hec_count on this thread's library state: device time of the count kernel(s) and
  * of the squarefree kernel (CUDA events on the launch stream, ms), number of kernel launches (one count
  * launch per group of fields whose tables share one shared-memory image, plus the squarefree kernel), the
  * regime used for the largest field (hec_regime) and its table layout (0 global 32-bit extended, 1 shared
  * 16-bit extended, 2 shared 32-bit half, 3 shared 16+8-bit half), the largest dynamic shared memory per
- * CTA, grid and block size of the last count launch. */
+ * CTA, grid and block size of the last count launch, and which fields used the radix-4 split. */
 typedef struct hec_count_stats {
     float count_kernel_ms;
     float squarefree_kernel_ms;
@@ -161,6 +171,7 @@ typedef struct hec_count_stats {
     uint32_t block;
     uint32_t chains_per_lane;
     uint32_t table_mode;
+    uint32_t radix4_fields;    /* bit k-1 set: N_k was computed with the radix-4 split */
 } hec_count_stats;
 int hec_last_count_stats(hec_count_stats *out);
 

@@ -34,26 +34,50 @@ __device__ __forceinline__ uint32_t mod_once(uint32_t x, uint32_t M, uint32_t rc
 // Table policies.  A policy turns the chain state v and the per-lane offset u (= uniform part + lane term,
 // both in units of SC) into the next state with ONE pass through the Zech table; DESIGN.md "Table layouts".
 //
-// Extended tables (EXT16 in shared memory, GLOBAL32 in global memory): the state is the stored table value
-// (0 = "the element is zero", else OFF + W), the table is tabulated over idx in [0, 2 LMAX + M) so that
-// v + u never needs a reduction modulo M and the zero state maps to OFF (= log 1) by itself.
-template <typename T, bool kGlobal>
-struct ExtTable {
+// Extended tables (EXT16 in shared memory, GLOBAL32 in global memory): the state is the stored table value,
+// a log W in [0, M) or Z0 = M + LP ("the element is zero"), LP = M + PADL.  The table is tabulated over
+// idx = v + u, u in [0, LP):  idx in [0, M + LP) -> Zech of idx mod M (Z0 where 1 + alpha^idx = 0);
+// idx in [Z0, Z0 + LP) -> 0 (the accumulator was zero: acc x^m + c = c, W = log 1 = 0).  So v + u never
+// needs a reduction modulo M and the zero state is absorbed by the table itself.
+__device__ __forceinline__ uint32_t lds_u16(uint32_t addr) {
+    uint16_t r;
+    asm("ld.shared.u16 %0, [%1];" : "=h"(r) : "r"(addr));
+    return r;
+}
+
+// EXT16: 16-bit entries in shared memory.  Offsets are in bytes (SC = 2) and carry the table's shared-memory
+// address, so a chain step is one shift-add and one LDS.
+struct ExtTableS16 {
+    static constexpr uint32_t SC = 2;
+    uint32_t tb;          // shared-memory byte address of entry 0
+    uint32_t M, Z0;
+    __device__ __forceinline__ uint32_t init() const { return 0u; }                        // W_1 = log 1 = 0
+    __device__ __forceinline__ uint32_t ub_init(uint32_t delta) const { return tb + 2u * delta; }
+    __device__ __forceinline__ uint32_t ub_next(uint32_t ub, uint32_t inc) const {         // inc = 2 * (increment mod M)
+        const uint32_t nx = ub + inc;
+        return nx >= tb + 2u * M ? nx - 2u * M : nx;
+    }
+    __device__ __forceinline__ uint32_t step(uint32_t v, uint32_t u) const { return lds_u16(2u * v + u); }
+    __device__ __forceinline__ uint32_t ld(uint32_t idx) const { return lds_u16(2u * idx + tb); }
+    __device__ __forceinline__ bool zero(uint32_t v) const { return v >= M; }
+    __device__ __forceinline__ uint32_t odd(uint32_t v) const { return v & 1u; }
+};
+
+// GLOBAL32: 32-bit entries in global memory, read through L1 (the L2-resident regime).
+struct ExtTableG32 {
     static constexpr uint32_t SC = 1;
-    const T *t;
-    uint32_t M, OFF;
-    __device__ __forceinline__ uint32_t init() const { return OFF; }                       // W_1 = log 1 = 0
+    const uint32_t *t;
+    uint32_t M, Z0;
+    __device__ __forceinline__ uint32_t init() const { return 0u; }
     __device__ __forceinline__ uint32_t ub_init(uint32_t delta) const { return delta; }    // delta in [0, M)
     __device__ __forceinline__ uint32_t ub_next(uint32_t ub, uint32_t inc) const {
         const uint32_t nx = ub + inc;
         return nx >= M ? nx - M : nx;
     }
-    __device__ __forceinline__ uint32_t step(uint32_t v, uint32_t u) const {
-        if constexpr (kGlobal) return (uint32_t)__ldg(t + (v + u));
-        else return (uint32_t)t[v + u];
-    }
-    __device__ __forceinline__ bool zero(uint32_t v) const { return v == 0u; }
-    __device__ __forceinline__ uint32_t odd(uint32_t v) const { return v & 1u; }           // OFF is even
+    __device__ __forceinline__ uint32_t ld(uint32_t idx) const { return __ldg(t + idx); }
+    __device__ __forceinline__ uint32_t step(uint32_t v, uint32_t u) const { return ld(v + u); }
+    __device__ __forceinline__ bool zero(uint32_t v) const { return v >= M; }
+    __device__ __forceinline__ uint32_t odd(uint32_t v) const { return v & 1u; }
 };
 
 // Half tables in shared memory, for fields whose extended table does not fit.  With h = M/2 and
@@ -142,11 +166,187 @@ __device__ __forceinline__ void horner_all_x(const Pol pol, const uint32_t M, co
     }
 }
 
+// ---------------------------------------------------------------------------------------------------------
+// Radix-4 evaluation (not in the paper).  When 4 | M the 4th roots of unity
+// i^j = alpha^{j M/4} lie in the field, and with f(X) = sum_{r<4} X^r F_r(X^4) the four points of a coset
+// x mu_4 share the four values G_r = x^r F_r(x^4):
+//     f(i^j x) = sum_r i^{jr} G_r        t0 = G0 + G2, t1 = G0 - G2, t2 = G1 + G3, t3 = G1 - G3
+//     f(x) = t0 + t2,  f(-x) = t0 - t2,  f(ix) = t1 + i t3,  f(-ix) = t1 - i t3.
+// Per coset: one relative Horner chain per residue class of the exponent (deg f + 1 - 4 lookups for a dense f)
+// and a butterfly of 8 Zech additions a + b = a (1 + b/a) -> log a + Z[log b - log a] (reading G5), instead of
+// 4 deg f lookups.  f is still evaluated at every x of F_{q^k} (Algorithm 1 line 7).
+// Values are logs in [0, M); "zero" is any value >= M.  The lanes stride the coset index n = log x < M/4.
+constexpr uint32_t kBigZero = 0x40000000u;
+
+__device__ __forceinline__ uint32_t wrap_once(uint32_t x, uint32_t M) { return min(x, x - M); }   // [0, 2M) -> [0, M)
+
+// Zech arguments of a + w b and a - w b for nonzero a, b and log w = off in [0, M/4]:  a + w b = a (1 + w b / a).
+// A result a + Z may be zero: then Z = Z0 and the sum stays >= M.
+template <typename Pol>
+__device__ __forceinline__ void zech_add_sub(const Pol &pol, uint32_t M, uint32_t hM, uint32_t a, uint32_t b, uint32_t off,
+                                             uint32_t &z_add, uint32_t &z_sub) {
+    uint32_t dd = b - a + off;                  // in (-M, M + M/4]
+    dd = min(dd, dd + M);                       // congruent to log(w b / a), in [0, M + M/4]: inside the periodic part
+    z_add = pol.ld(dd);                         // 1 + w b / a
+    z_sub = pol.ld(dd + hM);                    // 1 - w b / a   (-1 = alpha^{M/2})
+}
+// s = a + w b, d = a - w b for operands that may be zero (>= M)
+template <typename Pol>
+__device__ __forceinline__ void zech_add_sub_any(const Pol &pol, uint32_t M, uint32_t hM, uint32_t a, uint32_t b, uint32_t off,
+                                                 uint32_t &s, uint32_t &d) {
+    const bool pa = a >= M, pb = b >= M;
+    a = pa ? kBigZero : a;
+    b = pb ? kBigZero : b;
+    uint32_t dd = b - a + off;
+    dd = min(dd, dd + M);
+    dd = (pa || pb) ? pol.Z0 : dd;              // constant region of the table: Z = 0, i.e. a + 0 = a
+    const uint32_t z1 = pol.ld(dd), z2 = pol.ld(dd + hM);
+    s = wrap_once(a + z1, M);
+    d = wrap_once(a + z2, M);
+    if (pa) {                                   // 0 + w b = w b, 0 - w b = -w b   (stay huge when b is zero too)
+        s = wrap_once(b + off, M);
+        d = wrap_once(b + off + hM, M);
+    }
+}
+
+template <int D, int U, typename Pol>
+__device__ __forceinline__ void radix4_all_x(const Pol pol, const uint32_t M, const uint32_t rcpM, const uint32_t lane,
+                                             const uint32_t nz, const uint32_t lcj, uint32_t &n_sq, uint32_t &n_zero) {
+    constexpr int NT = D - 3;                   // terms 0..D-4 can continue a chain
+    const uint32_t S = M >> 2, hM = M >> 1, qM = M >> 2;
+    uint32_t lterm[U];            // lanes past the last coset (tiny fields) use lane term 0; they are masked out below
+#pragma unroll
+    for (int u = 0; u < U; u++) lterm[u] = lane + 32u * u < S ? lane + 32u * u : 0u;
+
+    // ---- per-curve chain structure (all warp-uniform); chain offsets in units of Pol::SC
+    uint32_t ub[NT], inc[NT], gap[NT], cm = 0;
+    uint32_t last_lc[4] = {0, 0, 0, 0}, last_e[4] = {0, 0, 0, 0}, have = 0;
+#pragma unroll
+    for (int i = D; i >= 0; i--) {
+        const int r = i & 3;
+        const uint32_t lci = __shfl_sync(0xffffffffu, lcj, i);
+        if (i < NT) { ub[i] = 0; inc[i] = 0; gap[i] = 0; }
+        if (nz & (1u << i)) {
+            if (i < NT && (have & (1u << r))) {
+                const uint32_t m = last_e[r] - (uint32_t)i;
+                gap[i] = m * Pol::SC;
+                ub[i] = pol.ub_init(last_lc[r] >= lci ? last_lc[r] - lci : last_lc[r] + M - lci);
+                inc[i] = mod_once(m * (32u * U), M, rcpM) * Pol::SC;
+                cm |= 1u << i;
+            }
+            have |= 1u << r;
+            last_lc[r] = lci;
+            last_e[r] = (uint32_t)i;
+        }
+    }
+    // log G_r = W_r + K_r(n), K_r(n) = log c_{e_T} + e_T n: kept per lane, advanced per pass
+    uint32_t kc[4][U], kinc[4];
+#pragma unroll
+    for (int r = 0; r < 4; r++) {
+        kinc[r] = mod_once(last_e[r] * (32u * U), M, rcpM);
+#pragma unroll
+        for (int u = 0; u < U; u++) kc[r][u] = mod_once(last_lc[r] + last_e[r] * lterm[u], M, rcpM);
+    }
+
+    uint32_t acc = 0, n_odd = 0, n_nz = 0, passes = 0;      // acc: low half counts odd logs, high half nonzero values
+    for (uint32_t base = 0; base < S; base += 32u * U) {
+        uint32_t l[U][4];
+        uint32_t mx = 0;                                     // some value is zero  <=>  mx >= M
+#pragma unroll
+        for (int r = 0; r < 4; r++) {
+            if (!(have & (1u << r))) {                       // warp-uniform: no term with exponent = r mod 4
+#pragma unroll
+                for (int u = 0; u < U; u++) l[u][r] = kBigZero;
+                mx = kBigZero;
+                continue;
+            }
+            uint32_t v[U];
+#pragma unroll
+            for (int u = 0; u < U; u++) v[u] = 0u;           // W_1 = log 1
+#pragma unroll
+            for (int i = NT - 1; i >= 0; i--) {
+                if ((i & 3) != r) continue;
+                if (cm & (1u << i)) {
+                    const uint32_t ubi = ub[i], m = gap[i];
+#pragma unroll
+                    for (int u = 0; u < U; u++) v[u] = pol.step(v[u], m * lterm[u] + ubi);
+                    ub[i] = pol.ub_next(ubi, inc[i]);
+                }
+            }
+#pragma unroll
+            for (int u = 0; u < U; u++) {
+                l[u][r] = wrap_once(v[u] + kc[r][u], M);     // a zero chain (v = Z0) stays >= M
+                kc[r][u] = wrap_once(kc[r][u] + kinc[r], M);
+                mx = max(mx, l[u][r]);
+            }
+        }
+        uint32_t t[U][4];
+        if (!__any_sync(0xffffffffu, mx >= M)) {
+            mx = 0;
+#pragma unroll
+            for (int u = 0; u < U; u++) {
+                uint32_t za, zs;
+                zech_add_sub(pol, M, hM, l[u][0], l[u][2], 0u, za, zs);
+                t[u][0] = wrap_once(l[u][0] + za, M);
+                t[u][1] = wrap_once(l[u][0] + zs, M);
+                zech_add_sub(pol, M, hM, l[u][1], l[u][3], 0u, za, zs);
+                t[u][2] = wrap_once(l[u][1] + za, M);
+                t[u][3] = wrap_once(l[u][1] + zs, M);
+                mx = max(max(mx, max(t[u][0], t[u][1])), max(t[u][2], t[u][3]));
+            }
+        } else {
+#pragma unroll
+            for (int u = 0; u < U; u++) {
+                zech_add_sub_any(pol, M, hM, l[u][0], l[u][2], 0u, t[u][0], t[u][1]);
+                zech_add_sub_any(pol, M, hM, l[u][1], l[u][3], 0u, t[u][2], t[u][3]);
+            }
+            mx = kBigZero;
+        }
+        if (!__any_sync(0xffffffffu, mx >= M)) {
+#pragma unroll
+            for (int u = 0; u < U; u++) {
+                const bool valid = base + lane + 32u * u < S;
+#pragma unroll
+                for (int h = 0; h < 2; h++) {
+                    const uint32_t a = t[u][h], b = t[u][2 + h];
+                    uint32_t z[2];
+                    zech_add_sub(pol, M, hM, a, b, h ? qM : 0u, z[0], z[1]);   // h = 1: t1 +- i t3
+#pragma unroll
+                    for (int j = 0; j < 2; j++)
+                        if (valid && z[j] < M) acc += ((a ^ z[j]) & 1u) + 0x10000u;    // log f = a + Z (M is even)
+                }
+            }
+        } else {
+#pragma unroll
+            for (int u = 0; u < U; u++) {
+                const bool valid = base + lane + 32u * u < S;
+#pragma unroll
+                for (int h = 0; h < 2; h++) {
+                    uint32_t w[2];
+                    zech_add_sub_any(pol, M, hM, t[u][h], t[u][2 + h], h ? qM : 0u, w[0], w[1]);
+#pragma unroll
+                    for (int j = 0; j < 2; j++)
+                        if (valid && w[j] < M) acc += (w[j] & 1u) + 0x10000u;
+                }
+            }
+        }
+        if ((++passes & 2047u) == 0u) { n_odd += acc & 0xFFFFu; n_nz += acc >> 16; acc = 0; }   // <= 4 U per pass
+    }
+    n_odd += acc & 0xFFFFu;
+    n_nz += acc >> 16;
+    const uint32_t n_valid = 4u * ((S + 31u - lane) >> 5);
+    n_zero = n_valid - n_nz;
+    n_sq = n_nz - n_odd;
+}
+
 // One launch computes N_k for k_lo <= k <= k_hi.  Fields below k_hi use EXT16 tables; field k_hi uses TOP.
-template <int G, int U, int TOP>
+// RADIX: fields with 4 | M whose table is an extended one are evaluated by radix4_all_x (UR cosets per lane per
+// pass); all other fields by horner_all_x (U points per lane per pass).
+template <int G, int U, int TOP, bool RADIX>
 __global__ void __launch_bounds__(kThreads, 1) hec_count_kernel(const __grid_constant__ HecCountParams P) {
     constexpr int D = 2 * G + 2;          // largest degree; coefficient slots 0..D
     constexpr int NC = D + 1;
+    constexpr int UR = 2;
     extern __shared__ uint4 smem_blob[];
 
     for (uint32_t i = threadIdx.x; i < P.blob_bytes / 16; i += blockDim.x) smem_blob[i] = P.blob[i];
@@ -156,77 +356,93 @@ __global__ void __launch_bounds__(kThreads, 1) hec_count_kernel(const __grid_con
     const uint32_t warp = threadIdx.x >> 5;
     const unsigned long long stride = (unsigned long long)gridDim.x * kWarps;
     const char *smem = reinterpret_cast<const char *>(smem_blob);
+    const uint32_t smem_base = (uint32_t)__cvta_generic_to_shared(smem_blob);
 
     for (unsigned long long curve = (unsigned long long)blockIdx.x * kWarps + warp; curve < P.n; curve += stride) {
         // ---- a2: coefficient load (lane j holds c_j) and boundary checks (readings G13, hec.h)
         uint32_t cj = 0;
         if (lane < NC) cj = P.coeffs[curve * NC + lane];
         const bool bad_range = __any_sync(0xffffffffu, cj >= P.q);
-        const uint32_t top2 = __shfl_sync(0xffffffffu, cj, D) | __shfl_sync(0xffffffffu, cj, D - 1);
+        const uint32_t nz = __ballot_sync(0xffffffffu, cj != 0);          // bit j: c_j != 0
         const bool mine = lane + 1 >= P.k_lo && lane + 1 <= P.k_hi;
-        if (bad_range || top2 == 0) {
+        if (bad_range || (nz >> (D - 1)) == 0) {
             if (lane == 0) atomicMin(&P.err[bad_range ? 0 : 1], curve);
             if (mine) P.out[curve * G + lane] = 0;
             continue;
         }
-        uint32_t c[NC];
-#pragma unroll
-        for (int i = 0; i < NC; i++) c[i] = __shfl_sync(0xffffffffu, cj, i);
 
         uint32_t my_count = 0;   // lane k-1 keeps N_k
-#pragma unroll 1
-        for (uint32_t k = P.k_lo; k <= P.k_hi; k++) {
+#pragma unroll
+        for (uint32_t k = 1; k <= (uint32_t)G; k++) {
+            if (k < P.k_lo || k > P.k_hi) continue;
             const HecFieldDev &F = P.f[k - 1];
             const uint32_t M = F.M;
             // embed: log of c_j in F_{q^k} (reading G6)
             const uint32_t lcj = (lane < NC && cj != 0) ? __ldg(F.emb + cj) : HEC_LOG_ZERO;
-            uint32_t delta[D], incr[D], gap[D];
-            uint32_t nzmask = 0, prev_lc = 0, prev_e = 0;
-            bool started = false;
-#pragma unroll
-            for (int i = D; i >= 0; i--) {
-                const uint32_t lci = __shfl_sync(0xffffffffu, lcj, i);
-                if (i < D) { delta[i] = 0; incr[i] = 0; gap[i] = 0; }
-                if (c[i] != 0) {
-                    if (started && i < D) {
-                        const uint32_t m = prev_e - (uint32_t)i;
-                        gap[i] = m;
-                        delta[i] = prev_lc >= lci ? prev_lc - lci : prev_lc + M - lci;
-                        incr[i] = mod_once(m * (32u * U), M, F.rcpM);
-                        nzmask |= 1u << i;
+            // ---- a3 + a4: f at every x != 0, classify, per-lane partial sums of
+            //   n_zero = #{x != 0 : f(x) = 0},  n_sq = #{x != 0 : f(x) a nonzero square}      (reading G3)
+            uint32_t n_zero, n_sq;
+            bool done = false;
+            if constexpr (RADIX) {
+                if ((M & 3u) == 0u && (TOP == HEC_TAB_EXT16 || TOP == HEC_TAB_GLOBAL32 || k < P.k_hi)) {
+                    if (TOP == HEC_TAB_EXT16 || k < P.k_hi) {
+                        const ExtTableS16 pol{smem_base + F.smem_off, M, F.z0};
+                        radix4_all_x<D, UR>(pol, M, F.rcpM, lane, nz, lcj, n_sq, n_zero);
+                    } else if constexpr (TOP == HEC_TAB_GLOBAL32) {
+                        const ExtTableG32 pol{F.gtab, M, F.z0};
+                        radix4_all_x<D, UR>(pol, M, F.rcpM, lane, nz, lcj, n_sq, n_zero);
                     }
-                    started = true;
-                    prev_lc = lci;
-                    prev_e = (uint32_t)i;
+                    done = true;
                 }
             }
-            // ---- a3 + a4: Horner at every x != 0, classify, per-lane partial sums
-            uint32_t n_odd, n_zero;
-            if (TOP == HEC_TAB_EXT16 || k < P.k_hi) {
-                const ExtTable<uint16_t, false> pol{reinterpret_cast<const uint16_t *>(smem + F.smem_off), M, F.off};
-                horner_all_x<D, U>(pol, M, lane, F.lane_cap, nzmask, delta, incr, gap, n_odd, n_zero);
-            } else if constexpr (TOP == HEC_TAB_GLOBAL32) {
-                const ExtTable<uint32_t, true> pol{F.gtab, M, F.off};
-                horner_all_x<D, U>(pol, M, lane, F.lane_cap, nzmask, delta, incr, gap, n_odd, n_zero);
-            } else if constexpr (TOP == HEC_TAB_HALF32) {
-                const HalfTable<4> pol{smem + F.smem_off, nullptr, M, 4u * M, 2u * M, 4u * ((M >> 1) + 1u)};
-                horner_all_x<D, U>(pol, M, lane, F.lane_cap, nzmask, delta, incr, gap, n_odd, n_zero);
-            } else if constexpr (TOP == HEC_TAB_HALF24) {
-                const HalfTable<3> pol{smem + F.smem_off, smem + F.smem_off2, M, 2u * M, M, 2u * ((M >> 1) + 1u)};
-                horner_all_x<D, U>(pol, M, lane, F.lane_cap, nzmask, delta, incr, gap, n_odd, n_zero);
+            if (!done) {
+                uint32_t delta[D], incr[D], gap[D];
+                uint32_t nzmask = 0, prev_lc = 0, prev_e = 0;
+                bool started = false;
+#pragma unroll
+                for (int i = D; i >= 0; i--) {
+                    const uint32_t lci = __shfl_sync(0xffffffffu, lcj, i);
+                    if (i < D) { delta[i] = 0; incr[i] = 0; gap[i] = 0; }
+                    if (nz & (1u << i)) {
+                        if (started && i < D) {
+                            const uint32_t m = prev_e - (uint32_t)i;
+                            gap[i] = m;
+                            delta[i] = prev_lc >= lci ? prev_lc - lci : prev_lc + M - lci;
+                            incr[i] = mod_once(m * (32u * U), M, F.rcpM);
+                            nzmask |= 1u << i;
+                        }
+                        started = true;
+                        prev_lc = lci;
+                        prev_e = (uint32_t)i;
+                    }
+                }
+                uint32_t n_odd;
+                if (TOP == HEC_TAB_EXT16 || k < P.k_hi) {
+                    const ExtTableS16 pol{smem_base + F.smem_off, M, F.z0};
+                    horner_all_x<D, U>(pol, M, lane, F.lane_cap, nzmask, delta, incr, gap, n_odd, n_zero);
+                } else if constexpr (TOP == HEC_TAB_GLOBAL32) {
+                    const ExtTableG32 pol{F.gtab, M, F.z0};
+                    horner_all_x<D, U>(pol, M, lane, F.lane_cap, nzmask, delta, incr, gap, n_odd, n_zero);
+                } else if constexpr (TOP == HEC_TAB_HALF32) {
+                    const HalfTable<4> pol{smem + F.smem_off, nullptr, M, 4u * M, 2u * M, 4u * ((M >> 1) + 1u)};
+                    horner_all_x<D, U>(pol, M, lane, F.lane_cap, nzmask, delta, incr, gap, n_odd, n_zero);
+                } else if constexpr (TOP == HEC_TAB_HALF24) {
+                    const HalfTable<3> pol{smem + F.smem_off, smem + F.smem_off2, M, 2u * M, M, 2u * ((M >> 1) + 1u)};
+                    horner_all_x<D, U>(pol, M, lane, F.lane_cap, nzmask, delta, incr, gap, n_odd, n_zero);
+                }
+                // f(x) = A_T x^{e_T}; log f = log c_{e_T} + W_T + e_T log x; a nonzero value is a square iff its log
+                // is even (reading G4; M is even).  log x = base + lane + 32u has the parity of the lane.
+                const uint32_t n_valid = (M + 31u - lane) >> 5;
+                const uint32_t flip = (prev_lc ^ (prev_e & lane)) & 1u;
+                n_sq = flip ? n_odd : n_valid - n_zero - n_odd;
             }
-            // f(x) = A_T x^{e_T}; log f = log c_{e_T} + W_T + e_T log x; a nonzero value is a square iff its log
-            // is even (reading G4; M is even).  log x = base + lane + 32u has the parity of the lane.
-            const uint32_t n_valid = (M + 31u - lane) >> 5;
-            const uint32_t flip = (prev_lc ^ (prev_e & lane)) & 1u;
-            const uint32_t rsq_lane = flip ? n_odd : n_valid - n_zero - n_odd;
             const uint32_t r0 = __reduce_add_sync(0xffffffffu, n_zero);
-            const uint32_t rsq = __reduce_add_sync(0xffffffffu, rsq_lane);
+            const uint32_t rsq = __reduce_add_sync(0xffffffffu, n_sq);
             // ---- a5: x = 0 (reading G15) and the points at infinity
             const uint32_t lc0 = __shfl_sync(0xffffffffu, lcj, 0);
             const uint32_t lcD = __shfl_sync(0xffffffffu, lcj, D);
-            const uint32_t x0 = c[0] == 0 ? 1u : ((lc0 & 1u) ? 0u : 2u);
-            const uint32_t inf = c[D] == 0 ? 1u : ((lcD & 1u) ? 0u : 2u);
+            const uint32_t x0 = (nz & 1u) == 0 ? 1u : ((lc0 & 1u) ? 0u : 2u);
+            const uint32_t inf = ((nz >> D) & 1u) == 0 ? 1u : ((lcD & 1u) ? 0u : 2u);
             const uint32_t Nk = r0 + 2u * rsq + x0 + inf;
             if (lane + 1 == k) my_count = Nk;
         }
@@ -339,6 +555,7 @@ struct LibState {
     std::mutex mu;
     cudaStream_t stream = nullptr;
     int regime = HEC_REGIME_AUTO;
+    int eval = HEC_EVAL_AUTO;
     std::map<std::tuple<uint32_t, uint32_t, int>, std::unique_ptr<DevicePlan>> plans;
     hec_count_stats stats{};
     cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};
@@ -379,14 +596,14 @@ hec_table_geom table_geom(uint32_t M, uint32_t D, uint32_t U) {
 
 template <typename T>
 void fill_extended(const hec_field &F, const hec_table_geom &t, T *out) {
-    const uint32_t M = t.M, OFF = t.lmax;
-    for (uint32_t i = 0; i < t.lmax; i++) out[i] = (T)OFF;
+    const uint32_t M = t.M, Z0 = M + t.lmax;
     uint32_t n = 0;
-    for (uint32_t i = OFF; i < t.entries; i++) {
+    for (uint32_t i = 0; i < Z0; i++) {
         const uint32_t z = F.zech[n];
-        out[i] = (T)(z == M ? 0u : OFF + z);
+        out[i] = (T)(z == M ? Z0 : z);
         if (++n == M) n = 0;
     }
+    for (uint32_t i = Z0; i < t.entries; i++) out[i] = (T)0u;
 }
 
 // Half table (kernel comment "Half tables"): entry b in [0, h] holds Z(h - b) - h, entry h + 1 holds -h
@@ -440,7 +657,7 @@ int build_plan(LibState &S, uint32_t q, uint32_t g, int regime, DevicePlan **out
     // ---- table mode of every field and the grouping into launches (one shared-memory image per launch)
     auto ext16_bytes = [&](uint32_t k) -> uint32_t {
         const hec_table_geom &t = geom[k - 1];
-        if ((uint64_t)t.lmax + t.M > 65536u) return 0;               // stored values must fit 16 bits
+        if ((uint64_t)t.lmax + t.M > 65535u) return 0;               // Z0 = M + LP must fit 16 bits
         const uint64_t b = (uint64_t)t.entries * 2u;
         return b <= budget ? align16((uint32_t)b) : 0;
     };
@@ -505,7 +722,7 @@ int build_plan(LibState &S, uint32_t q, uint32_t g, int regime, DevicePlan **out
         for (uint32_t k = G.k_lo; k <= G.k_hi; k++) {
             const hec_table_geom &t = geom[k - 1];
             HecFieldDev &fd = plan->f[k - 1];
-            fd.M = t.M; fd.mode = (uint32_t)mode[k - 1]; fd.off = t.lmax; fd.rcpM = (uint32_t)((1ull << 32) / t.M);
+            fd.M = t.M; fd.mode = (uint32_t)mode[k - 1]; fd.z0 = t.M + t.lmax; fd.rcpM = (uint32_t)((1ull << 32) / t.M);
             fd.lane_cap = std::min<uint32_t>(32u * U, t.M);
             fd.smem_off = so; fd.smem_off2 = 0; fd.pad_ = 0; fd.gtab = nullptr;
             uint8_t *dst = host.data() + blob_off[gi] + so;
@@ -566,9 +783,9 @@ int build_plan(LibState &S, uint32_t q, uint32_t g, int regime, DevicePlan **out
     return HEC_OK;
 }
 
-template <int G, int U, int TOP>
+template <int G, int U, int TOP, bool RADIX>
 int launch_one(LibState &S, const LaunchPlan &L, const HecCountParams &P) {
-    auto kern = hec_count_kernel<G, U, TOP>;
+    auto kern = hec_count_kernel<G, U, TOP, RADIX>;
     HEC_CUDA_OK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)L.smem_bytes));
     uint32_t grid = (uint32_t)std::min<unsigned long long>((P.n + kWarps - 1) / kWarps, (unsigned long long)S.sm_count);
     if (grid == 0) grid = 1;
@@ -588,11 +805,22 @@ int launch_count(LibState &S, const DevicePlan &plan, HecCountParams P) {
     for (const LaunchPlan &L : plan.launches) {
         P.blob = L.blob; P.blob_bytes = L.blob_bytes; P.k_lo = L.k_lo; P.k_hi = L.k_hi;
         int rc;
+        const bool radix = S.eval != HEC_EVAL_HORNER;
         switch (L.top_mode) {
-            case HEC_TAB_GLOBAL32: rc = launch_one<G, U, HEC_TAB_GLOBAL32>(S, L, P); break;
-            case HEC_TAB_HALF32: rc = launch_one<G, U, HEC_TAB_HALF32>(S, L, P); break;
-            case HEC_TAB_HALF24: rc = launch_one<G, U, HEC_TAB_HALF24>(S, L, P); break;
-            default: rc = launch_one<G, U, HEC_TAB_EXT16>(S, L, P); break;
+            case HEC_TAB_GLOBAL32:
+                rc = radix ? launch_one<G, U, HEC_TAB_GLOBAL32, true>(S, L, P) : launch_one<G, U, HEC_TAB_GLOBAL32, false>(S, L, P);
+                break;
+            case HEC_TAB_HALF32: rc = launch_one<G, U, HEC_TAB_HALF32, false>(S, L, P); break;
+            case HEC_TAB_HALF24: rc = launch_one<G, U, HEC_TAB_HALF24, false>(S, L, P); break;
+            default:
+                rc = radix ? launch_one<G, U, HEC_TAB_EXT16, true>(S, L, P) : launch_one<G, U, HEC_TAB_EXT16, false>(S, L, P);
+                break;
+        }
+        if (rc) return rc;
+        for (uint32_t k = L.k_lo; k <= L.k_hi; k++) {
+            const bool ext = plan.f[k - 1].mode == HEC_TAB_EXT16 || plan.f[k - 1].mode == HEC_TAB_GLOBAL32;
+            if (radix && ext && (L.top_mode == HEC_TAB_EXT16 || L.top_mode == HEC_TAB_GLOBAL32) && plan.f[k - 1].M % 4u == 0)
+                S.stats.radix4_fields |= 1u << (k - 1);
         }
         if (rc) return rc;
     }
@@ -631,6 +859,13 @@ int hec_set_regime(int regime) {
     if (regime < HEC_REGIME_AUTO || regime > HEC_REGIME_SMEM_HALF) HEC_FAIL(HEC_ERR_INVALID_ARG, "unknown regime");
     std::lock_guard<std::mutex> lock(g_state.mu);
     g_state.regime = regime;
+    return HEC_OK;
+}
+
+int hec_set_eval(int eval) {
+    if (eval != HEC_EVAL_AUTO && eval != HEC_EVAL_HORNER) HEC_FAIL(HEC_ERR_INVALID_ARG, "unknown evaluation scheme");
+    std::lock_guard<std::mutex> lock(g_state.mu);
+    g_state.eval = eval;
     return HEC_OK;
 }
 

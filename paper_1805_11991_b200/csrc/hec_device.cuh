@@ -29,7 +29,7 @@ enum HecTableMode : uint32_t {
 struct HecFieldDev {
     uint32_t M;          // q^k - 1
     uint32_t mode;       // HecTableMode
-    uint32_t off;        // extended tables: OFF = LMAX = M + PADL (even)
+    uint32_t z0;         // extended tables: Z0 = M + LP, the stored value of the zero element (LP = M + PADL)
     uint32_t rcpM;       // floor(2^32 / M), for x mod M with one correction step
     uint32_t smem_off;   // byte offset inside the launch's blob (16-byte aligned): table / low plane
     uint32_t smem_off2;  // HALF24: byte offset of the high plane

@@ -32,16 +32,16 @@ const hec_field *hec_cached_field(uint32_t p, uint32_t r, uint32_t k);
 void hec_clear_field_cache();
 
 // ---------------------------------------------------------------------------- device side
-// Geometry of one extended Zech table (DESIGN.md "Table layout").  Stored value of a lookup result:
-//   0            the element is zero (1 + alpha^n = 0)
-//   OFF + Z(n)   otherwise, OFF = LMAX even
-// Index space: idx = stored value + L, L in [0, LMAX), LMAX = M + PADL.
-//   idx in [0, LMAX)                 -> OFF          (accumulator was zero: acc*x^m + c = c, i.e. W = log 1 = 0)
-//   idx in [OFF, OFF + M + LMAX)     -> stored Zech of (idx - OFF) mod M
+// Geometry of one extended Zech table (DESIGN.md "Table layouts").  Stored value of a lookup result:
+//   Z(n) in [0, M)   the log of 1 + alpha^n
+//   Z0 = M + LP      the element is zero (1 + alpha^n = 0), LP = M + PADL
+// Index space: idx = stored value + L, L in [0, LP).
+//   idx in [0, M + LP)       -> stored Zech of idx mod M
+//   idx in [Z0, Z0 + LP)     -> 0   (accumulator was zero: acc*x^m + c = c, i.e. W = log 1 = 0)
 struct hec_table_geom {
     uint32_t M;        // Q - 1
     uint32_t padl;     // largest lane term m * (32 U - 1) + 1, rounded up to even
-    uint32_t lmax;     // M + padl  (= OFF)
+    uint32_t lmax;     // LP = M + padl
     uint32_t entries;  // 2 * lmax + M
 };
 

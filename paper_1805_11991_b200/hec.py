@@ -22,6 +22,7 @@ HEC_OK = 0
 HEC_ERR_INVALID_FIELD, HEC_ERR_INVALID_ARG, HEC_ERR_COEFF_RANGE, HEC_ERR_DEGREE = -1, -2, -3, -4
 HEC_ERR_CAPACITY, HEC_ERR_UNSUPPORTED, HEC_ERR_CUDA, HEC_ERR_NOMEM = -5, -6, -7, -8
 REGIME_AUTO, REGIME_SMEM, REGIME_L2, REGIME_SMEM_HALF = 0, 1, 2, 3
+EVAL_AUTO, EVAL_HORNER = 0, 1
 TABLE_MODES = {0: "global32-extended", 1: "smem16-extended", 2: "smem32-half", 3: "smem16+8-half"}
 MAX_GENUS = 5
 
@@ -31,7 +32,7 @@ SYMBOLS = [
     "hec_field_degree", "hec_field_q", "hec_field_Q", "hec_field_embed_unit", "hec_field_modulus",
     "hec_field_antilog", "hec_field_log", "hec_field_zech", "hec_field_embed", "hec_count", "hec_histogram",
     "hec_histogram_merge",
-    "hec_set_stream", "hec_set_regime", "hec_last_count_stats", "hec_launch_count", "hec_gather_bench",
+    "hec_set_stream", "hec_set_regime", "hec_set_eval", "hec_last_count_stats", "hec_launch_count", "hec_gather_bench",
     "hec_shutdown",
 ]
 
@@ -46,7 +47,7 @@ class CountStats(ctypes.Structure):
     _fields_ = [("count_kernel_ms", ctypes.c_float), ("squarefree_kernel_ms", ctypes.c_float),
                 ("launches", ctypes.c_uint32), ("regime", ctypes.c_uint32), ("smem_bytes", ctypes.c_uint32),
                 ("grid", ctypes.c_uint32), ("block", ctypes.c_uint32), ("chains_per_lane", ctypes.c_uint32),
-                ("table_mode", ctypes.c_uint32)]
+                ("table_mode", ctypes.c_uint32), ("radix4_fields", ctypes.c_uint32)]
 
 
 def lib():
@@ -74,6 +75,7 @@ def lib():
         L.hec_histogram_merge.argtypes = [vp, vp, sz, u32, vp, vp, sz, ctypes.POINTER(sz)]
         L.hec_set_stream.argtypes = [vp]
         L.hec_set_regime.argtypes = [ctypes.c_int]
+        L.hec_set_eval.argtypes = [ctypes.c_int]
         L.hec_last_count_stats.argtypes = [ctypes.POINTER(CountStats)]
         L.hec_launch_count.restype = ctypes.c_uint64
         L.hec_gather_bench.argtypes = [ctypes.c_int, u32, u32, u32, u32, u32, u32,
@@ -162,6 +164,10 @@ def set_stream(cuda_stream: int | None):
 
 def set_regime(regime: int):
     _check(lib().hec_set_regime(regime))
+
+
+def set_eval(scheme: int):
+    _check(lib().hec_set_eval(scheme))
 
 
 def count(q: int, g: int, coeffs, out_counts=None, out_squarefree=None, want_squarefree: bool = True):

@@ -14,8 +14,10 @@ from paper_1805_11991_b200 import hec, workloads as W
 pytestmark = pytest.mark.gpu
 
 
-@pytest.fixture(scope="module")
-def torch_cuda():
+@pytest.fixture(scope="module", params=["auto", "horner"])
+def torch_cuda(request):
+    """Every test runs under both evaluation schemes of hec_count: the default (radix-4 split where 4 | q^k - 1)
+    and the paper's one-Horner-chain-per-x scheme; the oracle is the same for both."""
     import torch
     from paper_1805_11991_b200 import build as hb
     hb.build_lib()
@@ -23,7 +25,10 @@ def torch_cuda():
     torch.cuda.set_device(0)
     hec.set_stream(torch.cuda.current_stream().cuda_stream)
     hec.set_regime(hec.REGIME_AUTO)
-    return torch
+    hec.set_eval(hec.EVAL_AUTO if request.param == "auto" else hec.EVAL_HORNER)
+    torch.eval_scheme = request.param
+    yield torch
+    hec.set_eval(hec.EVAL_AUTO)
 
 
 def _dev(torch, rows):
@@ -266,13 +271,34 @@ def test_full_config2(torch_cuda):
 def test_full_config4_headline(torch_cuda):
     stats = _full_size_checks(torch_cuda, 4, 96)
     assert stats["regime"] == hec.REGIME_SMEM
+    assert stats["radix4_fields"] == (0b1111 if torch_cuda.eval_scheme == "auto" else 0)
+
+
+def test_eval_schemes_agree_full_config4(torch_cuda):
+    """All 2^24 rows of the headline workload: radix-4 split and plain Horner give identical counts."""
+    if torch_cuda.eval_scheme != "auto":
+        pytest.skip("compares both schemes in one run")
+    cfg = W.CONFIGS[4]
+    d_rows = _dev(torch_cuda, W.generate(cfg))
+    try:
+        a, _ = hec.count(cfg.q, cfg.g, d_rows, want_squarefree=False)
+        hec.set_eval(hec.EVAL_HORNER)
+        b, _ = hec.count(cfg.q, cfg.g, d_rows, want_squarefree=False)
+        assert hec.last_count_stats()["radix4_fields"] == 0
+    finally:
+        hec.set_eval(hec.EVAL_AUTO)
+    assert bool((a == b).all())
 
 
 def test_full_config5_half_table(torch_cuda):
+    if torch_cuda.eval_scheme != "auto":
+        pytest.skip("half-table layouts have one evaluation scheme")
     stats = _full_size_checks(torch_cuda, 5, 64)
     assert stats["regime"] == hec.REGIME_SMEM_HALF and stats["table_mode"] == 2
 
 
 def test_full_config3_half_planes(torch_cuda):
+    if torch_cuda.eval_scheme != "auto":
+        pytest.skip("half-table layouts have one evaluation scheme")
     stats = _full_size_checks(torch_cuda, 3, 16)
     assert stats["regime"] == hec.REGIME_SMEM_HALF and stats["table_mode"] == 3
