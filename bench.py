@@ -52,6 +52,44 @@ def algorithmic_lookups(cfg: W.Workload, rows: np.ndarray) -> int:
     return int(steps.sum()) * nx
 
 
+# loads per Zech value (single) and per butterfly pair (Z[n], Z[n + M/2]) in each table layout (hec_radix.cuh)
+LOADS = {0: (1, None), 1: (1, None), 2: (1, None), 3: (2, None), 4: (1, 1), 5: (1, 2), 6: (2, 3), 7: (1, 1)}
+
+
+def executed_loads(cfg: W.Workload, rows: np.ndarray, stats: dict) -> int:
+    """Table loads the count kernel issues for this batch, from the rows' zero patterns (exact up to the rare
+    re-evaluated cosets).  Horner scheme: one lookup per nonzero term after the first, per nonzero x.
+    Radix-R scheme (hec_radix.cuh): per coset of R points, (#terms - #nonempty residue classes mod R) chain
+    lookups plus one pair lookup per butterfly whose two inputs are both nonzero."""
+    nzm = rows != 0
+    n, ncoef = rows.shape
+    top_mode = stats["table_mode"]
+    total = 0
+    for k in range(1, cfg.g + 1):
+        M = cfg.q ** k - 1
+        R = (stats["radix_fields"] >> (4 * (k - 1))) & 15
+        mode = top_mode if k == cfg.g else (4 if R else 1)
+        single, pair = LOADS[mode]
+        if R == 0:
+            total += int((nzm.sum(axis=1) - 1).sum()) * M * single
+            continue
+        present = np.zeros((n, R), dtype=bool)
+        for r in range(R):
+            present[:, r] = nzm[:, r::R].any(axis=1)
+        chain = int((nzm.sum(axis=1) - present.sum(axis=1)).sum())
+        pairs = 0
+        H = R // 2
+        while H >= 1:
+            for blk in range(0, R, 2 * H):
+                for j in range(H):
+                    a, b = present[:, blk + j].copy(), present[:, blk + j + H].copy()
+                    pairs += int((a & b).sum())
+                    present[:, blk + j] = present[:, blk + j + H] = a | b
+            H //= 2
+        total += (chain * single + pairs * pair) * (M // R)
+    return total
+
+
 class ClockSampler:
     """Samples SM clock and throttle reasons during the timed region (pynvml, 100 ms period)."""
     REASONS = {0x4: "sw_power_cap", 0x8: "hw_slowdown", 0x20: "sw_thermal_slowdown", 0x40: "hw_thermal_slowdown",
@@ -172,6 +210,8 @@ def run_ours(args, cfg):
         dist.barrier()
     stream = torch.cuda.current_stream()
     hec.set_stream(stream.cuda_stream)
+    hec.set_eval({"auto": hec.EVAL_AUTO, "horner": hec.EVAL_HORNER, "radix2": hec.EVAL_RADIX2, "radix4": hec.EVAL_RADIX4,
+                  "radix8": hec.EVAL_RADIX8}[args.eval])
     hec.set_regime({"auto": hec.REGIME_AUTO, "smem": hec.REGIME_SMEM, "l2": hec.REGIME_L2, "half": hec.REGIME_SMEM_HALF}[args.regime])
 
     rows = workload_rows(cfg, rank)
@@ -194,16 +234,18 @@ def run_ours(args, cfg):
 
     for _ in range(args.warmup):
         stats, tup, mult = step()
-    # measured lookup ceiling at the same footprint and entry width as the largest field's table
+    # measured lookup ceiling at the same footprint and word width as the largest field's table
     regime, mode = stats["regime"], stats["table_mode"]
     Mtop = q ** g - 1
-    ext_entries = 3 * Mtop + 2 * min(32 * stats["chains_per_lane"], Mtop) * (2 * g + 2)
+    ext_entries = 3 * Mtop + 2 * min(32 * 4, Mtop) * (2 * g + 2)
     # (where, entries, entry bytes) of the gather micro-benchmark that matches the largest field's table
     where, ceil_entries, ceil_bytes = {0: (1, ext_entries, 4), 1: (0, ext_entries, 2),
-                                       2: (0, Mtop // 2 + 2, 4), 3: (0, Mtop // 2 + 2, 2)}[mode]
+                                       2: (0, Mtop // 2 + 2, 4), 3: (0, Mtop // 2 + 2, 2),
+                                       4: (0, Mtop, 4), 5: (0, Mtop // 2 + 2, 4), 6: (0, Mtop // 2 + 2, 2),
+                                       7: (1, 2 * Mtop, 4)}[mode]
     gather_rate, _ = hec.gather_bench(where, max(ceil_entries, 1024), ceil_bytes, 1024, 1, 4,
                                       8192 if where == 0 else 1024)
-    loads_per_lookup = 2 if mode == 3 else 1           # 16+8-bit planes: two shared-memory loads per Zech lookup
+    executed = executed_loads(cfg, rows, stats)         # loads the kernel really issues (radix split: far fewer)
 
     sync_all()
     launches0 = hec.launch_count()
@@ -263,13 +305,16 @@ def run_ours(args, cfg):
     hbm_bytes = rows.nbytes + n * g * 4 + n
     roofline = {
         "bound": "smem" if mode != 0 else "l1/l2",
-        "table_layout": hec.TABLE_MODES[mode], "smem_loads_per_lookup": loads_per_lookup,
-        "kernel": "hec_count_kernel",
+        "table_layout": hec.TABLE_MODES[mode],
+        "kernel": "hec_count_radix_kernel" if stats["radix_fields"] else "hec_count_kernel",
+        "radix_per_field": [(stats["radix_fields"] >> (4 * k)) & 15 for k in range(g)],
         "achieved": achieved / 1e9, "peak": gather_rate / 1e9, "unit": "Glookups/s", "frac": achieved / gather_rate,
         "peak_source": "measured in this run: hec_gather_bench, dependent random gathers, same footprint and entry width",
         "peak_model": conflict_free / EXPECTED_WAVEFRONTS / 1e9 if mode != 0 else None,
         "peak_conflict_free": conflict_free / 1e9, "frac_conflict_free": achieved / conflict_free,
-        "lookups_per_launch": lookups, "kernel_ms": k_ms, "squarefree_kernel_ms": float(np.mean(sq_ms)),
+        "lookups_per_launch": lookups, "executed_loads_per_launch": executed,
+        "executed": executed / (k_ms * 1e-3) / 1e9, "frac_executed": executed / (k_ms * 1e-3) / gather_rate,
+        "kernel_ms": k_ms, "squarefree_kernel_ms": float(np.mean(sq_ms)),
         "kernel_share_of_step": k_ms * args.steps / elapsed_ms,
         "hbm": {"achieved_gbs": hbm_bytes / (k_ms * 1e-3) / 1e9, "peak_gbs": hbm_peak,
                 "frac": hbm_bytes / (k_ms * 1e-3) / 1e9 / hbm_peak, "algorithmic_bytes_per_launch": hbm_bytes},
@@ -280,7 +325,7 @@ def run_ours(args, cfg):
         "warmup": args.warmup, "ms_per_step": elapsed_ms / args.steps, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "u32", "data": "synthetic",
         "config": {"workload": cfg.name, "q": q, "g": g, "n_curves_per_gpu": n, "regime": {1: "smem", 2: "l2", 3: "smem-half"}[regime],
-                   "table_layout": hec.TABLE_MODES[mode], "count_launches": stats["launches"] - 1,
+                   "eval": args.eval, "table_layout": hec.TABLE_MODES[mode], "count_launches": stats["launches"] - 1,
                    "grid": stats["grid"], "block": stats["block"], "smem_bytes": stats["smem_bytes"],
                    "chains_per_lane": stats["chains_per_lane"], "parallelism": f"curve-sharded x{world}",
                    "l2": f"inputs+outputs {hbm_bytes / 1e6:.0f} MB per step vs 126 MB L2: larger than L2"
@@ -315,6 +360,8 @@ def main():
     ap.add_argument("--config", type=int, default=4, choices=sorted(W.CONFIGS))
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--regime", default="auto", choices=["auto", "smem", "l2", "half"])
+    ap.add_argument("--eval", default="auto", choices=["auto", "horner", "radix2", "radix4", "radix8"],
+                    help="evaluation scheme of hec_count (auto: radix split; horner: the paper's one chain per x)")
     ap.add_argument("--cpu-seconds", type=float, default=15.0, help="CPU work of the cpu_baseline sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--curves", type=int, default=0,

@@ -134,12 +134,12 @@ int hec_histogram_merge(const uint32_t *in_tuples, const uint64_t *in_mult, size
 int hec_set_stream(void *cuda_stream);
 
 typedef enum hec_regime {
-    HEC_REGIME_AUTO = 0,       /* per field: extended 16-bit table in shared memory if it fits, else a half table
-                                  (Z(-n) = Z(n) - n; 32-bit, else 16+8-bit planes) in shared memory if it fits,
-                                  else the L2-resident table */
-    HEC_REGIME_SMEM = 1,       /* force the extended shared-memory table for the largest field (HEC_ERR_INVALID_ARG
+    HEC_REGIME_AUTO = 0,       /* per field: full table in shared memory if it fits (Horner: extended 16-bit table; radix:
+                                  2x16-bit pair table), else a half table (Z(-n) = Z(n) - n; 32-bit, else 16+8-bit / 16+1-bit
+                                  planes) in shared memory if it fits, else the L2-resident table */
+    HEC_REGIME_SMEM = 1,       /* force the full shared-memory table for the largest field (HEC_ERR_INVALID_ARG
                                   when it cannot fit) */
-    HEC_REGIME_L2 = 2,         /* force the L2-resident (global memory, 32-bit entries) table for the largest field */
+    HEC_REGIME_L2 = 2,         /* force the L2-resident (global memory, 32-bit words) table for the largest field */
     HEC_REGIME_SMEM_HALF = 3   /* force the shared-memory half table for the largest field (HEC_ERR_INVALID_ARG when
                                   it cannot fit or the field has fewer than 2^13 elements) */
 } hec_regime;
@@ -147,20 +147,26 @@ int hec_set_regime(int regime);
 
 /* Evaluation scheme of hec_count (results are identical; f is evaluated at every x either way). */
 typedef enum hec_eval {
-    HEC_EVAL_AUTO = 0,         /* fields with 4 | q^k - 1 whose table is an extended one: radix-4 split, f(X) = sum_r X^r F_r(X^4):
-                                  the four points x, ix, -x, -ix of a coset share the four Horner chains F_r(x^4) and are
-                                  combined by a butterfly of Zech additions (about 2.5x fewer lookups at degree 10);
-                                  all other fields: HEC_EVAL_HORNER */
-    HEC_EVAL_HORNER = 1        /* the paper's scheme (Algorithm 1 line 8): one Horner chain per x */
+    HEC_EVAL_AUTO = 0,         /* radix-R split (not in the paper): with R in {2, 4, 8} the largest power of two dividing
+                                  q^k - 1 (capped per table layout), f(X) = sum_{r<R} X^r F_r(X^R): the R points x zeta^j of a
+                                  coset of the R-th roots of unity share the R Horner chains F_r(x^R) and are combined by an
+                                  R-point butterfly network of Zech additions, one table entry serving a + w b and a - w b
+                                  (about 5x fewer lookups at degree 10).  Tables: pairs (Z[n], Z[n + M/2]) or half tables. */
+    HEC_EVAL_HORNER = 1,       /* the paper's scheme (Algorithm 1 line 8): one Horner chain per x */
+    HEC_EVAL_RADIX2 = 2,       /* as AUTO with R capped at 2 / 4 / 8 (tuning and tests) */
+    HEC_EVAL_RADIX4 = 4,
+    HEC_EVAL_RADIX8 = 8
 } hec_eval;
 int hec_set_eval(int eval);
 
 /* Statistics of the last hec_count on this thread's library state: device time of the count kernel(s) and
  * of the squarefree kernel (CUDA events on the launch stream, ms), number of kernel launches (one count
  * launch per group of fields whose tables share one shared-memory image, plus the squarefree kernel), the
- * regime used for the largest field (hec_regime) and its table layout (0 global 32-bit extended, 1 shared
- * 16-bit extended, 2 shared 32-bit half, 3 shared 16+8-bit half), the largest dynamic shared memory per
- * CTA, grid and block size of the last count launch, and which fields used the radix-4 split. */
+ * regime used for the largest field (hec_regime) and its table layout -- Horner kernel: 0 global 32-bit
+ * extended, 1 shared 16-bit extended, 2 shared 32-bit half, 3 shared 16+8-bit half; radix kernel: 4 shared
+ * 2x16-bit pairs, 5 shared 32-bit half, 6 shared 16+1-bit half, 7 global 2x32-bit pairs --, the largest
+ * dynamic shared memory per CTA, grid and block size of the last count launch, independent x (Horner) or
+ * cosets (radix) per lane per pass, and the radix of every field. */
 typedef struct hec_count_stats {
     float count_kernel_ms;
     float squarefree_kernel_ms;
@@ -171,7 +177,7 @@ typedef struct hec_count_stats {
     uint32_t block;
     uint32_t chains_per_lane;
     uint32_t table_mode;
-    uint32_t radix4_fields;    /* bit k-1 set: N_k was computed with the radix-4 split */
+    uint32_t radix_fields;     /* nibble k-1: radix R used for N_k (0: one Horner chain per x) */
 } hec_count_stats;
 int hec_last_count_stats(hec_count_stats *out);
 

@@ -16,8 +16,10 @@
 #include <vector>
 
 #include "hec_device.cuh"
+#include "hec_radix.cuh"
 
 uint64_t hec_launch_counter::value = 0;
+void hec_histogram_release_pool();
 
 namespace {
 
@@ -166,187 +168,12 @@ __device__ __forceinline__ void horner_all_x(const Pol pol, const uint32_t M, co
     }
 }
 
-// ---------------------------------------------------------------------------------------------------------
-// Radix-4 evaluation (not in the paper).  When 4 | M the 4th roots of unity
-// i^j = alpha^{j M/4} lie in the field, and with f(X) = sum_{r<4} X^r F_r(X^4) the four points of a coset
-// x mu_4 share the four values G_r = x^r F_r(x^4):
-//     f(i^j x) = sum_r i^{jr} G_r        t0 = G0 + G2, t1 = G0 - G2, t2 = G1 + G3, t3 = G1 - G3
-//     f(x) = t0 + t2,  f(-x) = t0 - t2,  f(ix) = t1 + i t3,  f(-ix) = t1 - i t3.
-// Per coset: one relative Horner chain per residue class of the exponent (deg f + 1 - 4 lookups for a dense f)
-// and a butterfly of 8 Zech additions a + b = a (1 + b/a) -> log a + Z[log b - log a] (reading G5), instead of
-// 4 deg f lookups.  f is still evaluated at every x of F_{q^k} (Algorithm 1 line 7).
-// Values are logs in [0, M); "zero" is any value >= M.  The lanes stride the coset index n = log x < M/4.
-constexpr uint32_t kBigZero = 0x40000000u;
-
-__device__ __forceinline__ uint32_t wrap_once(uint32_t x, uint32_t M) { return min(x, x - M); }   // [0, 2M) -> [0, M)
-
-// Zech arguments of a + w b and a - w b for nonzero a, b and log w = off in [0, M/4]:  a + w b = a (1 + w b / a).
-// A result a + Z may be zero: then Z = Z0 and the sum stays >= M.
-template <typename Pol>
-__device__ __forceinline__ void zech_add_sub(const Pol &pol, uint32_t M, uint32_t hM, uint32_t a, uint32_t b, uint32_t off,
-                                             uint32_t &z_add, uint32_t &z_sub) {
-    uint32_t dd = b - a + off;                  // in (-M, M + M/4]
-    dd = min(dd, dd + M);                       // congruent to log(w b / a), in [0, M + M/4]: inside the periodic part
-    z_add = pol.ld(dd);                         // 1 + w b / a
-    z_sub = pol.ld(dd + hM);                    // 1 - w b / a   (-1 = alpha^{M/2})
-}
-// s = a + w b, d = a - w b for operands that may be zero (>= M)
-template <typename Pol>
-__device__ __forceinline__ void zech_add_sub_any(const Pol &pol, uint32_t M, uint32_t hM, uint32_t a, uint32_t b, uint32_t off,
-                                                 uint32_t &s, uint32_t &d) {
-    const bool pa = a >= M, pb = b >= M;
-    a = pa ? kBigZero : a;
-    b = pb ? kBigZero : b;
-    uint32_t dd = b - a + off;
-    dd = min(dd, dd + M);
-    dd = (pa || pb) ? pol.Z0 : dd;              // constant region of the table: Z = 0, i.e. a + 0 = a
-    const uint32_t z1 = pol.ld(dd), z2 = pol.ld(dd + hM);
-    s = wrap_once(a + z1, M);
-    d = wrap_once(a + z2, M);
-    if (pa) {                                   // 0 + w b = w b, 0 - w b = -w b   (stay huge when b is zero too)
-        s = wrap_once(b + off, M);
-        d = wrap_once(b + off + hM, M);
-    }
-}
-
-template <int D, int U, typename Pol>
-__device__ __forceinline__ void radix4_all_x(const Pol pol, const uint32_t M, const uint32_t rcpM, const uint32_t lane,
-                                             const uint32_t nz, const uint32_t lcj, uint32_t &n_sq, uint32_t &n_zero) {
-    constexpr int NT = D - 3;                   // terms 0..D-4 can continue a chain
-    const uint32_t S = M >> 2, hM = M >> 1, qM = M >> 2;
-    uint32_t lterm[U];            // lanes past the last coset (tiny fields) use lane term 0; they are masked out below
-#pragma unroll
-    for (int u = 0; u < U; u++) lterm[u] = lane + 32u * u < S ? lane + 32u * u : 0u;
-
-    // ---- per-curve chain structure (all warp-uniform); chain offsets in units of Pol::SC
-    uint32_t ub[NT], inc[NT], gap[NT], cm = 0;
-    uint32_t last_lc[4] = {0, 0, 0, 0}, last_e[4] = {0, 0, 0, 0}, have = 0;
-#pragma unroll
-    for (int i = D; i >= 0; i--) {
-        const int r = i & 3;
-        const uint32_t lci = __shfl_sync(0xffffffffu, lcj, i);
-        if (i < NT) { ub[i] = 0; inc[i] = 0; gap[i] = 0; }
-        if (nz & (1u << i)) {
-            if (i < NT && (have & (1u << r))) {
-                const uint32_t m = last_e[r] - (uint32_t)i;
-                gap[i] = m * Pol::SC;
-                ub[i] = pol.ub_init(last_lc[r] >= lci ? last_lc[r] - lci : last_lc[r] + M - lci);
-                inc[i] = mod_once(m * (32u * U), M, rcpM) * Pol::SC;
-                cm |= 1u << i;
-            }
-            have |= 1u << r;
-            last_lc[r] = lci;
-            last_e[r] = (uint32_t)i;
-        }
-    }
-    // log G_r = W_r + K_r(n), K_r(n) = log c_{e_T} + e_T n: kept per lane, advanced per pass
-    uint32_t kc[4][U], kinc[4];
-#pragma unroll
-    for (int r = 0; r < 4; r++) {
-        kinc[r] = mod_once(last_e[r] * (32u * U), M, rcpM);
-#pragma unroll
-        for (int u = 0; u < U; u++) kc[r][u] = mod_once(last_lc[r] + last_e[r] * lterm[u], M, rcpM);
-    }
-
-    uint32_t acc = 0, n_odd = 0, n_nz = 0, passes = 0;      // acc: low half counts odd logs, high half nonzero values
-    for (uint32_t base = 0; base < S; base += 32u * U) {
-        uint32_t l[U][4];
-        uint32_t mx = 0;                                     // some value is zero  <=>  mx >= M
-#pragma unroll
-        for (int r = 0; r < 4; r++) {
-            if (!(have & (1u << r))) {                       // warp-uniform: no term with exponent = r mod 4
-#pragma unroll
-                for (int u = 0; u < U; u++) l[u][r] = kBigZero;
-                mx = kBigZero;
-                continue;
-            }
-            uint32_t v[U];
-#pragma unroll
-            for (int u = 0; u < U; u++) v[u] = 0u;           // W_1 = log 1
-#pragma unroll
-            for (int i = NT - 1; i >= 0; i--) {
-                if ((i & 3) != r) continue;
-                if (cm & (1u << i)) {
-                    const uint32_t ubi = ub[i], m = gap[i];
-#pragma unroll
-                    for (int u = 0; u < U; u++) v[u] = pol.step(v[u], m * lterm[u] + ubi);
-                    ub[i] = pol.ub_next(ubi, inc[i]);
-                }
-            }
-#pragma unroll
-            for (int u = 0; u < U; u++) {
-                l[u][r] = wrap_once(v[u] + kc[r][u], M);     // a zero chain (v = Z0) stays >= M
-                kc[r][u] = wrap_once(kc[r][u] + kinc[r], M);
-                mx = max(mx, l[u][r]);
-            }
-        }
-        uint32_t t[U][4];
-        if (!__any_sync(0xffffffffu, mx >= M)) {
-            mx = 0;
-#pragma unroll
-            for (int u = 0; u < U; u++) {
-                uint32_t za, zs;
-                zech_add_sub(pol, M, hM, l[u][0], l[u][2], 0u, za, zs);
-                t[u][0] = wrap_once(l[u][0] + za, M);
-                t[u][1] = wrap_once(l[u][0] + zs, M);
-                zech_add_sub(pol, M, hM, l[u][1], l[u][3], 0u, za, zs);
-                t[u][2] = wrap_once(l[u][1] + za, M);
-                t[u][3] = wrap_once(l[u][1] + zs, M);
-                mx = max(max(mx, max(t[u][0], t[u][1])), max(t[u][2], t[u][3]));
-            }
-        } else {
-#pragma unroll
-            for (int u = 0; u < U; u++) {
-                zech_add_sub_any(pol, M, hM, l[u][0], l[u][2], 0u, t[u][0], t[u][1]);
-                zech_add_sub_any(pol, M, hM, l[u][1], l[u][3], 0u, t[u][2], t[u][3]);
-            }
-            mx = kBigZero;
-        }
-        if (!__any_sync(0xffffffffu, mx >= M)) {
-#pragma unroll
-            for (int u = 0; u < U; u++) {
-                const bool valid = base + lane + 32u * u < S;
-#pragma unroll
-                for (int h = 0; h < 2; h++) {
-                    const uint32_t a = t[u][h], b = t[u][2 + h];
-                    uint32_t z[2];
-                    zech_add_sub(pol, M, hM, a, b, h ? qM : 0u, z[0], z[1]);   // h = 1: t1 +- i t3
-#pragma unroll
-                    for (int j = 0; j < 2; j++)
-                        if (valid && z[j] < M) acc += ((a ^ z[j]) & 1u) + 0x10000u;    // log f = a + Z (M is even)
-                }
-            }
-        } else {
-#pragma unroll
-            for (int u = 0; u < U; u++) {
-                const bool valid = base + lane + 32u * u < S;
-#pragma unroll
-                for (int h = 0; h < 2; h++) {
-                    uint32_t w[2];
-                    zech_add_sub_any(pol, M, hM, t[u][h], t[u][2 + h], h ? qM : 0u, w[0], w[1]);
-#pragma unroll
-                    for (int j = 0; j < 2; j++)
-                        if (valid && w[j] < M) acc += (w[j] & 1u) + 0x10000u;
-                }
-            }
-        }
-        if ((++passes & 2047u) == 0u) { n_odd += acc & 0xFFFFu; n_nz += acc >> 16; acc = 0; }   // <= 4 U per pass
-    }
-    n_odd += acc & 0xFFFFu;
-    n_nz += acc >> 16;
-    const uint32_t n_valid = 4u * ((S + 31u - lane) >> 5);
-    n_zero = n_valid - n_nz;
-    n_sq = n_nz - n_odd;
-}
-
-// One launch computes N_k for k_lo <= k <= k_hi.  Fields below k_hi use EXT16 tables; field k_hi uses TOP.
-// RADIX: fields with 4 | M whose table is an extended one are evaluated by radix4_all_x (UR cosets per lane per
-// pass); all other fields by horner_all_x (U points per lane per pass).
-template <int G, int U, int TOP, bool RADIX>
+// One launch computes N_k for k_lo <= k <= k_hi with one Horner chain per x (Algorithm 1 line 8):
+// the paper's evaluation scheme (HEC_EVAL_HORNER).  Fields below k_hi use EXT16 tables; field k_hi uses TOP.
+template <int G, int U, int TOP>
 __global__ void __launch_bounds__(kThreads, 1) hec_count_kernel(const __grid_constant__ HecCountParams P) {
     constexpr int D = 2 * G + 2;          // largest degree; coefficient slots 0..D
     constexpr int NC = D + 1;
-    constexpr int UR = 2;
     extern __shared__ uint4 smem_blob[];
 
     for (uint32_t i = threadIdx.x; i < P.blob_bytes / 16; i += blockDim.x) smem_blob[i] = P.blob[i];
@@ -382,20 +209,7 @@ __global__ void __launch_bounds__(kThreads, 1) hec_count_kernel(const __grid_con
             // ---- a3 + a4: f at every x != 0, classify, per-lane partial sums of
             //   n_zero = #{x != 0 : f(x) = 0},  n_sq = #{x != 0 : f(x) a nonzero square}      (reading G3)
             uint32_t n_zero, n_sq;
-            bool done = false;
-            if constexpr (RADIX) {
-                if ((M & 3u) == 0u && (TOP == HEC_TAB_EXT16 || TOP == HEC_TAB_GLOBAL32 || k < P.k_hi)) {
-                    if (TOP == HEC_TAB_EXT16 || k < P.k_hi) {
-                        const ExtTableS16 pol{smem_base + F.smem_off, M, F.z0};
-                        radix4_all_x<D, UR>(pol, M, F.rcpM, lane, nz, lcj, n_sq, n_zero);
-                    } else if constexpr (TOP == HEC_TAB_GLOBAL32) {
-                        const ExtTableG32 pol{F.gtab, M, F.z0};
-                        radix4_all_x<D, UR>(pol, M, F.rcpM, lane, nz, lcj, n_sq, n_zero);
-                    }
-                    done = true;
-                }
-            }
-            if (!done) {
+            {
                 uint32_t delta[D], incr[D], gap[D];
                 uint32_t nzmask = 0, prev_lc = 0, prev_e = 0;
                 bool started = false;
@@ -435,6 +249,81 @@ __global__ void __launch_bounds__(kThreads, 1) hec_count_kernel(const __grid_con
                 const uint32_t n_valid = (M + 31u - lane) >> 5;
                 const uint32_t flip = (prev_lc ^ (prev_e & lane)) & 1u;
                 n_sq = flip ? n_odd : n_valid - n_zero - n_odd;
+            }
+            const uint32_t r0 = __reduce_add_sync(0xffffffffu, n_zero);
+            const uint32_t rsq = __reduce_add_sync(0xffffffffu, n_sq);
+            // ---- a5: x = 0 (reading G15) and the points at infinity
+            const uint32_t lc0 = __shfl_sync(0xffffffffu, lcj, 0);
+            const uint32_t lcD = __shfl_sync(0xffffffffu, lcj, D);
+            const uint32_t x0 = (nz & 1u) == 0 ? 1u : ((lc0 & 1u) ? 0u : 2u);
+            const uint32_t inf = ((nz >> D) & 1u) == 0 ? 1u : ((lcD & 1u) ? 0u : 2u);
+            const uint32_t Nk = r0 + 2u * rsq + x0 + inf;
+            if (lane + 1 == k) my_count = Nk;
+        }
+        if (mine) P.out[curve * G + lane] = my_count;
+    }
+}
+
+// One launch of the radix-R evaluation (hec_radix.cuh; HEC_EVAL_AUTO) for k_lo <= k <= k_hi.  Fields below k_hi
+// use PAIR16 tables with the packed 16x2 arithmetic; field k_hi uses TOP.  Same mapping as above: persistent
+// CTAs, one warp per curve, the lanes stride the coset index n = log x < M / R.
+template <int D, typename Ar, typename Pol>
+__device__ __forceinline__ void radix_dispatch(const uint32_t R, const Pol pol, const uint32_t M, const uint32_t rcpM,
+                                               const uint32_t lane, const uint32_t nz, const uint32_t lcj,
+                                               volatile uint32_t *scratch, uint32_t &n_sq, uint32_t &n_zero) {
+    if (R == 8) hec_radix::radix_all_x<D, 8, Ar>(pol, M, rcpM, lane, nz, lcj, scratch, n_sq, n_zero);
+    else if (R == 4) hec_radix::radix_all_x<D, 4, Ar>(pol, M, rcpM, lane, nz, lcj, scratch, n_sq, n_zero);
+    else hec_radix::radix_all_x<D, 2, Ar>(pol, M, rcpM, lane, nz, lcj, scratch, n_sq, n_zero);
+}
+
+template <int G, int TOP>
+__global__ void __launch_bounds__(kThreads, 1) hec_count_radix_kernel(const __grid_constant__ HecCountParams P) {
+    constexpr int D = 2 * G + 2;
+    constexpr int NC = D + 1;
+    extern __shared__ uint4 smem_blob[];
+
+    for (uint32_t i = threadIdx.x; i < P.blob_bytes / 16; i += blockDim.x) smem_blob[i] = P.blob[i];
+    __syncthreads();
+
+    const uint32_t lane = threadIdx.x & 31u;
+    const uint32_t warp = threadIdx.x >> 5;
+    const unsigned long long stride = (unsigned long long)gridDim.x * kWarps;
+    const uint32_t smem_base = (uint32_t)__cvta_generic_to_shared(smem_blob);
+    volatile uint32_t *scratch = reinterpret_cast<volatile uint32_t *>(reinterpret_cast<char *>(smem_blob) + P.scratch_off) +
+                                 warp * hec_radix::kScratchWords;
+
+    for (unsigned long long curve = (unsigned long long)blockIdx.x * kWarps + warp; curve < P.n; curve += stride) {
+        // ---- a2: coefficient load (lane j holds c_j) and boundary checks (readings G13, hec.h)
+        uint32_t cj = 0;
+        if (lane < NC) cj = P.coeffs[curve * NC + lane];
+        const bool bad_range = __any_sync(0xffffffffu, cj >= P.q);
+        const uint32_t nz = __ballot_sync(0xffffffffu, cj != 0);
+        const bool mine = lane + 1 >= P.k_lo && lane + 1 <= P.k_hi;
+        if (bad_range || (nz >> (D - 1)) == 0) {
+            if (lane == 0) atomicMin(&P.err[bad_range ? 0 : 1], curve);
+            if (mine) P.out[curve * G + lane] = 0;
+            continue;
+        }
+        uint32_t my_count = 0;   // lane k-1 keeps N_k
+#pragma unroll 1
+        for (uint32_t k = P.k_lo; k <= P.k_hi; k++) {
+            const HecFieldDev &F = P.f[k - 1];
+            const uint32_t M = F.M;
+            const uint32_t lcj = (lane < NC && cj != 0) ? __ldg(F.emb + cj) : 0u;     // reading G6
+            // ---- a3 + a4 (reading G3)
+            uint32_t n_zero, n_sq;
+            if (TOP == HEC_TAB_PAIR16 || k < P.k_hi) {
+                const hec_radix::PairS16 pol{smem_base + F.smem_off};
+                radix_dispatch<D, hec_radix::ArPacked>(F.radix, pol, M, F.rcpM, lane, nz, lcj, scratch, n_sq, n_zero);
+            } else if constexpr (TOP == HEC_TAB_RHALF32) {
+                const hec_radix::HalfS32 pol{smem_base + F.smem_off, smem_base + F.smem_off + 4u * (M >> 1)};
+                radix_dispatch<D, hec_radix::ArScalar>(F.radix, pol, M, F.rcpM, lane, nz, lcj, scratch, n_sq, n_zero);
+            } else if constexpr (TOP == HEC_TAB_RHALF17) {
+                const hec_radix::HalfS17 pol{smem_base + F.smem_off, smem_base + F.smem_off + 2u * (M >> 1), smem_base + F.smem_off2};
+                radix_dispatch<D, hec_radix::ArScalar>(F.radix, pol, M, F.rcpM, lane, nz, lcj, scratch, n_sq, n_zero);
+            } else if constexpr (TOP == HEC_TAB_GPAIR64) {
+                const hec_radix::PairG64 pol{reinterpret_cast<const uint2 *>(F.gtab)};
+                radix_dispatch<D, hec_radix::ArScalar>(F.radix, pol, M, F.rcpM, lane, nz, lcj, scratch, n_sq, n_zero);
             }
             const uint32_t r0 = __reduce_add_sync(0xffffffffu, n_zero);
             const uint32_t rsq = __reduce_add_sync(0xffffffffu, n_sq);
@@ -532,11 +421,12 @@ struct LaunchPlan {
     int top_mode = HEC_TAB_EXT16;
     const uint4 *blob = nullptr;      // device image of this launch's shared-memory tables
     uint32_t blob_bytes = 0;          // multiple of 16
-    uint32_t smem_bytes = 16;
+    uint32_t smem_bytes = 16;         // dynamic shared memory of the launch (blob + radix scratch)
 };
 
 struct DevicePlan {
     uint32_t q = 0, g = 0, p = 0, r = 0;
+    bool radix = false;               // tables of the radix-R evaluation (hec_radix.cuh) or of the Horner kernel
     int top_mode = HEC_TAB_EXT16;     // table mode of the largest field
     int U = 4;
     void *d_blob = nullptr;           // all device tables in one allocation
@@ -556,7 +446,7 @@ struct LibState {
     cudaStream_t stream = nullptr;
     int regime = HEC_REGIME_AUTO;
     int eval = HEC_EVAL_AUTO;
-    std::map<std::tuple<uint32_t, uint32_t, int>, std::unique_ptr<DevicePlan>> plans;
+    std::map<std::tuple<uint32_t, uint32_t, int, int>, std::unique_ptr<DevicePlan>> plans;
     hec_count_stats stats{};
     cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};
     // staging buffers for host-pointer calls
@@ -627,12 +517,47 @@ void fill_half24(const hec_field &F, uint32_t M, uint16_t *lo, int8_t *hi) {
     }
 }
 
+// Tables of the radix evaluation (hec_radix.cuh "Table policies").  A vanishing sum (the paper's sentinel,
+// PAPER.md:254) is stored as 0, a value Z never takes otherwise.
+uint32_t zech0(const hec_field &F, uint32_t M, uint32_t n) { const uint32_t z = F.zech[n]; return z == M ? 0u : z; }
+void fill_pair16(const hec_field &F, uint32_t M, uint32_t *out) {
+    const uint32_t h = M >> 1;
+    for (uint32_t n = 0; n < M; n++) out[n] = zech0(F, M, n) | (zech0(F, M, n + h >= M ? n + h - M : n + h) << 16);
+}
+void fill_gpair64(const hec_field &F, uint32_t M, uint32_t *out) {
+    const uint32_t h = M >> 1;
+    for (uint32_t n = 0; n < M; n++) { out[2 * n] = zech0(F, M, n); out[2 * n + 1] = zech0(F, M, n + h >= M ? n + h - M : n + h); }
+}
+void fill_rhalf32(const hec_field &F, uint32_t M, uint32_t *out) {
+    for (uint32_t i = 0; i <= (M >> 1); i++) out[i] = zech0(F, M, i);
+}
+void fill_rhalf17(const hec_field &F, uint32_t M, uint16_t *lo, uint8_t *bits) {
+    const uint32_t h = M >> 1;
+    for (uint32_t i = 0; i <= h; i++) {
+        lo[i] = (uint16_t)(zech0(F, M, i) & 0xFFFFu);
+        bits[i] = (uint8_t)(((zech0(F, M, i) >> 16) & 1u) | (((zech0(F, M, h - i) >> 16) & 1u) << 1));
+    }
+}
+
 // Smallest field for which the half-table step is valid: the lane term must stay below h (kernel comment).
 constexpr uint32_t kHalfMinM = 1u << 13;
 constexpr uint32_t kHalf24MaxM = 1u << 22;      // |Z - h| < 127 * 65536
+constexpr uint32_t kRadixScratchBytes = kWarps * hec_radix::kScratchWords * 4u;
 
-int build_plan(LibState &S, uint32_t q, uint32_t g, int regime, DevicePlan **out) {
-    auto key = std::make_tuple(q, g, regime);
+// Radix of one field: the largest R in {2, 4, 8} with R | M, capped by the evaluation scheme.  Measured on B200
+// (profiles/): with a pair table one entry serves both butterfly outputs, so R = 8 wins; with a half table a
+// pair costs two (three) loads and R = 4 is the better trade for the short chains of genus 2.
+uint32_t pick_radix(uint32_t M, int eval, int mode, uint32_t g) {
+    uint32_t cap = eval == HEC_EVAL_RADIX2 ? 2u : eval == HEC_EVAL_RADIX4 ? 4u : 8u;
+    if (eval == HEC_EVAL_AUTO && mode == HEC_TAB_RHALF32 && g <= 2) cap = 4u;
+    uint32_t R = 2;
+    while (R < cap && M % (2u * R) == 0) R *= 2u;
+    return R;
+}
+
+int build_plan(LibState &S, uint32_t q, uint32_t g, int regime, int eval, DevicePlan **out) {
+    const bool radix = eval != HEC_EVAL_HORNER;
+    auto key = std::make_tuple(q, g, regime, eval);
     auto it = S.plans.find(key);
     if (it != S.plans.end()) { *out = it->second.get(); return HEC_OK; }
 
@@ -642,10 +567,12 @@ int build_plan(LibState &S, uint32_t q, uint32_t g, int regime, DevicePlan **out
     for (uint32_t i = 0; i < g; i++) { Qg *= q; if (Qg > HEC_MAX_FIELD_SIZE) HEC_FAIL(HEC_ERR_INVALID_FIELD, "q^g exceeds HEC_MAX_FIELD_SIZE (2^26)"); }
 
     std::unique_ptr<DevicePlan> plan(new DevicePlan);
-    plan->q = q; plan->g = g; plan->p = p; plan->r = r;
+    plan->q = q; plan->g = g; plan->p = p; plan->r = r; plan->radix = radix;
     const uint32_t D = 2 * g + 2;
     const uint32_t U = (uint32_t)plan->U;
-    const uint32_t budget = (uint32_t)S.smem_optin - 1024u;
+    const uint32_t budget = (uint32_t)S.smem_optin - 1024u - (radix ? kRadixScratchBytes : 0u);
+    const int base_mode = radix ? HEC_TAB_PAIR16 : HEC_TAB_EXT16;      // layout of the fields below the top of a launch
+    const int global_mode = radix ? HEC_TAB_GPAIR64 : HEC_TAB_GLOBAL32;
 
     std::vector<const hec_field *> fields(g);
     std::vector<hec_table_geom> geom(g);
@@ -655,20 +582,39 @@ int build_plan(LibState &S, uint32_t q, uint32_t g, int regime, DevicePlan **out
         geom[k - 1] = table_geom(fields[k - 1]->Q - 1, D, U);
     }
     // ---- table mode of every field and the grouping into launches (one shared-memory image per launch)
-    auto ext16_bytes = [&](uint32_t k) -> uint32_t {
+    auto mode_bytes = [&](uint32_t k, int mode) -> uint32_t {      // 0: the layout cannot hold this field
         const hec_table_geom &t = geom[k - 1];
-        if ((uint64_t)t.lmax + t.M > 65535u) return 0;               // Z0 = M + LP must fit 16 bits
-        const uint64_t b = (uint64_t)t.entries * 2u;
+        const uint32_t M = t.M;
+        uint64_t b = 0;
+        switch (mode) {
+            case HEC_TAB_EXT16:
+                if ((uint64_t)t.lmax + t.M > 65535u) return 0;           // Z0 = M + LP must fit 16 bits
+                b = (uint64_t)t.entries * 2u;
+                break;
+            case HEC_TAB_HALF32:
+            case HEC_TAB_HALF24: {
+                if (M < kHalfMinM || (mode == HEC_TAB_HALF24 && M >= kHalf24MaxM)) return 0;
+                const uint64_t e = half_entries(M);
+                b = mode == HEC_TAB_HALF32 ? e * 4u : (uint64_t)align16((uint32_t)(e * 2u)) + e;
+                break;
+            }
+            case HEC_TAB_PAIR16:
+                if (M > 32768u) return 0;                                 // both halves of a packed value stay below 2 M <= 65536
+                b = (uint64_t)M * 4u;
+                break;
+            case HEC_TAB_RHALF32:
+                b = ((uint64_t)(M >> 1) + 1u) * 4u;
+                break;
+            case HEC_TAB_RHALF17:
+                if (M >= (1u << 17)) return 0;
+                b = (uint64_t)align16(((M >> 1) + 1u) * 2u) + (M >> 1) + 1u;
+                break;
+            default:
+                return 1u;                                                // global tables take no shared memory
+        }
         return b <= budget ? align16((uint32_t)b) : 0;
     };
-    auto half_bytes = [&](uint32_t k, int mode) -> uint32_t {
-        const uint32_t M = geom[k - 1].M;
-        if (M < kHalfMinM || (mode == HEC_TAB_HALF24 && M >= kHalf24MaxM)) return 0;
-        const uint64_t e = half_entries(M);
-        const uint64_t b = mode == HEC_TAB_HALF32 ? e * 4u : (uint64_t)align16((uint32_t)(e * 2u)) + e;
-        return b <= budget ? align16((uint32_t)b) : 0;
-    };
-    std::vector<int> mode(g, HEC_TAB_EXT16);
+    std::vector<int> mode(g, base_mode);
     std::vector<uint32_t> bytes(g, 0);
     for (uint32_t k = 1; k <= g; k++) {
         const bool top = k == g;
@@ -676,23 +622,23 @@ int build_plan(LibState &S, uint32_t q, uint32_t g, int regime, DevicePlan **out
         uint32_t b = 0;
         auto try_mode = [&](int cand) {
             if (m >= 0) return;
-            const uint32_t cb = cand == HEC_TAB_EXT16 ? ext16_bytes(k) : cand == HEC_TAB_GLOBAL32 ? 1u : half_bytes(k, cand);
-            if (cb) { m = cand; b = cand == HEC_TAB_GLOBAL32 ? 0u : cb; }
+            const uint32_t cb = mode_bytes(k, cand);
+            if (cb) { m = cand; b = cand == global_mode ? 0u : cb; }
         };
+        const int half_a = radix ? HEC_TAB_RHALF32 : HEC_TAB_HALF32, half_b = radix ? HEC_TAB_RHALF17 : HEC_TAB_HALF24;
         if (top && regime == HEC_REGIME_L2) {
-            try_mode(HEC_TAB_GLOBAL32);
+            try_mode(global_mode);
         } else if (top && regime == HEC_REGIME_SMEM) {
-            try_mode(HEC_TAB_EXT16);
-            if (m < 0) HEC_FAIL(HEC_ERR_INVALID_ARG, "HEC_REGIME_SMEM: the extended Zech table of the largest field does not fit shared memory");
+            try_mode(base_mode);
+            if (m < 0) HEC_FAIL(HEC_ERR_INVALID_ARG, "HEC_REGIME_SMEM: the full Zech table of the largest field does not fit shared memory");
         } else if (top && regime == HEC_REGIME_SMEM_HALF) {
-            try_mode(HEC_TAB_HALF32);
-            try_mode(HEC_TAB_HALF24);
+            if (geom[k - 1].M >= kHalfMinM) { try_mode(half_a); try_mode(half_b); }
             if (m < 0) HEC_FAIL(HEC_ERR_INVALID_ARG, "HEC_REGIME_SMEM_HALF: the half table of the largest field does not fit shared memory (or the field is below 2^13 elements)");
         } else {
-            try_mode(HEC_TAB_EXT16);
-            try_mode(HEC_TAB_HALF32);
-            try_mode(HEC_TAB_HALF24);
-            try_mode(HEC_TAB_GLOBAL32);
+            try_mode(base_mode);
+            try_mode(half_a);
+            try_mode(half_b);
+            try_mode(global_mode);
         }
         mode[k - 1] = m;
         bytes[k - 1] = b;
@@ -706,12 +652,12 @@ int build_plan(LibState &S, uint32_t q, uint32_t g, int regime, DevicePlan **out
             if (cur.k_hi >= cur.k_lo && cur.smem + bytes[k - 1] > budget) { groups.push_back(cur); cur = Group{k, 0, 0}; }
             cur.k_hi = k;
             cur.smem += bytes[k - 1];
-            if (mode[k - 1] != HEC_TAB_EXT16) { groups.push_back(cur); cur = Group{k + 1, 0, 0}; }   // only the top of a launch may differ
+            if (mode[k - 1] != base_mode) { groups.push_back(cur); cur = Group{k + 1, 0, 0}; }   // only the top of a launch may differ
         }
         if (cur.k_hi >= cur.k_lo) groups.push_back(cur);
     }
 
-    // ---- one device allocation: [launch blobs][global 32-bit tables][embed tables][squarefree tables]
+    // ---- one device allocation: [launch blobs][global tables][embed tables][squarefree tables]
     std::vector<uint8_t> host;
     auto reserve = [&](size_t nbytes) { size_t o = host.size(); host.resize(o + ((nbytes + 255) & ~(size_t)255)); return o; };
     std::vector<size_t> blob_off(groups.size()), gtab_off(g, 0), emb_off(g, 0);
@@ -724,7 +670,8 @@ int build_plan(LibState &S, uint32_t q, uint32_t g, int regime, DevicePlan **out
             HecFieldDev &fd = plan->f[k - 1];
             fd.M = t.M; fd.mode = (uint32_t)mode[k - 1]; fd.z0 = t.M + t.lmax; fd.rcpM = (uint32_t)((1ull << 32) / t.M);
             fd.lane_cap = std::min<uint32_t>(32u * U, t.M);
-            fd.smem_off = so; fd.smem_off2 = 0; fd.pad_ = 0; fd.gtab = nullptr;
+            fd.smem_off = so; fd.smem_off2 = 0; fd.gtab = nullptr;
+            fd.radix = radix ? pick_radix(t.M, eval, mode[k - 1], g) : 0u;
             uint8_t *dst = host.data() + blob_off[gi] + so;
             switch (mode[k - 1]) {
                 case HEC_TAB_EXT16:
@@ -739,6 +686,18 @@ int build_plan(LibState &S, uint32_t q, uint32_t g, int regime, DevicePlan **out
                     fill_half24(*fields[k - 1], t.M, reinterpret_cast<uint16_t *>(dst), reinterpret_cast<int8_t *>(dst + lo_bytes));
                     break;
                 }
+                case HEC_TAB_PAIR16:
+                    fill_pair16(*fields[k - 1], t.M, reinterpret_cast<uint32_t *>(dst));
+                    break;
+                case HEC_TAB_RHALF32:
+                    fill_rhalf32(*fields[k - 1], t.M, reinterpret_cast<uint32_t *>(dst));
+                    break;
+                case HEC_TAB_RHALF17: {
+                    const uint32_t lo_bytes = align16(((t.M >> 1) + 1u) * 2u);
+                    fd.smem_off2 = so + lo_bytes;
+                    fill_rhalf17(*fields[k - 1], t.M, reinterpret_cast<uint16_t *>(dst), dst + lo_bytes);
+                    break;
+                }
                 default:
                     break;
             }
@@ -750,6 +709,9 @@ int build_plan(LibState &S, uint32_t q, uint32_t g, int regime, DevicePlan **out
         if (mode[k - 1] == HEC_TAB_GLOBAL32) {
             gtab_off[k - 1] = reserve((size_t)t.entries * 4u);
             fill_extended<uint32_t>(*fields[k - 1], t, reinterpret_cast<uint32_t *>(host.data() + gtab_off[k - 1]));
+        } else if (mode[k - 1] == HEC_TAB_GPAIR64) {
+            gtab_off[k - 1] = reserve((size_t)t.M * 8u);
+            fill_gpair64(*fields[k - 1], t.M, reinterpret_cast<uint32_t *>(host.data() + gtab_off[k - 1]));
         }
         emb_off[k - 1] = reserve((size_t)q * 4u);
         uint32_t *e = reinterpret_cast<uint32_t *>(host.data() + emb_off[k - 1]);
@@ -768,11 +730,12 @@ int build_plan(LibState &S, uint32_t q, uint32_t g, int regime, DevicePlan **out
         L.top_mode = mode[L.k_hi - 1];
         L.blob = reinterpret_cast<const uint4 *>(base + blob_off[gi]);
         L.blob_bytes = align16(groups[gi].smem);
-        L.smem_bytes = std::max<uint32_t>(L.blob_bytes, 16u);
+        L.smem_bytes = std::max<uint32_t>(L.blob_bytes, 16u) + (radix ? kRadixScratchBytes : 0u);
         plan->launches.push_back(L);
     }
     for (uint32_t k = 1; k <= g; k++) {
-        plan->f[k - 1].gtab = mode[k - 1] == HEC_TAB_GLOBAL32 ? reinterpret_cast<const uint32_t *>(base + gtab_off[k - 1]) : nullptr;
+        const bool glob = mode[k - 1] == HEC_TAB_GLOBAL32 || mode[k - 1] == HEC_TAB_GPAIR64;
+        plan->f[k - 1].gtab = glob ? reinterpret_cast<const uint32_t *>(base + gtab_off[k - 1]) : nullptr;
         plan->f[k - 1].emb = reinterpret_cast<const uint32_t *>(base + emb_off[k - 1]);
     }
     plan->sq_zech = reinterpret_cast<const uint32_t *>(base + sqz_off);
@@ -783,9 +746,8 @@ int build_plan(LibState &S, uint32_t q, uint32_t g, int regime, DevicePlan **out
     return HEC_OK;
 }
 
-template <int G, int U, int TOP, bool RADIX>
-int launch_one(LibState &S, const LaunchPlan &L, const HecCountParams &P) {
-    auto kern = hec_count_kernel<G, U, TOP, RADIX>;
+template <typename Kern>
+int launch_kernel(LibState &S, Kern kern, const LaunchPlan &L, const HecCountParams &P, uint32_t chains) {
     HEC_CUDA_OK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)L.smem_bytes));
     uint32_t grid = (uint32_t)std::min<unsigned long long>((P.n + kWarps - 1) / kWarps, (unsigned long long)S.sm_count);
     if (grid == 0) grid = 1;
@@ -793,7 +755,7 @@ int launch_one(LibState &S, const LaunchPlan &L, const HecCountParams &P) {
     hec_launch_counter::value++;
     S.stats.grid = grid;
     S.stats.block = kThreads;
-    S.stats.chains_per_lane = U;
+    S.stats.chains_per_lane = chains;
     S.stats.smem_bytes = std::max(S.stats.smem_bytes, L.smem_bytes);
     S.stats.launches++;
     HEC_CUDA_OK(cudaGetLastError());
@@ -804,25 +766,21 @@ template <int G, int U>
 int launch_count(LibState &S, const DevicePlan &plan, HecCountParams P) {
     for (const LaunchPlan &L : plan.launches) {
         P.blob = L.blob; P.blob_bytes = L.blob_bytes; P.k_lo = L.k_lo; P.k_hi = L.k_hi;
+        P.scratch_off = std::max<uint32_t>(L.blob_bytes, 16u);
         int rc;
-        const bool radix = S.eval != HEC_EVAL_HORNER;
         switch (L.top_mode) {
-            case HEC_TAB_GLOBAL32:
-                rc = radix ? launch_one<G, U, HEC_TAB_GLOBAL32, true>(S, L, P) : launch_one<G, U, HEC_TAB_GLOBAL32, false>(S, L, P);
-                break;
-            case HEC_TAB_HALF32: rc = launch_one<G, U, HEC_TAB_HALF32, false>(S, L, P); break;
-            case HEC_TAB_HALF24: rc = launch_one<G, U, HEC_TAB_HALF24, false>(S, L, P); break;
-            default:
-                rc = radix ? launch_one<G, U, HEC_TAB_EXT16, true>(S, L, P) : launch_one<G, U, HEC_TAB_EXT16, false>(S, L, P);
-                break;
+            case HEC_TAB_GLOBAL32: rc = launch_kernel(S, hec_count_kernel<G, U, HEC_TAB_GLOBAL32>, L, P, U); break;
+            case HEC_TAB_HALF32: rc = launch_kernel(S, hec_count_kernel<G, U, HEC_TAB_HALF32>, L, P, U); break;
+            case HEC_TAB_HALF24: rc = launch_kernel(S, hec_count_kernel<G, U, HEC_TAB_HALF24>, L, P, U); break;
+            case HEC_TAB_EXT16: rc = launch_kernel(S, hec_count_kernel<G, U, HEC_TAB_EXT16>, L, P, U); break;
+            case HEC_TAB_PAIR16: rc = launch_kernel(S, hec_count_radix_kernel<G, HEC_TAB_PAIR16>, L, P, 2); break;
+            case HEC_TAB_RHALF32: rc = launch_kernel(S, hec_count_radix_kernel<G, HEC_TAB_RHALF32>, L, P, 1); break;
+            case HEC_TAB_RHALF17: rc = launch_kernel(S, hec_count_radix_kernel<G, HEC_TAB_RHALF17>, L, P, 1); break;
+            default: rc = launch_kernel(S, hec_count_radix_kernel<G, HEC_TAB_GPAIR64>, L, P, 1); break;
         }
         if (rc) return rc;
-        for (uint32_t k = L.k_lo; k <= L.k_hi; k++) {
-            const bool ext = plan.f[k - 1].mode == HEC_TAB_EXT16 || plan.f[k - 1].mode == HEC_TAB_GLOBAL32;
-            if (radix && ext && (L.top_mode == HEC_TAB_EXT16 || L.top_mode == HEC_TAB_GLOBAL32) && plan.f[k - 1].M % 4u == 0)
-                S.stats.radix4_fields |= 1u << (k - 1);
-        }
-        if (rc) return rc;
+        if (plan.radix)
+            for (uint32_t k = L.k_lo; k <= L.k_hi; k++) S.stats.radix_fields |= plan.f[k - 1].radix << (4u * (k - 1));
     }
     return HEC_OK;
 }
@@ -863,7 +821,7 @@ int hec_set_regime(int regime) {
 }
 
 int hec_set_eval(int eval) {
-    if (eval != HEC_EVAL_AUTO && eval != HEC_EVAL_HORNER) HEC_FAIL(HEC_ERR_INVALID_ARG, "unknown evaluation scheme");
+    if (eval != HEC_EVAL_AUTO && eval != HEC_EVAL_HORNER && eval != HEC_EVAL_RADIX2 && eval != HEC_EVAL_RADIX4 && eval != HEC_EVAL_RADIX8) HEC_FAIL(HEC_ERR_INVALID_ARG, "unknown evaluation scheme");
     std::lock_guard<std::mutex> lock(g_state.mu);
     g_state.eval = eval;
     return HEC_OK;
@@ -898,7 +856,7 @@ int hec_count(uint32_t q, uint32_t g, const uint16_t *coeffs, size_t n, uint32_t
     if (dev_in != dev_out || dev_sf != dev_out) HEC_FAIL(HEC_ERR_INVALID_ARG, "coeffs/out_counts/out_squarefree must all be host or all device pointers");
 
     DevicePlan *plan = nullptr;
-    rc = build_plan(S, q, g, S.regime, &plan);
+    rc = build_plan(S, q, g, S.regime, S.eval, &plan);
     if (rc) return rc;
 
     const size_t ncoef = 2 * (size_t)g + 3;
@@ -927,12 +885,13 @@ int hec_count(uint32_t q, uint32_t g, const uint16_t *coeffs, size_t n, uint32_t
 
     HecCountParams P;
     P.coeffs = d_coeffs; P.out = d_counts; P.n = n; P.q = q;
-    P.blob = nullptr; P.blob_bytes = 0; P.err = plan->d_err; P.k_lo = 1; P.k_hi = g;
+    P.blob = nullptr; P.blob_bytes = 0; P.err = plan->d_err; P.k_lo = 1; P.k_hi = g; P.scratch_off = 0;
     for (uint32_t k = 0; k < HEC_MAX_GENUS; k++) P.f[k] = plan->f[k < g ? k : 0];
 
     S.stats = hec_count_stats{};
     S.stats.table_mode = (uint32_t)plan->top_mode;
-    S.stats.regime = plan->top_mode == HEC_TAB_EXT16 ? HEC_REGIME_SMEM : plan->top_mode == HEC_TAB_GLOBAL32 ? HEC_REGIME_L2 : HEC_REGIME_SMEM_HALF;
+    S.stats.regime = (plan->top_mode == HEC_TAB_EXT16 || plan->top_mode == HEC_TAB_PAIR16) ? HEC_REGIME_SMEM
+                     : (plan->top_mode == HEC_TAB_GLOBAL32 || plan->top_mode == HEC_TAB_GPAIR64) ? HEC_REGIME_L2 : HEC_REGIME_SMEM_HALF;
     HEC_CUDA_OK(cudaEventRecord(S.ev[0], S.stream));
     switch (g) {
         case 1: rc = launch_count<1, 4>(S, *plan, P); break;
@@ -978,6 +937,7 @@ void hec_shutdown(void) {
     std::lock_guard<std::mutex> lock(g_state.mu);
     g_state.plans.clear();
     if (g_state.d_stage) { cudaFree(g_state.d_stage); g_state.d_stage = nullptr; g_state.stage_bytes = 0; }
+    hec_histogram_release_pool();
     hec_clear_field_cache();
 }
 

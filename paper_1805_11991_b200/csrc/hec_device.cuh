@@ -22,7 +22,12 @@ enum HecTableMode : uint32_t {
     HEC_TAB_GLOBAL32 = 0,   // extended table, 32-bit entries, global memory (L1/L2-resident regime)
     HEC_TAB_EXT16 = 1,      // extended table, 16-bit entries, shared memory
     HEC_TAB_HALF32 = 2,     // half table (Z(-n) = Z(n) - n), 32-bit entries, shared memory
-    HEC_TAB_HALF24 = 3      // half table, 16-bit low plane + signed 8-bit high plane, shared memory
+    HEC_TAB_HALF24 = 3,     // half table, 16-bit low plane + signed 8-bit high plane, shared memory
+    // tables of the radix-R evaluation (hec_radix.cuh): entries serve the pair (Z[n], Z[n + M/2])
+    HEC_TAB_PAIR16 = 4,     // M 32-bit entries (Z[n] | Z[n + M/2] << 16), shared memory, M <= 32768
+    HEC_TAB_RHALF32 = 5,    // Z[0 .. M/2], 32-bit entries, shared memory
+    HEC_TAB_RHALF17 = 6,    // Z[0 .. M/2]: 16-bit plane + byte plane with bit 16 of entries i and M/2 - i, shared memory, M < 2^17
+    HEC_TAB_GPAIR64 = 7     // M entries (Z[n], Z[n + M/2]) as two 32-bit words, global memory (L1/L2-resident regime)
 };
 
 // One field F_{q^k} as the count kernel sees it.
@@ -34,8 +39,8 @@ struct HecFieldDev {
     uint32_t smem_off;   // byte offset inside the launch's blob (16-byte aligned): table / low plane
     uint32_t smem_off2;  // HALF24: byte offset of the high plane
     uint32_t lane_cap;   // lanes with lane + 32u >= lane_cap use lane term 0 (they are masked out anyway)
-    uint32_t pad_;
-    const uint32_t *gtab;   // GLOBAL32: extended table in global memory
+    uint32_t radix;      // radix evaluation: R in {2, 4, 8}, the largest with R | M; 0 for the Horner tables
+    const uint32_t *gtab;   // GLOBAL32: extended table in global memory; GPAIR64: the pair table
     const uint32_t *emb;    // q entries: log in F_{q^k} of the embedded coefficient, HEC_LOG_ZERO for 0
 };
 
@@ -47,7 +52,9 @@ struct HecCountParams {
     uint32_t blob_bytes;           // multiple of 16
     const uint4 *blob;             // this launch's concatenated shared-memory tables
     unsigned long long *err;       // err[0] = first row with a coefficient >= q, err[1] = first row of degree < 2g+1
-    uint32_t k_lo, k_hi;           // this launch computes N_k for k_lo <= k <= k_hi; only field k_hi may be non-EXT16
+    uint32_t k_lo, k_hi;           // this launch computes N_k for k_lo <= k <= k_hi; only field k_hi may differ from the
+                                   // launch's base layout (EXT16 for the Horner kernel, PAIR16 for the radix kernel)
+    uint32_t scratch_off;          // radix kernel: byte offset (after the blob) of the per-warp scratch words
     HecFieldDev f[HEC_MAX_GENUS];
 };
 

@@ -4,6 +4,8 @@
 // aggregate in a per-CTA shared-memory hash table (shared-memory atomics), merge into a global hash table,
 // compact the occupied slots, LSD-radix-sort the distinct keys (ascending lexicographic order) and unpack.
 #include <algorithm>
+#include <map>
+#include <mutex>
 #include <vector>
 
 #include "hec_device.cuh"
@@ -212,16 +214,58 @@ __global__ void hist_unpack_kernel(const unsigned long long *keys, const unsigne
     out_mult[i] = cnt[i];
 }
 
-struct DeviceBuf {
-    void *p = nullptr;
-    ~DeviceBuf() { if (p) cudaFree(p); }
-    int alloc(size_t bytes) {
-        if (cudaMalloc(&p, std::max<size_t>(bytes, 16)) != cudaSuccess) { cudaGetLastError(); p = nullptr; HEC_FAIL(HEC_ERR_NOMEM, "device allocation failed in hec_histogram"); }
+// Device scratch comes from a small caching pool (best fit, grow-only, released by hec_shutdown): a call needs up to
+// ~1 GB of hash-table and sort buffers, and cudaMalloc/cudaFree of that size cost far more than the kernels.
+struct Pool {
+    std::mutex mu;
+    std::vector<std::pair<void *, size_t>> idle;
+    std::map<void *, size_t> live;
+    int get(size_t bytes, void **out) {
+        std::lock_guard<std::mutex> lock(mu);
+        size_t best = idle.size();
+        for (size_t i = 0; i < idle.size(); i++)
+            if (idle[i].second >= bytes && idle[i].second <= 2 * bytes + (1u << 20) && (best == idle.size() || idle[i].second < idle[best].second)) best = i;
+        if (best != idle.size()) {
+            *out = idle[best].first;
+            live[*out] = idle[best].second;
+            idle.erase(idle.begin() + (long)best);
+            return HEC_OK;
+        }
+        void *p = nullptr;
+        if (cudaMalloc(&p, bytes) != cudaSuccess) {
+            cudaGetLastError();
+            for (auto &b : idle) cudaFree(b.first);          // drop the cache and retry once
+            idle.clear();
+            if (cudaMalloc(&p, bytes) != cudaSuccess) { cudaGetLastError(); HEC_FAIL(HEC_ERR_NOMEM, "device allocation failed in hec_histogram"); }
+        }
+        live[p] = bytes;
+        *out = p;
         return HEC_OK;
     }
+    void put(void *p) {
+        std::lock_guard<std::mutex> lock(mu);
+        auto it = live.find(p);
+        if (it == live.end()) return;
+        idle.emplace_back(p, it->second);
+        live.erase(it);
+    }
+    void clear() {
+        std::lock_guard<std::mutex> lock(mu);
+        for (auto &b : idle) cudaFree(b.first);
+        idle.clear();
+    }
+};
+Pool g_pool;
+
+struct DeviceBuf {
+    void *p = nullptr;
+    ~DeviceBuf() { if (p) g_pool.put(p); }
+    int alloc(size_t bytes) { return g_pool.get(std::max<size_t>(bytes, 256), &p); }
 };
 
 }  // namespace
+
+void hec_histogram_release_pool() { g_pool.clear(); }
 
 static int histogram_impl(const uint32_t *counts, const uint8_t *mask, const uint64_t *weights, size_t n, uint32_t g,
                           uint32_t *out_tuples, uint64_t *out_mult, size_t cap, size_t *out_m) {

@@ -1,0 +1,432 @@
+// Radix-R evaluation of f at every x of F_{q^k}^x (not in the paper, which runs one
+// Horner chain per x: Algorithm 1 line 8).  f is still evaluated at EVERY x (Algorithm 1 line 7,
+// PAPER.md:141); the points are only grouped so that they share work.
+//
+// M = q^k - 1 is even, so for R in {2, 4, 8} with R | M the R-th roots of unity zeta^j = alpha^{j M/R} lie in the
+// field.  Split f(X) = sum_{r<R} X^r F_r(X^R) and put G_r(x) = x^r F_r(x^R).  The R points of the coset
+// x mu_R share the R values G_r:
+//     f(zeta^j x) = sum_r zeta^{jr} G_r(x)                     (an R-point DFT of (G_r) in Zech arithmetic)
+// * G_r: one relative Horner chain in x^R per residue class (hec_count.cu header): #terms - #classes lookups
+//   per coset instead of R * deg f.
+// * DFT: log2 R stages of R/2 butterflies (a, b) -> (a + w b, a - w b).  In Zech form (reading G5)
+//     a + w b = a (1 + w b / a) -> log a + Z[n],   a - w b -> log a + Z[n + M/2],   n = log b - log a + log w
+//   (-1 = alpha^{M/2}), so ONE table entry holding the pair (Z[n], Z[n + M/2]) serves both outputs.
+//   Decimation in frequency with the output twiddles deferred: value i carries a pending factor zeta^{pend[i]}
+//   that only enters the NEXT butterfly's log w, so no log is ever adjusted by itself.
+// * The last stage only classifies (zero / parity of the log, reading G4): parity(log a + Z) = parity(log a) ^ parity(Z).
+//
+// Zero handling without a branch or a select in the hot loop: the tables store 0
+// ("multiply by 1") where 1 + alpha^n = 0, so the fast path stays well formed; a running minimum over the
+// looked-up values (Z is never 0 otherwise) flags every coset in which some intermediate or final value
+// vanished.  Flagged cosets (about 1e-4 of the points) are queued per warp in shared memory and re-evaluated
+// 32 at a time by exact_coset(), a plain scalar Zech evaluation that treats the zero element explicitly.
+// Classes without any nonzero coefficient (G_r = 0 identically) are warp-uniform and take uniform branches.
+//
+// Two arithmetics: ArScalar (one coset per 32-bit register) for any table policy, and ArPacked (two cosets
+// per register in 16-bit halves, VIADD.16x2 / VIADDMNMX.U16x2 / VIMNMX3.U16x2) for 16-bit fields with 2 M <= 65536.
+#pragma once
+
+#include <cstdint>
+
+namespace hec_radix {
+
+constexpr uint32_t kZero = 0x40000000u;      // "the element is zero" in the exact path (any value >= M)
+constexpr int kQueueCap = 96;                // flagged cosets per warp: < 32 pending + <= 64 new per pass
+constexpr int kScratchWords = 16 + kQueueCap;   // per warp: logs of the coefficients + queue
+
+__device__ __forceinline__ uint32_t lds_u32(uint32_t addr) {
+    uint32_t r;
+    asm("ld.shared.u32 %0, [%1];" : "=r"(r) : "r"(addr));
+    return r;
+}
+__device__ __forceinline__ uint32_t lds_u16(uint32_t addr) {
+    uint16_t r;
+    asm("ld.shared.u16 %0, [%1];" : "=h"(r) : "r"(addr));
+    return r;
+}
+__device__ __forceinline__ uint32_t lds_u8(uint32_t addr) {
+    uint32_t r;
+    asm("ld.shared.u8 %0, [%1];" : "=r"(r) : "r"(addr));
+    return r;
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// Table policies.  pair(n): (Z[n], Z[n + h]) for n in [0, M), h = M/2; single(n): Z[n].  Where the sum is
+// zero (n = h for the first, n = 0 for the second) the returned value is unspecified-but-in-range: callers
+// test n.  pair_word (PairS16 only): both values in one 32-bit word, 0 where the sum is zero.
+// ---------------------------------------------------------------------------------------------------------
+
+// PAIR16: shared memory, M 32-bit entries, lo16 = Z[n], hi16 = Z[n + h]  (M <= 32768).
+struct PairS16 {
+    uint32_t tb;                                             // shared byte address of entry 0
+    __device__ __forceinline__ uint32_t pair_word(uint32_t n) const { return lds_u32(tb + 4u * n); }
+    __device__ __forceinline__ void pair(uint32_t n, uint32_t, uint32_t, uint32_t &za, uint32_t &zs) const {
+        const uint32_t w = pair_word(n);
+        za = w & 0xFFFFu;
+        zs = w >> 16;
+    }
+    __device__ __forceinline__ uint32_t single(uint32_t n, uint32_t, uint32_t) const { return lds_u16(tb + 4u * n); }
+};
+
+// RHALF32: shared memory, HT[i] = Z[i] for 0 <= i <= h (HT[h] = 0), 32-bit entries.  Z(-m) = Z(m) - m (reading
+// G16) gives Z[i + h] = HT[h - i] + i + h (mod M) for 0 <= i < h, so with i = n mod h the pair is
+// (HT[i], HT[h - i] + i + h), swapped when n >= h.
+struct HalfS32 {
+    uint32_t tb, tbh;                                        // shared byte addresses of HT[0] and HT[h]
+    __device__ __forceinline__ void pair(uint32_t n, uint32_t M, uint32_t h, uint32_t &za, uint32_t &zs) const {
+        const uint32_t i = min(n, n - h);
+        const uint32_t t1 = lds_u32(tb + 4u * i);
+        uint32_t t2 = lds_u32(tbh - 4u * i) + i + h;
+        t2 = min(t2, t2 - M);
+        const bool sw = n >= h;
+        za = sw ? t2 : t1;
+        zs = sw ? t1 : t2;
+    }
+    __device__ __forceinline__ uint32_t single(uint32_t n, uint32_t M, uint32_t h) const {
+        const uint32_t i = min(n, M - n);
+        const uint32_t t = lds_u32(tb + 4u * i);
+        const uint32_t u = t + n;
+        return n > h ? min(u, u - M) : t;
+    }
+};
+
+// RHALF17: as RHALF32 for M < 2^17: a 16-bit plane with the low halves of HT[0..h] and a byte plane whose
+// entry i holds bit 16 of HT[i] (bit 0) and of HT[h - i] (bit 1): three loads per pair.
+struct HalfS17 {
+    uint32_t tb, tbh, bb;                                    // 16-bit plane: HT[0], HT[h]; byte plane
+    __device__ __forceinline__ void pair(uint32_t n, uint32_t M, uint32_t h, uint32_t &za, uint32_t &zs) const {
+        const uint32_t i = min(n, n - h);
+        const uint32_t l1 = lds_u16(tb + 2u * i), l2 = lds_u16(tbh - 2u * i), b = lds_u8(bb + i);
+        const uint32_t t1 = l1 + ((b & 1u) << 16);
+        uint32_t t2 = l2 + ((b & 2u) << 15) + i + h;
+        t2 = min(t2, t2 - M);
+        const bool sw = n >= h;
+        za = sw ? t2 : t1;
+        zs = sw ? t1 : t2;
+    }
+    __device__ __forceinline__ uint32_t single(uint32_t n, uint32_t M, uint32_t h) const {
+        const uint32_t i = min(n, M - n);
+        const uint32_t t = lds_u16(tb + 2u * i) + ((lds_u8(bb + i) & 1u) << 16);
+        const uint32_t u = t + n;
+        return n > h ? min(u, u - M) : t;
+    }
+};
+
+// GPAIR64: global memory (L1/L2-resident regime), M entries (Z[n], Z[n + h]) as uint2.
+struct PairG64 {
+    const uint2 *t;
+    __device__ __forceinline__ void pair(uint32_t n, uint32_t, uint32_t, uint32_t &za, uint32_t &zs) const {
+        const uint2 w = __ldg(t + n);
+        za = w.x;
+        zs = w.y;
+    }
+    __device__ __forceinline__ uint32_t single(uint32_t n, uint32_t, uint32_t) const { return __ldg(&t[n].x); }
+};
+
+// ---------------------------------------------------------------------------------------------------------
+// Arithmetics of the fast path.  A value V holds LANES logs in [0, M).
+// ---------------------------------------------------------------------------------------------------------
+struct ArScalar {
+    static constexpr int LANES = 1;
+    uint32_t M, h;
+    __device__ __forceinline__ ArScalar(uint32_t M_) : M(M_), h(M_ >> 1) {}
+    __device__ __forceinline__ uint32_t rep(uint32_t c) const { return c; }
+    __device__ __forceinline__ uint32_t wrap(uint32_t x) const { return min(x, x - M); }              // [0, 2M) -> [0, M)
+    __device__ __forceinline__ uint32_t subm(uint32_t b, uint32_t a) const { return wrap(b + M - a); }
+    __device__ __forceinline__ uint32_t mn_init() const { return 0xFFFFFFFFu; }
+    template <typename Pol>
+    __device__ __forceinline__ void lookup_pair(const Pol &pol, uint32_t n, uint32_t &za, uint32_t &zs, uint32_t &mn) const {
+        pol.pair(n, M, h, za, zs);
+        mn = min(mn, min(n, n - h));                          // 0 iff n in {0, h}: one of the two sums vanished
+    }
+    template <typename Pol>
+    __device__ __forceinline__ uint32_t lookup_single(const Pol &pol, uint32_t n, uint32_t &mn) const {
+        mn = min(mn, n ^ h);
+        return pol.single(n, M, h);
+    }
+    __device__ __forceinline__ uint32_t parity2(uint32_t a, uint32_t za, uint32_t zs) const { return ((a ^ za) & 1u) + ((a ^ zs) & 1u); }
+    __device__ __forceinline__ uint32_t parity1(uint32_t a) const { return a & 1u; }
+    __device__ __forceinline__ bool flagged(uint32_t mn, int) const { return mn == 0u; }
+    __device__ __forceinline__ uint32_t keep(uint32_t v, bool k0, bool) const { return k0 ? v : 0u; }
+    __device__ __forceinline__ uint32_t total(uint32_t v) const { return v; }
+    __device__ __forceinline__ uint32_t join(uint32_t a, uint32_t) const { return a; }
+};
+
+struct ArPacked {
+    static constexpr int LANES = 2;
+    uint32_t M2, nM2, h2;
+    __device__ __forceinline__ ArPacked(uint32_t M_) : M2(M_ * 0x10001u), nM2(((0x10000u - M_) & 0xFFFFu) * 0x10001u), h2((M_ >> 1) * 0x10001u) {}
+    __device__ __forceinline__ uint32_t rep(uint32_t c) const { return c * 0x10001u; }
+    __device__ __forceinline__ uint32_t wrap(uint32_t x) const { return __viaddmin_u16x2(x, nM2, x); }
+    __device__ __forceinline__ uint32_t subm(uint32_t b, uint32_t a) const { return wrap(b + M2 - a); }   // halves stay in (0, 2M): no borrow
+    __device__ __forceinline__ uint32_t mn_init() const { return 0xFFFFFFFFu; }
+    __device__ __forceinline__ void lookup_pair(const PairS16 &pol, uint32_t n, uint32_t &za, uint32_t &zs, uint32_t &mn) const {
+        const uint32_t w0 = pol.pair_word(n & 0xFFFFu), w1 = pol.pair_word(n >> 16);
+        za = __byte_perm(w0, w1, 0x5410);
+        zs = __byte_perm(w0, w1, 0x7632);
+        mn = __vimin3_u16x2(mn, za, zs);                      // a stored 0 marks a vanished sum (per coset: per half)
+    }
+    __device__ __forceinline__ uint32_t lookup_single(const PairS16 &pol, uint32_t n, uint32_t &mn) const {
+        const uint32_t z0 = pol.single(n & 0xFFFFu, 0, 0), z1 = pol.single(n >> 16, 0, 0);
+        const uint32_t z = __byte_perm(z0, z1, 0x5410);
+        mn = __vminu2(mn, z);
+        return z;
+    }
+    __device__ __forceinline__ uint32_t parity2(uint32_t a, uint32_t za, uint32_t zs) const {
+        return ((a ^ za) & 0x10001u) + ((a ^ zs) & 0x10001u);
+    }
+    __device__ __forceinline__ uint32_t parity1(uint32_t a) const { return a & 0x10001u; }
+    __device__ __forceinline__ bool flagged(uint32_t mn, int c) const { return c ? (mn >> 16) == 0u : (mn & 0xFFFFu) == 0u; }
+    __device__ __forceinline__ uint32_t keep(uint32_t v, bool k0, bool k1) const { return v & ((k0 ? 0xFFFFu : 0u) | (k1 ? 0xFFFF0000u : 0u)); }
+    __device__ __forceinline__ uint32_t total(uint32_t v) const { return (v & 0xFFFFu) + (v >> 16); }
+    __device__ __forceinline__ uint32_t join(uint32_t a, uint32_t b) const { return a | (b << 16); }
+};
+
+// ---------------------------------------------------------------------------------------------------------
+// Exact evaluation of one coset (the rare path).  lc[i] = log of c_i in this field (entries with bit i of nz
+// clear are not read).  Returns (#nonzero values << 16) | #nonzero values with odd log among f(zeta^j x), j < R.
+// ---------------------------------------------------------------------------------------------------------
+template <int D, int R, typename Pol>
+__device__ __noinline__ uint32_t exact_coset(const Pol pol, const uint32_t M, const uint32_t nz, const volatile uint32_t *lc, const uint32_t n) {
+    const uint32_t h = M >> 1, unit = M / R;
+    auto wrap = [M](uint32_t x) { return min(x, x - M); };
+    uint32_t v[R];
+    int pend[R];
+    for (int r = 0; r < R; r++) {
+        uint32_t acc = kZero;
+        for (int i = r + R * ((D - r) / R); i >= r; i -= R) {
+            if (acc < M) acc = wrap(acc + R * n);                          // acc * x^R;  R n < M
+            if ((nz >> i) & 1u) {                                          // acc + c_i
+                const uint32_t b = lc[i];
+                if (acc >= M) {
+                    acc = b;
+                } else {
+                    const uint32_t dd = wrap(b + M - acc);
+                    acc = dd == h ? kZero : wrap(acc + pol.single(dd, M, h));
+                }
+            }
+        }
+        if (acc < M) acc = wrap(acc + r * n);                              // G_r = x^r F_r(x^R);  r n < M
+        v[r] = acc;
+        pend[r] = 0;
+    }
+    for (int H = R / 2; H >= 1; H >>= 1)
+        for (int blk = 0; blk < R; blk += 2 * H)
+            for (int j = 0; j < H; j++) {
+                const int i1 = blk + j, i2 = i1 + H;
+                const uint32_t off = (uint32_t)((pend[i2] - pend[i1]) & (R - 1)) * unit;
+                pend[i2] = (pend[i1] + j * (R / (2 * H))) & (R - 1);
+                const uint32_t a = v[i1], b = v[i2];
+                uint32_t s, d;
+                if (a < M && b < M) {
+                    const uint32_t dd = wrap(wrap(b + M - a) + off);
+                    uint32_t za, zs;
+                    pol.pair(dd, M, h, za, zs);
+                    s = dd == h ? kZero : wrap(a + za);
+                    d = dd == 0 ? kZero : wrap(a + zs);
+                } else if (a < M) {
+                    s = a; d = a;
+                } else if (b < M) {
+                    s = wrap(b + off);
+                    d = wrap(s + h);
+                } else {
+                    s = kZero; d = kZero;
+                }
+                v[i1] = s;
+                v[i2] = d;
+            }
+    uint32_t res = 0;
+    for (int i = 0; i < R; i++)
+        if (v[i] < M) res += 0x10000u + (v[i] & 1u);                       // every final pending twiddle is zeta^0
+    return res;
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// The butterfly network of the fast path on LANES cosets at once.  present: bit r set iff G_r is not
+// identically zero (warp-uniform; some G_r is present because the leading coefficient is nonzero, so no final
+// value is identically zero).  Adds to ps the number of odd logs among the values (per lane of V) and folds the
+// zero indicator of every lookup into mn.
+// ---------------------------------------------------------------------------------------------------------
+template <int R, bool ALL, typename Ar, typename Pol>
+__device__ __forceinline__ void network(const Ar &ar, const Pol &pol, const uint32_t unit, uint32_t present,
+                                        uint32_t (&v)[R], uint32_t &ps, uint32_t &mn) {
+    int pend[R];
+#pragma unroll
+    for (int i = 0; i < R; i++) pend[i] = 0;
+#pragma unroll
+    for (int H = R / 2; H >= 1; H >>= 1) {
+#pragma unroll
+        for (int blk = 0; blk < R; blk += 2 * H) {
+#pragma unroll
+            for (int j = 0; j < H; j++) {
+                const int i1 = blk + j, i2 = i1 + H;
+                const int oe = (pend[i2] - pend[i1]) & (R - 1);
+                pend[i2] = (pend[i1] + j * (R / (2 * H))) & (R - 1);
+                const bool pa = ALL || ((present >> i1) & 1u), pb = ALL || ((present >> i2) & 1u);
+                if (pa && pb) {
+                    uint32_t n = ar.subm(v[i2], v[i1]);
+                    if (oe) n = ar.wrap(n + ar.rep((uint32_t)oe * unit));
+                    uint32_t za, zs;
+                    ar.lookup_pair(pol, n, za, zs, mn);
+                    const uint32_t a = v[i1];
+                    if (H > 1) {
+                        v[i1] = ar.wrap(a + za);
+                        v[i2] = ar.wrap(a + zs);
+                    } else {
+                        ps += ar.parity2(a, za, zs);
+                    }
+                } else if (pa) {                                           // b = 0: both outputs are a
+                    if (H > 1) v[i2] = v[i1];
+                    else ps += 2u * ar.parity1(v[i1]);
+                } else if (pb) {                                           // a = 0: w b and -w b
+                    uint32_t t = v[i2];
+                    if (oe) t = ar.wrap(t + ar.rep((uint32_t)oe * unit));
+                    const uint32_t u = ar.wrap(t + ar.rep(unit * (R / 2)));
+                    if (H > 1) { v[i1] = t; v[i2] = u; }
+                    else ps += ar.parity1(t) + ar.parity1(u);
+                }
+                if (!ALL && (pa || pb)) present |= (1u << i1) | (1u << i2);
+            }
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// All x in F_{q^k}^x for one curve, one warp.  lcj: lane j holds the log of c_j in this field (any value when
+// c_j = 0), nz: bit j set iff c_j != 0, scratch: kScratchWords words of shared memory owned by this warp.
+// Returns this lane's share of n_zero = #{x != 0: f(x) = 0} and n_sq = #{x != 0: f(x) a nonzero square}.
+// ---------------------------------------------------------------------------------------------------------
+template <int D, int R, typename Ar, typename Pol>
+__device__ __forceinline__ void radix_all_x(const Pol pol, const uint32_t M, const uint32_t rcpM, const uint32_t lane,
+                                            const uint32_t nz, const uint32_t lcj, volatile uint32_t *scratch,
+                                            uint32_t &n_sq, uint32_t &n_zero) {
+    constexpr int L = Ar::LANES;
+    constexpr int NT = D + 1 > R ? D + 1 - R : 0;      // terms 0 .. NT-1 can continue a chain
+    constexpr int NTA = NT > 0 ? NT : 1;
+    const Ar ar(M);
+    const uint32_t S = M / R, unit = S;
+    auto mod = [M, rcpM](uint32_t x) {                 // x mod M for any 32-bit x
+        const uint32_t r = x - __umulhi(x, rcpM) * M;
+        return r >= M ? r - M : r;
+    };
+
+    __syncwarp();
+    if (lane <= (uint32_t)D) scratch[lane] = lcj;
+    __syncwarp();
+
+    // ---- per-curve structure (warp-uniform) and this lane's chain offsets for its first cosets
+    uint32_t n0[L];
+#pragma unroll
+    for (int c = 0; c < L; c++) n0[c] = lane + 32u * c < S ? lane + 32u * c : 0u;
+    const uint32_t step = mod(32u * L);
+    uint32_t ul[NTA], inc[NTA], kc[R], kinc[R];
+    uint32_t cm = 0, present = 0;
+    uint32_t last_lc[R], last_e[R];
+#pragma unroll
+    for (int r = 0; r < R; r++) { last_lc[r] = 0; last_e[r] = 0; }
+#pragma unroll
+    for (int i = D; i >= 0; i--) {
+        const int r = i % R;
+        const uint32_t lci = __shfl_sync(0xffffffffu, lcj, i);
+        if (i < NT) { ul[i] = 0; inc[i] = 0; }
+        if (nz & (1u << i)) {
+            if (i < NT && (present & (1u << r))) {
+                const uint32_t m = last_e[r] - (uint32_t)i;
+                const uint32_t delta = last_lc[r] >= lci ? last_lc[r] - lci : last_lc[r] + M - lci;
+                uint32_t t[2] = {0, 0};
+#pragma unroll
+                for (int c = 0; c < L; c++) t[c] = mod(delta + m * n0[c]);
+                ul[i] = ar.join(t[0], t[1]);
+                inc[i] = ar.rep(mod(m * step));
+                cm |= 1u << i;
+            }
+            present |= 1u << r;
+            last_lc[r] = lci;
+            last_e[r] = (uint32_t)i;
+        }
+    }
+#pragma unroll
+    for (int r = 0; r < R; r++) {                      // log G_r = W_r + K_r(n), K_r(n) = log c_{e_T} + e_T n
+        uint32_t t[2] = {0, 0};
+#pragma unroll
+        for (int c = 0; c < L; c++) t[c] = mod(last_lc[r] + last_e[r] * n0[c]);
+        kc[r] = ar.join(t[0], t[1]);
+        kinc[r] = ar.rep(mod(last_e[r] * step));
+    }
+    const bool all_present = present == (1u << R) - 1u;
+
+    uint32_t acc = 0, odd_fast = 0, passes = 0, pushed = 0, qn = 0, nz_exact = 0, odd_exact = 0;
+    auto drain = [&]() {
+        for (uint32_t j = lane; j < qn; j += 32u) {
+            const uint32_t res = exact_coset<D, R>(pol, M, nz, scratch, scratch[16 + j]);
+            nz_exact += res >> 16;
+            odd_exact += res & 0xFFFFu;
+        }
+    };
+    for (uint32_t base = 0; base < S; base += 32u * L) {
+        uint32_t v[R];
+        uint32_t mn = ar.mn_init();
+#pragma unroll
+        for (int r = 0; r < R; r++) {
+            uint32_t w = 0;
+            bool chained = false;
+#pragma unroll
+            for (int i = NT - 1; i >= 0; i--) {
+                if (i % R != r) continue;
+                if (cm & (1u << i)) {
+                    const uint32_t n = chained ? ar.wrap(w + ul[i]) : ul[i];
+                    w = ar.lookup_single(pol, n, mn);
+                    ul[i] = ar.wrap(ul[i] + inc[i]);
+                    chained = true;
+                }
+            }
+            v[r] = chained ? ar.wrap(w + kc[r]) : kc[r];
+            kc[r] = ar.wrap(kc[r] + kinc[r]);
+        }
+        uint32_t ps = 0;
+        if (all_present) network<R, true>(ar, pol, unit, present, v, ps, mn);
+        else network<R, false>(ar, pol, unit, present, v, ps, mn);
+        bool valid[2] = {false, false}, flag[2] = {false, false};
+        bool any_flag = false;
+#pragma unroll
+        for (int c = 0; c < L; c++) {
+            valid[c] = base + lane + 32u * c < S;
+            flag[c] = valid[c] && ar.flagged(mn, c);
+            any_flag |= flag[c];
+        }
+        if (__any_sync(0xffffffffu, any_flag)) {       // rare: queue the flagged cosets for exact evaluation
+#pragma unroll
+            for (int c = 0; c < L; c++) {
+                const uint32_t bal = __ballot_sync(0xffffffffu, flag[c]);
+                if (flag[c]) {
+                    scratch[16 + qn + __popc(bal & ((1u << lane) - 1u))] = base + lane + 32u * c;
+                    pushed++;
+                }
+                qn += __popc(bal);
+            }
+            __syncwarp();
+            if (qn >= 32u) {
+                drain();
+                qn = 0;
+                __syncwarp();
+            }
+        }
+        acc += ar.keep(ps, valid[0] && !flag[0], valid[1] && !flag[1]);
+        if ((++passes & 1023u) == 0u) { odd_fast += ar.total(acc); acc = 0; }      // <= R per lane of V per pass
+    }
+    odd_fast += ar.total(acc);
+    drain();
+    __syncwarp();
+    uint32_t n_valid = 0;                              // cosets of this lane
+#pragma unroll
+    for (int c = 0; c < L; c++) {
+        const uint32_t first = lane + 32u * c;
+        if (first < S) n_valid += (S - first + 32u * L - 1u) / (32u * L);
+    }
+    const uint32_t n_nz = (n_valid - pushed) * R + nz_exact;        // every value of an unflagged coset is nonzero
+    const uint32_t n_odd = odd_fast + odd_exact;
+    n_zero = n_valid * R - n_nz;
+    n_sq = n_nz - n_odd;
+}
+
+}  // namespace hec_radix

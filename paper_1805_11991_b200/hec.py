@@ -17,13 +17,15 @@ import numpy as np
 _PKG = Path(__file__).resolve().parent
 LIB_PATH = _PKG / "libhec.so"
 _lib = None
+_cap_hint: dict = {}     # (n, g, merge?) -> distinct tuples of the last histogram call of that shape
 
 HEC_OK = 0
 HEC_ERR_INVALID_FIELD, HEC_ERR_INVALID_ARG, HEC_ERR_COEFF_RANGE, HEC_ERR_DEGREE = -1, -2, -3, -4
 HEC_ERR_CAPACITY, HEC_ERR_UNSUPPORTED, HEC_ERR_CUDA, HEC_ERR_NOMEM = -5, -6, -7, -8
 REGIME_AUTO, REGIME_SMEM, REGIME_L2, REGIME_SMEM_HALF = 0, 1, 2, 3
-EVAL_AUTO, EVAL_HORNER = 0, 1
-TABLE_MODES = {0: "global32-extended", 1: "smem16-extended", 2: "smem32-half", 3: "smem16+8-half"}
+EVAL_AUTO, EVAL_HORNER, EVAL_RADIX2, EVAL_RADIX4, EVAL_RADIX8 = 0, 1, 2, 4, 8
+TABLE_MODES = {0: "global32-extended", 1: "smem16-extended", 2: "smem32-half", 3: "smem16+8-half",
+               4: "smem2x16-pair", 5: "smem32-rhalf", 6: "smem16+1-rhalf", 7: "global2x32-pair"}
 MAX_GENUS = 5
 
 # every symbol include/hec.h declares (tests check the library exports all of them)
@@ -47,7 +49,7 @@ class CountStats(ctypes.Structure):
     _fields_ = [("count_kernel_ms", ctypes.c_float), ("squarefree_kernel_ms", ctypes.c_float),
                 ("launches", ctypes.c_uint32), ("regime", ctypes.c_uint32), ("smem_bytes", ctypes.c_uint32),
                 ("grid", ctypes.c_uint32), ("block", ctypes.c_uint32), ("chains_per_lane", ctypes.c_uint32),
-                ("table_mode", ctypes.c_uint32), ("radix4_fields", ctypes.c_uint32)]
+                ("table_mode", ctypes.c_uint32), ("radix_fields", ctypes.c_uint32)]
 
 
 def lib():
@@ -208,20 +210,34 @@ def histogram(counts, mask=None, _weights=None):
     else:
         def call(*a):
             return L.hec_histogram(_ptr(counts), _ptr(mask), n, g, *a)
-    rc = call(None, None, 0, ctypes.byref(m))
-    if rc not in (HEC_OK, HEC_ERR_CAPACITY):
-        _check(rc)
-    cap = m.value
-    if _is_torch(counts):
-        import torch
-        tup = torch.empty((cap, g), dtype=torch.int32, device=counts.device)
-        mult = torch.empty((cap,), dtype=torch.int64, device=counts.device)
+    def buffers(cap):
+        if _is_torch(counts):
+            import torch
+            return (torch.empty((cap, g), dtype=torch.int32, device=counts.device),
+                    torch.empty((cap,), dtype=torch.int64, device=counts.device))
+        return np.empty((cap, g), dtype=np.uint32), np.empty((cap,), dtype=np.uint64)
+
+    # Capacity protocol of hec.h.  A repeated call on a batch of the same shape first tries the capacity the
+    # last one needed (+25 %), so the steady state is ONE library call; otherwise size with cap = 0 first.
+    key = (n, g, _weights is not None)
+    hint = _cap_hint.get(key)
+    if hint is None:
+        rc = call(None, None, 0, ctypes.byref(m))
+        if rc not in (HEC_OK, HEC_ERR_CAPACITY):
+            _check(rc)
+        cap = m.value
     else:
-        tup = np.empty((cap, g), dtype=np.uint32)
-        mult = np.empty((cap,), dtype=np.uint64)
+        cap = min(n, hint + hint // 4 + 1024)
+    tup, mult = buffers(cap)
     if cap:
-        _check(call(_ptr(tup), _ptr(mult), cap, ctypes.byref(m)))
-    return tup, mult
+        rc = call(_ptr(tup), _ptr(mult), cap, ctypes.byref(m))
+        if rc == HEC_ERR_CAPACITY:
+            cap = m.value
+            tup, mult = buffers(cap)
+            rc = call(_ptr(tup), _ptr(mult), cap, ctypes.byref(m))
+        _check(rc)
+    _cap_hint[key] = m.value
+    return tup[: m.value], mult[: m.value]
 
 
 def histogram_merge(tuples, mult):

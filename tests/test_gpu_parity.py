@@ -16,8 +16,8 @@ pytestmark = pytest.mark.gpu
 
 @pytest.fixture(scope="module", params=["auto", "horner"])
 def torch_cuda(request):
-    """Every test runs under both evaluation schemes of hec_count: the default (radix-4 split where 4 | q^k - 1)
-    and the paper's one-Horner-chain-per-x scheme; the oracle is the same for both."""
+    """Every test runs under both evaluation schemes of hec_count: the default (radix-R split over the cosets of
+    the R-th roots of unity) and the paper's one-Horner-chain-per-x scheme; the oracle is the same for both."""
     import torch
     from paper_1805_11991_b200 import build as hb
     hb.build_lib()
@@ -115,14 +115,16 @@ def test_sparse_and_zero_heavy_rows(torch_cuda):
 
 
 def test_regimes_agree(torch_cuda):
-    """Every table layout gives identical counts: extended 16-bit shared-memory table, L2-resident 32-bit
-    table, shared-memory half table (32-bit for q=13^4 and 293^2, 16+8-bit planes for 49^3)."""
-    modes = {hec.REGIME_SMEM: 1, hec.REGIME_L2: 0}
+    """Every table layout gives identical counts: full shared-memory table (extended 16-bit / 2x16-bit pairs),
+    L2-resident table, shared-memory half table (32-bit for q=13^4 and 293^2, 16+8-bit or 16+1-bit planes for 49^3)."""
+    radix = torch_cuda.eval_scheme == "auto"
+    modes = {hec.REGIME_SMEM: 4, hec.REGIME_L2: 7} if radix else {hec.REGIME_SMEM: 1, hec.REGIME_L2: 0}
+    h32, h24 = (5, 6) if radix else (2, 3)
     try:
         for cid, n, regimes, half_mode in [(2, 3000, (hec.REGIME_SMEM, hec.REGIME_L2), None),
-                                           (4, 600, (hec.REGIME_SMEM, hec.REGIME_L2, hec.REGIME_SMEM_HALF), 2),
-                                           (5, 300, (hec.REGIME_L2, hec.REGIME_SMEM_HALF, hec.REGIME_AUTO), 2),
-                                           (3, 200, (hec.REGIME_L2, hec.REGIME_SMEM_HALF, hec.REGIME_AUTO), 3)]:
+                                           (4, 600, (hec.REGIME_SMEM, hec.REGIME_L2, hec.REGIME_SMEM_HALF), h32),
+                                           (5, 300, (hec.REGIME_L2, hec.REGIME_SMEM_HALF, hec.REGIME_AUTO), h32),
+                                           (3, 200, (hec.REGIME_L2, hec.REGIME_SMEM_HALF, hec.REGIME_AUTO), h24)]:
             cfg = W.CONFIGS[cid]
             rows = np.concatenate([W.generate(cfg, 5000, n), W.edge_rows(cfg.q, cfg.g)])
             ref = None
@@ -152,6 +154,8 @@ def test_mixed_layout_launch_groups(torch_cuda, q, g, mode, min_launches):
     to the lower fields' extended tables; 19^4 = 130321: 16+8-bit half table in a launch of its own;
     11^5 = 161051: nothing fits, L2-resident).  Oracle on the fields k <= 3 and on a few rows of k = 4; the
     forced L2 regime must agree on everything."""
+    if torch_cuda.eval_scheme == "auto":        # radix tables: pairs / 32-bit half / 16+1-bit half / global pairs
+        mode, min_launches = {(17, 4): (5, 2), (19, 4): (6, 3), (9, 5): (5, 2), (11, 5): (7, 2)}[(q, g)]
     rng = np.random.default_rng(q)
     rows = rng.integers(0, q, size=(70, 2 * g + 3)).astype(np.uint16)
     rows[:, -1] = np.where(rng.random(70) < 0.5, rng.integers(1, q, 70), 0)
@@ -271,11 +275,12 @@ def test_full_config2(torch_cuda):
 def test_full_config4_headline(torch_cuda):
     stats = _full_size_checks(torch_cuda, 4, 96)
     assert stats["regime"] == hec.REGIME_SMEM
-    assert stats["radix4_fields"] == (0b1111 if torch_cuda.eval_scheme == "auto" else 0)
+    # 13^k - 1 = 12, 168, 2196, 28560: R = 4, 8, 4, 8
+    assert stats["radix_fields"] == (0x8484 if torch_cuda.eval_scheme == "auto" else 0)
 
 
 def test_eval_schemes_agree_full_config4(torch_cuda):
-    """All 2^24 rows of the headline workload: radix-4 split and plain Horner give identical counts."""
+    """All 2^24 rows of the headline workload: radix split and plain Horner give identical counts."""
     if torch_cuda.eval_scheme != "auto":
         pytest.skip("compares both schemes in one run")
     cfg = W.CONFIGS[4]
@@ -284,21 +289,64 @@ def test_eval_schemes_agree_full_config4(torch_cuda):
         a, _ = hec.count(cfg.q, cfg.g, d_rows, want_squarefree=False)
         hec.set_eval(hec.EVAL_HORNER)
         b, _ = hec.count(cfg.q, cfg.g, d_rows, want_squarefree=False)
-        assert hec.last_count_stats()["radix4_fields"] == 0
+        assert hec.last_count_stats()["radix_fields"] == 0
     finally:
         hec.set_eval(hec.EVAL_AUTO)
     assert bool((a == b).all())
 
 
 def test_full_config5_half_table(torch_cuda):
-    if torch_cuda.eval_scheme != "auto":
-        pytest.skip("half-table layouts have one evaluation scheme")
     stats = _full_size_checks(torch_cuda, 5, 64)
-    assert stats["regime"] == hec.REGIME_SMEM_HALF and stats["table_mode"] == 2
+    assert stats["regime"] == hec.REGIME_SMEM_HALF and stats["table_mode"] == (5 if torch_cuda.eval_scheme == "auto" else 2)
 
 
 def test_full_config3_half_planes(torch_cuda):
-    if torch_cuda.eval_scheme != "auto":
-        pytest.skip("half-table layouts have one evaluation scheme")
     stats = _full_size_checks(torch_cuda, 3, 16)
-    assert stats["regime"] == hec.REGIME_SMEM_HALF and stats["table_mode"] == 3
+    assert stats["regime"] == hec.REGIME_SMEM_HALF and stats["table_mode"] == (6 if torch_cuda.eval_scheme == "auto" else 3)
+
+
+# ------------------------------------------------------------------------------------------ radix split
+
+@pytest.mark.parametrize("cap", [hec.EVAL_RADIX2, hec.EVAL_RADIX4, hec.EVAL_RADIX8])
+def test_every_radix_against_oracle(torch_cuda, cap):
+    """R = 2, 4, 8 (capped; the field decides what divides q^k - 1) on fields of every residue of q^k - 1 mod 8,
+    dense and sparse rows, in every table layout the field admits: all against the oracle."""
+    if torch_cuda.eval_scheme != "auto":
+        pytest.skip("radix caps are set explicitly")
+    rng = np.random.default_rng(cap)
+    try:
+        hec.set_eval(cap)
+        for q, g, n in [(3, 2, 200), (7, 3, 120), (5, 3, 120), (9, 2, 300), (13, 3, 60), (27, 2, 200), (11, 1, 100), (3, 5, 60)]:
+            rows = rng.integers(0, q, size=(n, 2 * g + 3)).astype(np.uint16)
+            rows[rng.random(rows.shape) < 0.35] = 0
+            rows[:, -1] = np.where(rng.random(n) < 0.5, rng.integers(1, q, n), 0)
+            rows[:, -2] = np.where(rows[:, -1] == 0, rng.integers(1, q, n), rows[:, -2])
+            rows = np.concatenate([rows, W.edge_rows(q, g)[:40]])
+            ocnt, osf, _ = O.count(q, g, rows)
+            for regime in (hec.REGIME_AUTO, hec.REGIME_L2):
+                hec.set_regime(regime)
+                cnt, sf = _gpu_count(torch_cuda, q, g, rows)
+                st = hec.last_count_stats()
+                assert (cnt == ocnt).all(), (q, g, cap, regime, np.argwhere(cnt != ocnt)[:5])
+                assert (sf == osf).all()
+                for k in range(1, g + 1):
+                    R = (st["radix_fields"] >> (4 * (k - 1))) & 15
+                    assert R in (2, 4, 8) and R <= cap and (q ** k - 1) % R == 0
+                    assert R == cap or (q ** k - 1) % (2 * R) != 0
+        # the half-table layouts on fields that admit them, against the pair layout
+        for cid, n in [(4, 300), (5, 100), (3, 60)]:
+            cfg = W.CONFIGS[cid]
+            rows = np.concatenate([W.generate(cfg, 777, n), W.edge_rows(cfg.q, cfg.g)[:30]])
+            hec.set_regime(hec.REGIME_L2)
+            ref, _ = _gpu_count(torch_cuda, cfg.q, cfg.g, rows)
+            hec.set_regime(hec.REGIME_SMEM_HALF)
+            a, _ = _gpu_count(torch_cuda, cfg.q, cfg.g, rows)
+            assert (a == ref).all(), (cid, cap)
+            hec.set_eval(hec.EVAL_HORNER)
+            hec.set_regime(hec.REGIME_AUTO)
+            b, _ = _gpu_count(torch_cuda, cfg.q, cfg.g, rows)
+            hec.set_eval(cap)
+            assert (b == ref).all(), (cid, cap)
+    finally:
+        hec.set_regime(hec.REGIME_AUTO)
+        hec.set_eval(hec.EVAL_AUTO)
