@@ -59,34 +59,43 @@ LOADS = {0: (1, None), 1: (1, None), 2: (1, None), 3: (2, None), 4: (1, 1), 5: (
 def executed_loads(cfg: W.Workload, rows: np.ndarray, stats: dict) -> int:
     """Table loads the count kernel issues for this batch, from the rows' zero patterns (exact up to the rare
     re-evaluated cosets).  Horner scheme: one lookup per nonzero term after the first, per nonzero x.
-    Radix-R scheme (hec_radix.cuh): per coset of R points, (#terms - #nonempty residue classes mod R) chain
-    lookups plus one pair lookup per butterfly whose two inputs are both nonzero."""
+    Radix-R scheme (hec_radix.cuh): per curve and field the kernel takes the largest R' <= R (R = the field's
+    radix) for which every residue class mod R' holds a nonzero coefficient (R' = 2 if there is none); per coset
+    of R' points: (#terms - #nonempty classes) chain lookups plus one pair lookup per butterfly whose two inputs
+    are both nonzero."""
     nzm = rows != 0
     n, ncoef = rows.shape
     top_mode = stats["table_mode"]
     total = 0
     for k in range(1, cfg.g + 1):
         M = cfg.q ** k - 1
-        R = (stats["radix_fields"] >> (4 * (k - 1))) & 15
-        mode = top_mode if k == cfg.g else (4 if R else 1)
+        Rf = (stats["radix_fields"] >> (4 * (k - 1))) & 15
+        mode = top_mode if k == cfg.g else (4 if Rf else 1)
         single, pair = LOADS[mode]
-        if R == 0:
+        if Rf == 0:
             total += int((nzm.sum(axis=1) - 1).sum()) * M * single
             continue
-        present = np.zeros((n, R), dtype=bool)
-        for r in range(R):
-            present[:, r] = nzm[:, r::R].any(axis=1)
-        chain = int((nzm.sum(axis=1) - present.sum(axis=1)).sum())
-        pairs = 0
-        H = R // 2
-        while H >= 1:
-            for blk in range(0, R, 2 * H):
-                for j in range(H):
-                    a, b = present[:, blk + j].copy(), present[:, blk + j + H].copy()
-                    pairs += int((a & b).sum())
-                    present[:, blk + j] = present[:, blk + j + H] = a | b
-            H //= 2
-        total += (chain * single + pairs * pair) * (M // R)
+        todo = np.ones(n, dtype=bool)
+        R = Rf
+        while R >= 2:
+            present = np.zeros((n, R), dtype=bool)
+            for r in range(R):
+                present[:, r] = nzm[:, r::R].any(axis=1)
+            sel = todo & (present.all(axis=1) if R > 2 else True)
+            todo &= ~sel
+            pr = present[sel]
+            chain = int((nzm[sel].sum(axis=1) - pr.sum(axis=1)).sum())
+            pairs = 0
+            H = R // 2
+            while H >= 1:
+                for blk in range(0, R, 2 * H):
+                    for j in range(H):
+                        a, b = pr[:, blk + j].copy(), pr[:, blk + j + H].copy()
+                        pairs += int((a & b).sum())
+                        pr[:, blk + j] = pr[:, blk + j + H] = a | b
+                H //= 2
+            total += (chain * single + pairs * pair) * (M // R)
+            R //= 2
     return total
 
 

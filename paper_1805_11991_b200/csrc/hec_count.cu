@@ -267,13 +267,19 @@ __global__ void __launch_bounds__(kThreads, 1) hec_count_kernel(const __grid_con
 // One launch of the radix-R evaluation (hec_radix.cuh; HEC_EVAL_AUTO) for k_lo <= k <= k_hi.  Fields below k_hi
 // use PAIR16 tables with the packed 16x2 arithmetic; field k_hi uses TOP.  Same mapping as above: persistent
 // CTAs, one warp per curve, the lanes stride the coset index n = log x < M / R.
+// Per curve and field: the largest R' <= R (R = the field's radix, R' | R | M) for which every residue class
+// mod R' holds a nonzero coefficient runs the straight-line network; the branchy general network is kept only
+// for R = 2 (f even or odd in X, or D + 1 < R').  Measured (profiles/r01c_ncu_full_c4_radix.md): compiling the
+// general network for R = 4, 8 made the loop body overflow the instruction caches (41 % no_instruction stalls).
 template <int D, typename Ar, typename Pol>
 __device__ __forceinline__ void radix_dispatch(const uint32_t R, const Pol pol, const uint32_t M, const uint32_t rcpM,
                                                const uint32_t lane, const uint32_t nz, const uint32_t lcj,
                                                volatile uint32_t *scratch, uint32_t &n_sq, uint32_t &n_zero) {
-    if (R == 8) hec_radix::radix_all_x<D, 8, Ar>(pol, M, rcpM, lane, nz, lcj, scratch, n_sq, n_zero);
-    else if (R == 4) hec_radix::radix_all_x<D, 4, Ar>(pol, M, rcpM, lane, nz, lcj, scratch, n_sq, n_zero);
-    else hec_radix::radix_all_x<D, 2, Ar>(pol, M, rcpM, lane, nz, lcj, scratch, n_sq, n_zero);
+    using namespace hec_radix;
+    if (R >= 8 && all_classes_present<D, 8>(nz)) radix_all_x<D, 8, true, Ar>(pol, M, rcpM, lane, nz, lcj, scratch, n_sq, n_zero);
+    else if (R >= 4 && all_classes_present<D, 4>(nz)) radix_all_x<D, 4, true, Ar>(pol, M, rcpM, lane, nz, lcj, scratch, n_sq, n_zero);
+    else if (all_classes_present<D, 2>(nz)) radix_all_x<D, 2, true, Ar>(pol, M, rcpM, lane, nz, lcj, scratch, n_sq, n_zero);
+    else radix_all_x<D, 2, false, Ar>(pol, M, rcpM, lane, nz, lcj, scratch, n_sq, n_zero);
 }
 
 template <int G, int TOP>

@@ -291,12 +291,24 @@ __device__ __forceinline__ void network(const Ar &ar, const Pol &pol, const uint
     }
 }
 
+// Bit r of the result is set iff residue class r mod R holds a nonzero coefficient (nz: bit i set iff c_i != 0).
+template <int D, int R>
+__device__ __forceinline__ bool all_classes_present(const uint32_t nz) {
+    if (D + 1 < R) return false;
+    uint32_t m = nz;
+#pragma unroll
+    for (int s = R; s <= D; s += R) m |= nz >> s;
+    return (m & ((1u << R) - 1u)) == (1u << R) - 1u;
+}
+
 // ---------------------------------------------------------------------------------------------------------
 // All x in F_{q^k}^x for one curve, one warp.  lcj: lane j holds the log of c_j in this field (any value when
 // c_j = 0), nz: bit j set iff c_j != 0, scratch: kScratchWords words of shared memory owned by this warp.
 // Returns this lane's share of n_zero = #{x != 0: f(x) = 0} and n_sq = #{x != 0: f(x) a nonzero square}.
+// ALL: the caller guarantees that every residue class mod R holds a nonzero coefficient (the straight-line
+// network); otherwise the network takes warp-uniform branches around the absent classes.
 // ---------------------------------------------------------------------------------------------------------
-template <int D, int R, typename Ar, typename Pol>
+template <int D, int R, bool ALL, typename Ar, typename Pol>
 __device__ __forceinline__ void radix_all_x(const Pol pol, const uint32_t M, const uint32_t rcpM, const uint32_t lane,
                                             const uint32_t nz, const uint32_t lcj, volatile uint32_t *scratch,
                                             uint32_t &n_sq, uint32_t &n_zero) {
@@ -353,7 +365,6 @@ __device__ __forceinline__ void radix_all_x(const Pol pol, const uint32_t M, con
         kc[r] = ar.join(t[0], t[1]);
         kinc[r] = ar.rep(mod(last_e[r] * step));
     }
-    const bool all_present = present == (1u << R) - 1u;
 
     uint32_t acc = 0, odd_fast = 0, passes = 0, pushed = 0, qn = 0, nz_exact = 0, odd_exact = 0;
     auto drain = [&]() {
@@ -384,8 +395,7 @@ __device__ __forceinline__ void radix_all_x(const Pol pol, const uint32_t M, con
             kc[r] = ar.wrap(kc[r] + kinc[r]);
         }
         uint32_t ps = 0;
-        if (all_present) network<R, true>(ar, pol, unit, present, v, ps, mn);
-        else network<R, false>(ar, pol, unit, present, v, ps, mn);
+        network<R, ALL>(ar, pol, unit, present, v, ps, mn);
         bool valid[2] = {false, false}, flag[2] = {false, false};
         bool any_flag = false;
 #pragma unroll
