@@ -56,6 +56,14 @@ __device__ __forceinline__ uint32_t lds_u8(uint32_t addr) {
 // test n.  pair_word (PairS16 only): both values in one 32-bit word, 0 where the sum is zero.
 // ---------------------------------------------------------------------------------------------------------
 
+// Byte addresses tb + 4 lo16(n2) and tb + 4 hi16(n2) of the entries of a packed pair of indices: mask / shift and
+// one LEA each (written as mad.lo so that ptxas does not fold the scaling into a shift + mask + add: 4 instead of
+// 6 instructions per packed lookup).
+__device__ __forceinline__ void packed_addr(uint32_t tb, uint32_t n2, uint32_t &a0, uint32_t &a1) {
+    asm("{.reg .u32 t;\n\tand.b32 t, %2, 0xffff;\n\tmad.lo.u32 %0, t, 4, %3;\n\tshr.u32 t, %2, 16;\n\tmad.lo.u32 %1, t, 4, %3;}"
+        : "=r"(a0), "=r"(a1) : "r"(n2), "r"(tb));
+}
+
 // PAIR16: shared memory, M 32-bit entries, lo16 = Z[n], hi16 = Z[n + h]  (M <= 32768).
 struct PairS16 {
     uint32_t tb;                                             // shared byte address of entry 0
@@ -161,13 +169,17 @@ struct ArPacked {
     __device__ __forceinline__ uint32_t subm(uint32_t b, uint32_t a) const { return wrap(b + M2 - a); }   // halves stay in (0, 2M): no borrow
     __device__ __forceinline__ uint32_t mn_init() const { return 0xFFFFFFFFu; }
     __device__ __forceinline__ void lookup_pair(const PairS16 &pol, uint32_t n, uint32_t &za, uint32_t &zs, uint32_t &mn) const {
-        const uint32_t w0 = pol.pair_word(n & 0xFFFFu), w1 = pol.pair_word(n >> 16);
+        uint32_t a0, a1;
+        packed_addr(pol.tb, n, a0, a1);
+        const uint32_t w0 = lds_u32(a0), w1 = lds_u32(a1);
         za = __byte_perm(w0, w1, 0x5410);
         zs = __byte_perm(w0, w1, 0x7632);
         mn = __vimin3_u16x2(mn, za, zs);                      // a stored 0 marks a vanished sum (per coset: per half)
     }
     __device__ __forceinline__ uint32_t lookup_single(const PairS16 &pol, uint32_t n, uint32_t &mn) const {
-        const uint32_t z0 = pol.single(n & 0xFFFFu, 0, 0), z1 = pol.single(n >> 16, 0, 0);
+        uint32_t a0, a1;
+        packed_addr(pol.tb, n, a0, a1);
+        const uint32_t z0 = lds_u16(a0), z1 = lds_u16(a1);
         const uint32_t z = __byte_perm(z0, z1, 0x5410);
         mn = __vminu2(mn, z);
         return z;
