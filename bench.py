@@ -361,6 +361,102 @@ def run_ours(args, cfg):
     print(json.dumps(line), flush=True)
 
 
+# ------------------------------------------------------------------------------------------------ Table 1 of the paper
+
+# PAPER.md:313-326, runtimes in ms on 1x Tesla K80 / one core of a Xeon E5-2683: p -> (tables, CPU, GPU eval, GPU reduce)
+PAPER_TABLE1 = {101: (4.70, 0.63, 0.36, 0.10), 211: (23.8, 4.47, 1.47, 0.15), 307: (54.9, 12.1, 3.11, 0.22),
+                401: (99.2, 22.2, 0.95, 0.35), 503: (167, 36.3, 1.25, 0.83), 1009: (892, 148, 2.93, 6.49),
+                1511: (2545, 349, 394, 19.7), 2003: (5093, 789, 11.5, 36.1), 3001: (13474, 3669, 15.4, 82.6)}
+TABLE1_CURVE = [17, 12, 16, 11, 10, 13, 12]   # Y^2 = 12X^6 + 13X^5 + 10X^4 + 11X^3 + 16X^2 + 12X + 17, c_0 first
+
+
+def run_table1(args):
+    """the paper's own benchmark -- (N_1, N_2) of ONE genus-2 curve over F_p, F_{p^2} -- with
+    the table precomputation (hec_build_field_device) and the count (hec_count, split over the whole GPU) timed
+    separately like the paper's columns, every count checked against the oracle.  Prints one JSON line."""
+    import torch
+    from paper_1805_11991_b200 import build as hb, hec
+    from oracle import hec_oracle as O
+    hb.build_lib()
+    torch.cuda.set_device(0)
+    stream = torch.cuda.current_stream()
+    hec.set_stream(stream.cuda_stream)
+    hec.count(3, 2, np.array([[1, 0, 0, 0, 0, 1, 0]], dtype=np.uint16))       # context + module load
+    out = []
+    for p, (t_tab, t_cpu, t_eval, t_red) in PAPER_TABLE1.items():
+        rows = np.array([[c % p for c in TABLE1_CURVE]], dtype=np.uint16)
+        d_rows = torch.from_numpy(rows.view(np.int16)).cuda()
+        d_cnt = torch.empty((1, 2), dtype=torch.int32, device="cuda")
+        d_sf = torch.empty((1,), dtype=torch.uint8, device="cuda")
+        hec.shutdown()
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        for k in (1, 2):
+            hec.build_field_device(p, 1, k).close()
+        tables_ms = (time.perf_counter() - t0) * 1e3               # modulus search + kernels + copy of the tables to the host
+        t0 = time.perf_counter()
+        hec.build_field(p, 1, 2).close()
+        tables_host_ms = (time.perf_counter() - t0) * 1e3
+        t0 = time.perf_counter()
+        hec.count(p, 2, d_rows, d_cnt, d_sf)                        # first call: fields, table layouts, upload, kernels
+        first_ms = (time.perf_counter() - t0) * 1e3
+        for _ in range(args.warmup):
+            hec.count(p, 2, d_rows, d_cnt, d_sf)
+        torch.cuda.synchronize()
+        reps, kern = max(args.steps, 10), []
+        t0 = time.perf_counter()
+        for _ in range(reps):
+            hec.count(p, 2, d_rows, d_cnt, d_sf)
+            kern.append(hec.last_count_stats()["count_kernel_ms"])
+        call_ms = (time.perf_counter() - t0) * 1e3 / reps           # whole call incl. the status read-back
+        st = hec.last_count_stats()
+        cnt = d_cnt.cpu().numpy().view(np.uint32)
+        t0 = time.perf_counter()
+        ocnt, osf, _ = O.count(p, 2, rows)
+        oracle_ms = (time.perf_counter() - t0) * 1e3
+        k_ms = float(np.median(kern))
+        out.append({"p": p, "N": cnt[0].tolist(), "parity_ok": bool((cnt == ocnt).all() and int(d_sf.item()) == int(osf[0])),
+                    "tables_ms": tables_ms, "tables_host_ms": tables_host_ms, "first_call_ms": first_ms,
+                    "count_kernel_ms": k_ms, "count_call_ms": call_ms, "splits": st["splits"],
+                    "table_layout": hec.TABLE_MODES[st["table_mode"]], "xevals_per_s": (p + p * p) / (k_ms * 1e-3),
+                    "oracle_ms_1core": oracle_ms,
+                    "paper_ms": {"tables": t_tab, "cpu": t_cpu, "gpu_eval": t_eval, "gpu_reduce": t_red},
+                    "vs_paper_gpu": (t_eval + t_red) / k_ms, "vs_paper_tables": t_tab / tables_ms})
+    print(json.dumps({"metric": "table1_single_curve_ms", "unit": "ms", "higher_is_better": False, "data": "the paper's curve (PAPER.md:326)",
+                      "config": {"workload": "table1: one genus-2 curve over F_p and F_{p^2}", "g": 2},
+                      "note": "paper_ms: 1x Tesla K80 + one Xeon E5-2683 core (PAPER.md:301): context, other hardware",
+                      "rows": out}), flush=True)
+
+
+def run_curve_map(args):
+    """Algorithm 1 without lambda for one (q, g, d): device enumeration of the reduced polynomials,
+    hec_count, weighted histogram, twist doubling.  Prints one JSON line (time of the whole hec_curve_map call)."""
+    import torch
+    from paper_1805_11991_b200 import build as hb, hec
+    hb.build_lib()
+    torch.cuda.set_device(0)
+    hec.set_stream(torch.cuda.current_stream().cuda_stream)
+    q, g, d = (int(v) for v in args.curve_map.split(","))
+    total = hec.reduced_total(q, g, d)
+    hec.curve_map(3, 1, 4)                                     # context, module load
+    l0 = hec.launch_count()
+    t0 = time.perf_counter()
+    tup, w = hec.curve_map(q, g, d)
+    dt = time.perf_counter() - t0
+    launches = hec.launch_count() - l0
+    want = (q - 1) * (q ** d - q ** (d - 1))
+    m = {tuple(int(v) for v in t): int(x) for t, x in zip(tup, w)}
+    tw = lambda t: tuple((2 * q ** k + 2 - n) if k % 2 else n for k, n in enumerate(t, start=1))
+    print(json.dumps({
+        "metric": "reduced_polynomials_per_s", "value": total / dt, "unit": "curves/s", "higher_is_better": True,
+        "config": {"workload": f"curve map N_(g,d), q={q}, g={g}, d={d}", "reduced_polynomials": total,
+                   "squarefree_polynomials_covered": want, "x_evals_per_curve": sum(q ** k for k in range(1, g + 1))},
+        "seconds": dt, "polynomials_covered_per_s": want / dt, "distinct_tuples": int(len(w)), "gpu_launches": int(launches),
+        "checks": {"total_weight_is_number_of_squarefree_polynomials": int(w.sum()) == want,
+                   "twist_symmetric": all(m.get(tw(t)) == x for t, x in m.items())},
+        "data": "enumerated on the device (no input)"}), flush=True)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -375,7 +471,17 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--curves", type=int, default=0,
                     help="profiling only: first N curves of the workload (the line is then marked reduced and is not a bench value)")
+    ap.add_argument("--table1", action="store_true",
+                    help="the paper's Table 1 instead of the batch metric: one curve over F_p, F_{p^2}, p = 101 .. 3001")
+    ap.add_argument("--curve-map", default="", metavar="q,g,d",
+                    help="Algorithm 1 without lambda for one (q, g, d) instead of the batch metric, e.g. 13,4,9")
     args = ap.parse_args()
+    if args.table1:
+        run_table1(args)
+        return
+    if args.curve_map:
+        run_curve_map(args)
+        return
     cfg = W.CONFIGS[args.config]
     if args.curves:
         import dataclasses

@@ -69,6 +69,15 @@ typedef struct hec_field hec_field;
 hec_field *hec_build_field(uint32_t p, uint32_t r, uint32_t k);
 void hec_free_field(hec_field *F);
 
+/* hec_build_field_device -- the same field, with the tables built by CUDA kernels (the "tables" column of the
+ * paper's Table 1: the precomputation that dominates a single large-p curve).
+ * The modulus is found on the host by order tests (t^(Q-1) = 1, t^((Q-1)/l) != 1 for every prime l | Q-1); the
+ * antilog / log / Zech tables are computed on the current device and stream (hec_set_stream) and copied into the
+ * handle, so every accessor above works unchanged.  The result equals hec_build_field(p, r, k) entry for entry.
+ * Needs a CUDA device (NULL + HEC_ERR_CUDA message otherwise; no host fallback) and p < 65536.
+ * hec_count builds its own fields this way when q^k > 65536. */
+hec_field *hec_build_field_device(uint32_t p, uint32_t r, uint32_t k);
+
 /* Read-only accessors (paper's conventions: logs in [0, Q-2], zero <-> Q-1).  The out arrays are HOST
  * arrays owned by the caller with the stated number of elements.  A NULL field returns 0 / does nothing. */
 uint32_t hec_field_p(const hec_field *F);
@@ -128,6 +137,32 @@ int hec_histogram_merge(const uint32_t *in_tuples, const uint64_t *in_mult, size
                         uint32_t *out_tuples, uint64_t *out_mult, size_t cap, size_t *out_m);
 
 /* ------------------------------------------------------------------------------------------------
+ * Algorithm 1 around the hot path, without the partition lambda: SURVEY.md 8(f) NEXT-1.
+ *
+ * hec_reduced_total / hec_reduced_rows -- the reduced polynomials P~'_d(F_q) of sections 1.2-1.3,
+ * BEFORE the squarefree filter, generated by a kernel from their index (no input in HBM), d = 2g+1 or 2g+2:
+ *   family A0   c_d X^d + 1,  c_d = 1..q-1                                         mult q(q-1)/2
+ *   family A1   c_d X^d + X                                                        mult q(q-1)/2        (reading G18: the
+ *               printed set omits the support {d, 1}; without it the map misses these curves)
+ *   families B(i,j), 1 <= i <= d-2, 0 <= j < i:  c_d X^d + X^i + c_j X^j + c_{j-1} X^{j-1} + .. + c_0,
+ *               c_j = alpha^s, s < gamma = gcd(q-1, i-j), c_{j-1}..c_0 in F_q      mult q(q-1)^2/(2 gamma)
+ *   (reading G9: i and j are the two LARGEST indices below d with nonzero coefficient; c_{d-1} = 0 by X -> X - c_{d-1}/(d c_d)).
+ * Index order: A0, A1, then B(i,j) with j fastest; inside a family ((c_d - 1) gamma + s) q^j + sum_{l<j} c_l q^l.
+ *   out_coeffs[n][2g+3] uint16 (layout of hec_count), out_mult[n] uint64 = mult(f); both host or both device.
+ * Errors: HEC_ERR_UNSUPPORTED when p | d (reading G19: the printed set for p | d, misses every
+ * polynomial with c_{d-1} = 0 != c_{d-2} and cannot be followed), HEC_ERR_INVALID_ARG (d, index range), HEC_ERR_CUDA.
+ *
+ * hec_curve_map -- N_{g,d}: for every reduced f (in chunks of 2^22 rows: rows kernel -> hec_count -> weighted
+ * histogram of the squarefree rows), add mult(f) at (N_1..N_g) and at the tuple of the quadratic twist n f
+ * (Algorithm 1 lines 19-21; reading G8: N_k -> 2 q^k + 2 - N_k for odd k, N_k for even k).  The result equals
+ * #{f squarefree of degree d over F_q with that tuple} (eq. (1.2) without lambda).  Output as for hec_histogram:
+ * ascending lexicographic tuples, uint64 weights, two-call capacity protocol (*out_m always set).
+ */
+int hec_reduced_total(uint32_t q, uint32_t g, uint32_t d, uint64_t *out_total);
+int hec_reduced_rows(uint32_t q, uint32_t g, uint32_t d, uint64_t first, size_t n, uint16_t *out_coeffs, uint64_t *out_mult);
+int hec_curve_map(uint32_t q, uint32_t g, uint32_t d, uint32_t *out_tuples, uint64_t *out_weights, size_t cap, size_t *out_m);
+
+/* ------------------------------------------------------------------------------------------------
  * Execution control and instrumentation (used by the tests, bench.py and the ncu runs).
  */
 /* cudaStream_t (as void*) on which later calls enqueue their device work; NULL = default stream. */
@@ -178,6 +213,8 @@ typedef struct hec_count_stats {
     uint32_t chains_per_lane;
     uint32_t table_mode;
     uint32_t radix_fields;     /* nibble k-1: radix R used for N_k (0: one Horner chain per x) */
+    uint32_t splits;           /* warps per curve: 1 for batches; > 1 when a small batch (down to a single curve) is spread
+                                  over the whole GPU, each warp taking a slice of the x range of every field */
 } hec_count_stats;
 int hec_last_count_stats(hec_count_stats *out);
 

@@ -10,7 +10,7 @@ PKG = Path(__file__).resolve().parent
 ROOT = PKG.parent
 CSRC = PKG / "csrc"
 LIB = PKG / "libhec.so"
-SOURCES = ["hec_field.cpp", "hec_count.cu", "hec_histogram.cu", "hec_gather.cu"]
+SOURCES = ["hec_field.cpp", "hec_field_device.cu", "hec_count.cu", "hec_histogram.cu", "hec_enum.cu", "hec_gather.cu"]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
     "-Xcompiler", "-fPIC", "-Xcompiler", "-Wall", "-shared", "-cudart", "static",

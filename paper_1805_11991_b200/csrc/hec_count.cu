@@ -274,12 +274,13 @@ __global__ void __launch_bounds__(kThreads, 1) hec_count_kernel(const __grid_con
 template <int D, typename Ar, typename Pol>
 __device__ __forceinline__ void radix_dispatch(const uint32_t R, const Pol pol, const uint32_t M, const uint32_t rcpM,
                                                const uint32_t lane, const uint32_t nz, const uint32_t lcj,
-                                               volatile uint32_t *scratch, uint32_t &n_sq, uint32_t &n_zero) {
+                                               volatile uint32_t *scratch, const uint32_t part, const uint32_t splits,
+                                               uint32_t &n_sq, uint32_t &n_zero) {
     using namespace hec_radix;
-    if (R >= 8 && all_classes_present<D, 8>(nz)) radix_all_x<D, 8, true, Ar>(pol, M, rcpM, lane, nz, lcj, scratch, n_sq, n_zero);
-    else if (R >= 4 && all_classes_present<D, 4>(nz)) radix_all_x<D, 4, true, Ar>(pol, M, rcpM, lane, nz, lcj, scratch, n_sq, n_zero);
-    else if (all_classes_present<D, 2>(nz)) radix_all_x<D, 2, true, Ar>(pol, M, rcpM, lane, nz, lcj, scratch, n_sq, n_zero);
-    else radix_all_x<D, 2, false, Ar>(pol, M, rcpM, lane, nz, lcj, scratch, n_sq, n_zero);
+    if (R >= 8 && all_classes_present<D, 8>(nz)) radix_all_x<D, 8, true, Ar>(pol, M, rcpM, lane, nz, lcj, scratch, part, splits, n_sq, n_zero);
+    else if (R >= 4 && all_classes_present<D, 4>(nz)) radix_all_x<D, 4, true, Ar>(pol, M, rcpM, lane, nz, lcj, scratch, part, splits, n_sq, n_zero);
+    else if (all_classes_present<D, 2>(nz)) radix_all_x<D, 2, true, Ar>(pol, M, rcpM, lane, nz, lcj, scratch, part, splits, n_sq, n_zero);
+    else radix_all_x<D, 2, false, Ar>(pol, M, rcpM, lane, nz, lcj, scratch, part, splits, n_sq, n_zero);
 }
 
 template <int G, int TOP>
@@ -298,7 +299,11 @@ __global__ void __launch_bounds__(kThreads, 1) hec_count_radix_kernel(const __gr
     volatile uint32_t *scratch = reinterpret_cast<volatile uint32_t *>(reinterpret_cast<char *>(smem_blob) + P.scratch_off) +
                                  warp * hec_radix::kScratchWords;
 
-    for (unsigned long long curve = (unsigned long long)blockIdx.x * kWarps + warp; curve < P.n; curve += stride) {
+    // one work item = (curve, part): part `part` of P.splits slices of the coset range of every field
+    const unsigned long long items = P.n * P.splits;
+    for (unsigned long long item = (unsigned long long)blockIdx.x * kWarps + warp; item < items; item += stride) {
+        const unsigned long long curve = P.splits == 1u ? item : item / P.splits;
+        const uint32_t part = P.splits == 1u ? 0u : (uint32_t)(item - curve * P.splits);
         // ---- a2: coefficient load (lane j holds c_j) and boundary checks (readings G13, hec.h)
         uint32_t cj = 0;
         if (lane < NC) cj = P.coeffs[curve * NC + lane];
@@ -307,7 +312,7 @@ __global__ void __launch_bounds__(kThreads, 1) hec_count_radix_kernel(const __gr
         const bool mine = lane + 1 >= P.k_lo && lane + 1 <= P.k_hi;
         if (bad_range || (nz >> (D - 1)) == 0) {
             if (lane == 0) atomicMin(&P.err[bad_range ? 0 : 1], curve);
-            if (mine) P.out[curve * G + lane] = 0;
+            if (mine && P.splits == 1u) P.out[curve * G + lane] = 0;
             continue;
         }
         uint32_t my_count = 0;   // lane k-1 keeps N_k
@@ -320,16 +325,16 @@ __global__ void __launch_bounds__(kThreads, 1) hec_count_radix_kernel(const __gr
             uint32_t n_zero, n_sq;
             if (TOP == HEC_TAB_PAIR16 || k < P.k_hi) {
                 const hec_radix::PairS16 pol{smem_base + F.smem_off};
-                radix_dispatch<D, hec_radix::ArPacked>(F.radix, pol, M, F.rcpM, lane, nz, lcj, scratch, n_sq, n_zero);
+                radix_dispatch<D, hec_radix::ArPacked>(F.radix, pol, M, F.rcpM, lane, nz, lcj, scratch, part, P.splits, n_sq, n_zero);
             } else if constexpr (TOP == HEC_TAB_RHALF32) {
                 const hec_radix::HalfS32 pol{smem_base + F.smem_off, smem_base + F.smem_off + 4u * (M >> 1)};
-                radix_dispatch<D, hec_radix::ArScalar>(F.radix, pol, M, F.rcpM, lane, nz, lcj, scratch, n_sq, n_zero);
+                radix_dispatch<D, hec_radix::ArScalar>(F.radix, pol, M, F.rcpM, lane, nz, lcj, scratch, part, P.splits, n_sq, n_zero);
             } else if constexpr (TOP == HEC_TAB_RHALF17) {
                 const hec_radix::HalfS17 pol{smem_base + F.smem_off, smem_base + F.smem_off + 2u * (M >> 1), smem_base + F.smem_off2};
-                radix_dispatch<D, hec_radix::ArScalar>(F.radix, pol, M, F.rcpM, lane, nz, lcj, scratch, n_sq, n_zero);
+                radix_dispatch<D, hec_radix::ArScalar>(F.radix, pol, M, F.rcpM, lane, nz, lcj, scratch, part, P.splits, n_sq, n_zero);
             } else if constexpr (TOP == HEC_TAB_GPAIR64) {
                 const hec_radix::PairG64 pol{reinterpret_cast<const uint2 *>(F.gtab)};
-                radix_dispatch<D, hec_radix::ArScalar>(F.radix, pol, M, F.rcpM, lane, nz, lcj, scratch, n_sq, n_zero);
+                radix_dispatch<D, hec_radix::ArScalar>(F.radix, pol, M, F.rcpM, lane, nz, lcj, scratch, part, P.splits, n_sq, n_zero);
             }
             const uint32_t r0 = __reduce_add_sync(0xffffffffu, n_zero);
             const uint32_t rsq = __reduce_add_sync(0xffffffffu, n_sq);
@@ -338,10 +343,13 @@ __global__ void __launch_bounds__(kThreads, 1) hec_count_radix_kernel(const __gr
             const uint32_t lcD = __shfl_sync(0xffffffffu, lcj, D);
             const uint32_t x0 = (nz & 1u) == 0 ? 1u : ((lc0 & 1u) ? 0u : 2u);
             const uint32_t inf = ((nz >> D) & 1u) == 0 ? 1u : ((lcD & 1u) ? 0u : 2u);
-            const uint32_t Nk = r0 + 2u * rsq + x0 + inf;
+            const uint32_t Nk = r0 + 2u * rsq + (part == 0u ? x0 + inf : 0u);
             if (lane + 1 == k) my_count = Nk;
         }
-        if (mine) P.out[curve * G + lane] = my_count;
+        if (mine) {
+            if (P.splits == 1u) P.out[curve * G + lane] = my_count;
+            else if (my_count) atomicAdd(&P.out[curve * G + lane], my_count);
+        }
     }
 }
 
@@ -448,7 +456,7 @@ struct DevicePlan {
 };
 
 struct LibState {
-    std::mutex mu;
+    std::recursive_mutex mu;   // recursive: hec_count -> field cache -> hec_build_field_device -> hec_ensure_device
     cudaStream_t stream = nullptr;
     int regime = HEC_REGIME_AUTO;
     int eval = HEC_EVAL_AUTO;
@@ -475,6 +483,7 @@ int ensure_device(LibState &S) {
     HEC_CUDA_OK(cudaDeviceGetAttribute(&S.smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
     for (auto &e : S.ev) HEC_CUDA_OK(cudaEventCreate(&e));
     S.device_ready = true;
+    hec_allow_device_field_build(true);          // fields above 2^16 elements are now built by hec_field_device.cu
     return HEC_OK;
 }
 
@@ -755,7 +764,7 @@ int build_plan(LibState &S, uint32_t q, uint32_t g, int regime, int eval, Device
 template <typename Kern>
 int launch_kernel(LibState &S, Kern kern, const LaunchPlan &L, const HecCountParams &P, uint32_t chains) {
     HEC_CUDA_OK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)L.smem_bytes));
-    uint32_t grid = (uint32_t)std::min<unsigned long long>((P.n + kWarps - 1) / kWarps, (unsigned long long)S.sm_count);
+    uint32_t grid = (uint32_t)std::min<unsigned long long>((P.n * P.splits + kWarps - 1) / kWarps, (unsigned long long)S.sm_count);
     if (grid == 0) grid = 1;
     kern<<<grid, kThreads, L.smem_bytes, S.stream>>>(P);
     hec_launch_counter::value++;
@@ -802,7 +811,7 @@ bool is_device_pointer(const void *p) {
 // Shared with the other translation units.
 cudaStream_t hec_current_stream() { return g_state.stream; }
 int hec_ensure_device(int *sm_count, int *smem_optin) {
-    std::lock_guard<std::mutex> lock(g_state.mu);
+    std::lock_guard<std::recursive_mutex> lock(g_state.mu);
     int rc = ensure_device(g_state);
     if (rc) return rc;
     if (sm_count) *sm_count = g_state.sm_count;
@@ -814,28 +823,28 @@ bool hec_is_device_pointer(const void *p) { return is_device_pointer(p); }
 extern "C" {
 
 int hec_set_stream(void *cuda_stream) {
-    std::lock_guard<std::mutex> lock(g_state.mu);
+    std::lock_guard<std::recursive_mutex> lock(g_state.mu);
     g_state.stream = static_cast<cudaStream_t>(cuda_stream);
     return HEC_OK;
 }
 
 int hec_set_regime(int regime) {
     if (regime < HEC_REGIME_AUTO || regime > HEC_REGIME_SMEM_HALF) HEC_FAIL(HEC_ERR_INVALID_ARG, "unknown regime");
-    std::lock_guard<std::mutex> lock(g_state.mu);
+    std::lock_guard<std::recursive_mutex> lock(g_state.mu);
     g_state.regime = regime;
     return HEC_OK;
 }
 
 int hec_set_eval(int eval) {
     if (eval != HEC_EVAL_AUTO && eval != HEC_EVAL_HORNER && eval != HEC_EVAL_RADIX2 && eval != HEC_EVAL_RADIX4 && eval != HEC_EVAL_RADIX8) HEC_FAIL(HEC_ERR_INVALID_ARG, "unknown evaluation scheme");
-    std::lock_guard<std::mutex> lock(g_state.mu);
+    std::lock_guard<std::recursive_mutex> lock(g_state.mu);
     g_state.eval = eval;
     return HEC_OK;
 }
 
 int hec_last_count_stats(hec_count_stats *out) {
     if (!out) HEC_FAIL(HEC_ERR_INVALID_ARG, "out is NULL");
-    std::lock_guard<std::mutex> lock(g_state.mu);
+    std::lock_guard<std::recursive_mutex> lock(g_state.mu);
     *out = g_state.stats;
     return HEC_OK;
 }
@@ -853,7 +862,7 @@ int hec_count(uint32_t q, uint32_t g, const uint16_t *coeffs, size_t n, uint32_t
     if (n == 0) return HEC_OK;
     if (!coeffs || !out_counts) HEC_FAIL(HEC_ERR_INVALID_ARG, "coeffs and out_counts must not be NULL");
 
-    std::lock_guard<std::mutex> lock(g_state.mu);
+    std::lock_guard<std::recursive_mutex> lock(g_state.mu);
     LibState &S = g_state;
     int rc = ensure_device(S);
     if (rc) return rc;
@@ -892,12 +901,26 @@ int hec_count(uint32_t q, uint32_t g, const uint16_t *coeffs, size_t n, uint32_t
     HecCountParams P;
     P.coeffs = d_coeffs; P.out = d_counts; P.n = n; P.q = q;
     P.blob = nullptr; P.blob_bytes = 0; P.err = plan->d_err; P.k_lo = 1; P.k_hi = g; P.scratch_off = 0;
+    // Small batches (down to the single curve of the paper's Table 1): spread every curve over
+    // `splits` warps so that the whole GPU works on it; each warp takes a slice of the cosets of every field.
+    P.splits = 1;
+    if (plan->radix) {
+        const unsigned long long warps = (unsigned long long)S.sm_count * kWarps;
+        const uint32_t Mtop = plan->f[g - 1].M;
+        if (n < 2 * warps && Mtop >= 4096u) {
+            const unsigned long long want = (2 * warps + n - 1) / n;
+            P.splits = (uint32_t)std::max<unsigned long long>(1, std::min<unsigned long long>(want, Mtop / 2048u));
+        }
+    }
+    if (P.splits > 1) HEC_CUDA_OK(cudaMemsetAsync(d_counts, 0, cnt_bytes, S.stream));
+    const uint32_t splits_used = P.splits;
     for (uint32_t k = 0; k < HEC_MAX_GENUS; k++) P.f[k] = plan->f[k < g ? k : 0];
 
     S.stats = hec_count_stats{};
     S.stats.table_mode = (uint32_t)plan->top_mode;
     S.stats.regime = (plan->top_mode == HEC_TAB_EXT16 || plan->top_mode == HEC_TAB_PAIR16) ? HEC_REGIME_SMEM
                      : (plan->top_mode == HEC_TAB_GLOBAL32 || plan->top_mode == HEC_TAB_GPAIR64) ? HEC_REGIME_L2 : HEC_REGIME_SMEM_HALF;
+    S.stats.splits = splits_used;
     HEC_CUDA_OK(cudaEventRecord(S.ev[0], S.stream));
     switch (g) {
         case 1: rc = launch_count<1, 4>(S, *plan, P); break;
@@ -940,7 +963,7 @@ int hec_count(uint32_t q, uint32_t g, const uint16_t *coeffs, size_t n, uint32_t
 }
 
 void hec_shutdown(void) {
-    std::lock_guard<std::mutex> lock(g_state.mu);
+    std::lock_guard<std::recursive_mutex> lock(g_state.mu);
     g_state.plans.clear();
     if (g_state.d_stage) { cudaFree(g_state.d_stage); g_state.d_stage = nullptr; g_state.stage_bytes = 0; }
     hec_histogram_release_pool();

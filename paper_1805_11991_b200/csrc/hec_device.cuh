@@ -55,6 +55,7 @@ struct HecCountParams {
     uint32_t k_lo, k_hi;           // this launch computes N_k for k_lo <= k <= k_hi; only field k_hi may differ from the
                                    // launch's base layout (EXT16 for the Horner kernel, PAIR16 for the radix kernel)
     uint32_t scratch_off;          // radix kernel: byte offset (after the blob) of the per-warp scratch words
+    uint32_t splits;               // radix kernel: warps per curve (>= 1); > 1: out is pre-zeroed and accumulated with atomics
     HecFieldDev f[HEC_MAX_GENUS];
 };
 

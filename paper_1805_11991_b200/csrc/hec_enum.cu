@@ -1,0 +1,283 @@
+// Algorithm 1 of the paper around the hot path, without lambda:
+//   hec_reduced_total / hec_reduced_rows   the reduced polynomials P~'_d(F_q) of sections 1.2-1.3,
+//                                          generated on the device from their index, with mult(f);
+//   hec_curve_map                          for every reduced f: (N_1..N_g) by hec_count, squarefree filter, then
+//                                          "increment N at the tuple and at the tuple of the quadratic twist by mult(f)"
+//                                          (Algorithm 1 lines 19-21) as a weighted device histogram.
+// Readings: G9 (i, j are the two largest indices below d with nonzero coefficient), G8 (the
+// twist is n f, n a non-square: N_k -> 2 q^k + 2 - N_k for odd k, N_k for even k), G18 (the family c_d X^d + X, which
+// the printed set omits), G19 (only p not dividing d: the printed set for p | d is incomplete).
+//
+// Index order of P~'_d (before the squarefree filter), families one after the other:
+//   A0   c_d X^d + 1             c_d = 1 .. q-1 (integer encoding)                      mult q (q-1) / 2
+//   A1   c_d X^d + X             likewise                                               mult q (q-1) / 2
+//   B(i,j), i = 1 .. d-2, j = 0 .. i-1 (j fastest):  c_d X^d + X^i + c_j X^j + (c_{j-1} .. c_0 free)
+//        c_j = alpha^s, s = 0 .. gamma-1, gamma = gcd(q-1, i-j)  (alpha^0 .. alpha^{gamma-1} represent F_q^x / F_q^{x (i-j)})
+//        index inside the family = ((c_d - 1) gamma + s) q^j + sum_{l<j} c_l q^l      mult q (q-1)^2 / (2 gamma)
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <numeric>
+#include <vector>
+
+#include "hec_device.cuh"
+
+cudaStream_t hec_current_stream();
+int hec_ensure_device(int *sm_count, int *smem_optin);
+bool hec_is_device_pointer(const void *p);
+int hec_histogram_weighted(const uint32_t *counts, const uint8_t *mask, const uint64_t *weights, size_t n, uint32_t g,
+                           uint32_t *out_tuples, uint64_t *out_mult, size_t cap, size_t *out_m);
+
+namespace {
+
+constexpr int kMaxFamilies = 2 + 12 * 11 / 2;      // d <= 2 HEC_MAX_GENUS + 2 = 12: i <= 10, j < i
+
+struct Family {
+    unsigned long long first;      // index of the family's first polynomial
+    unsigned long long qj;         // q^j
+    unsigned long long mult;
+    uint32_t i, j, gamma;          // A0: i = 0, A1: i = 1, both with j = 0xFFFFFFFF
+};
+
+struct EnumParams {
+    Family fam[kMaxFamilies];
+    uint32_t nfam, q, d, ncoef;
+    unsigned long long total;
+    const uint32_t *antilog;       // F_q: alpha^s in the integer encoding, s < q-1 (device)
+};
+
+__global__ void __launch_bounds__(256) reduced_rows_kernel(const __grid_constant__ EnumParams E, unsigned long long first,
+                                                           unsigned long long n, uint16_t *__restrict__ rows,
+                                                           unsigned long long *__restrict__ mult) {
+    for (unsigned long long r = blockIdx.x * 256ull + threadIdx.x; r < n; r += gridDim.x * 256ull) {
+        const unsigned long long idx = first + r;
+        uint32_t lo = 0, hi = E.nfam - 1;                 // last family with fam.first <= idx
+        while (lo < hi) {
+            const uint32_t mid = (lo + hi + 1) >> 1;
+            if (E.fam[mid].first <= idx) lo = mid; else hi = mid - 1;
+        }
+        const Family &F = E.fam[lo];
+        unsigned long long t = idx - F.first;
+        uint16_t c[2 * HEC_MAX_GENUS + 3];
+#pragma unroll
+        for (int l = 0; l < 2 * (int)HEC_MAX_GENUS + 3; l++) c[l] = 0;
+        if (F.j == 0xFFFFFFFFu) {
+            c[F.i] = 1;
+            c[E.d] = (uint16_t)(t + 1);
+        } else {
+            unsigned long long low = t % F.qj;
+            t /= F.qj;
+            const uint32_t s = (uint32_t)(t % F.gamma);
+            const uint32_t cd = (uint32_t)(t / F.gamma) + 1u;
+            for (uint32_t l = 0; l < F.j; l++) { c[l] = (uint16_t)(low % E.q); low /= E.q; }
+            c[F.j] = (uint16_t)E.antilog[s];
+            c[F.i] = 1;
+            c[E.d] = (uint16_t)cd;
+        }
+        for (uint32_t l = 0; l < E.ncoef; l++) rows[r * E.ncoef + l] = c[l];
+        mult[r] = F.mult;
+    }
+}
+
+// tuples[m + r] = twist of tuples[r] (reading G8), weights copied.
+__global__ void __launch_bounds__(256) twist_kernel(uint32_t *tuples, unsigned long long *w, unsigned long long m, uint32_t g, uint32_t q) {
+    for (unsigned long long r = blockIdx.x * 256ull + threadIdx.x; r < m; r += gridDim.x * 256ull) {
+        unsigned long long qk = 1;
+        for (uint32_t k = 1; k <= g; k++) {
+            qk *= q;
+            const uint32_t v = tuples[r * g + k - 1];
+            tuples[(m + r) * g + k - 1] = (k & 1u) ? (uint32_t)(2 * qk + 2 - v) : v;
+        }
+        w[m + r] = w[r];
+    }
+}
+
+int build_families(uint32_t q, uint32_t g, uint32_t d, EnumParams &E) {
+    uint32_t p, r;
+    if (!hec_factor_q(q, &p, &r)) HEC_FAIL(HEC_ERR_INVALID_FIELD, "q must be an odd prime power below 65536");
+    if (g < 1 || g > HEC_MAX_GENUS) HEC_FAIL(HEC_ERR_INVALID_ARG, "g must be in [1, HEC_MAX_GENUS]");
+    if (d != 2 * g + 1 && d != 2 * g + 2) HEC_FAIL(HEC_ERR_INVALID_ARG, "d must be 2g+1 or 2g+2");
+    if (d % p == 0) HEC_FAIL(HEC_ERR_UNSUPPORTED, "reduced polynomials for p | d are not covered (reading G19)");
+    E.q = q; E.d = d; E.ncoef = 2 * g + 3; E.nfam = 0; E.antilog = nullptr;
+    unsigned long long at = 0;
+    const unsigned long long Q = q;
+    auto push = [&](uint32_t i, uint32_t j, uint32_t gamma, unsigned long long qj, unsigned long long size, unsigned long long mult) {
+        Family &F = E.fam[E.nfam++];
+        F.first = at; F.qj = qj; F.mult = mult; F.i = i; F.j = j; F.gamma = gamma;
+        at += size;
+    };
+    push(0, 0xFFFFFFFFu, 1, 1, Q - 1, Q * (Q - 1) / 2);
+    push(1, 0xFFFFFFFFu, 1, 1, Q - 1, Q * (Q - 1) / 2);
+    for (uint32_t i = 1; i + 2 <= d; i++) {
+        unsigned long long qj = 1;
+        for (uint32_t j = 0; j < i; j++) {
+            const uint32_t gamma = std::gcd(q - 1, i - j);
+            if (qj > (~0ull) / ((Q - 1) * gamma)) HEC_FAIL(HEC_ERR_UNSUPPORTED, "the number of reduced polynomials exceeds 2^64");
+            push(i, j, gamma, qj, (Q - 1) * gamma * qj, Q * (Q - 1) * (Q - 1) / (2ull * gamma));
+            qj *= Q;
+        }
+    }
+    E.total = at;
+    return HEC_OK;
+}
+
+}  // namespace
+
+namespace {
+
+struct Scratch {          // plain device buffer, freed on scope exit
+    void *p = nullptr;
+    ~Scratch() { if (p) cudaFree(p); }
+    int alloc(size_t bytes) {
+        if (cudaMalloc(&p, std::max<size_t>(bytes, 16)) != cudaSuccess) { cudaGetLastError(); p = nullptr; HEC_FAIL(HEC_ERR_NOMEM, "hec_enum: cudaMalloc failed"); }
+        return HEC_OK;
+    }
+};
+
+// alpha^0 .. alpha^15 of F_q on the device (gamma <= d - 2 <= 10 entries are ever read)
+int upload_generator_powers(uint32_t q, Scratch &buf, EnumParams &E) {
+    uint32_t p, r;
+    hec_factor_q(q, &p, &r);
+    const hec_field *Fq = hec_cached_field(p, r, 1);
+    if (!Fq) return HEC_ERR_INVALID_FIELD;
+    uint32_t h[16];
+    for (uint32_t s = 0; s < 16; s++) h[s] = Fq->antilog[s % (q - 1)];
+    int rc = buf.alloc(sizeof h);
+    if (rc) return rc;
+    HEC_CUDA_OK(cudaMemcpyAsync(buf.p, h, sizeof h, cudaMemcpyHostToDevice, hec_current_stream()));
+    HEC_CUDA_OK(cudaStreamSynchronize(hec_current_stream()));      // h is a stack array
+    E.antilog = static_cast<const uint32_t *>(buf.p);
+    return HEC_OK;
+}
+
+int launch_rows(const EnumParams &E, unsigned long long first, size_t n, uint16_t *d_rows, unsigned long long *d_mult, int sms) {
+    const unsigned grid = (unsigned)std::min<unsigned long long>((n + 255) / 256, (unsigned long long)sms * 8);
+    reduced_rows_kernel<<<grid, 256, 0, hec_current_stream()>>>(E, first, n, d_rows, d_mult);
+    hec_launch_counter::value++;
+    HEC_CUDA_OK(cudaGetLastError());
+    return HEC_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int hec_reduced_total(uint32_t q, uint32_t g, uint32_t d, uint64_t *out_total) {
+    if (!out_total) HEC_FAIL(HEC_ERR_INVALID_ARG, "out_total must not be NULL");
+    EnumParams E;
+    int rc = build_families(q, g, d, E);
+    if (rc) return rc;
+    *out_total = E.total;
+    return HEC_OK;
+}
+
+int hec_reduced_rows(uint32_t q, uint32_t g, uint32_t d, uint64_t first, size_t n, uint16_t *out_coeffs, uint64_t *out_mult) {
+    EnumParams E;
+    int rc = build_families(q, g, d, E);
+    if (rc) return rc;
+    if (first > E.total || n > E.total - first) HEC_FAIL(HEC_ERR_INVALID_ARG, "index range exceeds hec_reduced_total");
+    if (n == 0) return HEC_OK;
+    if (!out_coeffs || !out_mult) HEC_FAIL(HEC_ERR_INVALID_ARG, "out_coeffs and out_mult must not be NULL");
+    int sms = 0;
+    if ((rc = hec_ensure_device(&sms, nullptr))) return rc;
+    const bool dev = hec_is_device_pointer(out_coeffs);
+    if (hec_is_device_pointer(out_mult) != dev) HEC_FAIL(HEC_ERR_INVALID_ARG, "out_coeffs/out_mult must both be host or both device pointers");
+    Scratch gen, rows, mult;
+    if ((rc = upload_generator_powers(q, gen, E))) return rc;
+    uint16_t *d_rows = out_coeffs;
+    unsigned long long *d_mult = reinterpret_cast<unsigned long long *>(out_mult);
+    const size_t row_bytes = n * E.ncoef * sizeof(uint16_t);
+    if (!dev) {
+        if ((rc = rows.alloc(row_bytes)) || (rc = mult.alloc(n * 8))) return rc;
+        d_rows = static_cast<uint16_t *>(rows.p);
+        d_mult = static_cast<unsigned long long *>(mult.p);
+    }
+    if ((rc = launch_rows(E, first, n, d_rows, d_mult, sms))) return rc;
+    cudaStream_t st = hec_current_stream();
+    if (!dev) {
+        HEC_CUDA_OK(cudaMemcpyAsync(out_coeffs, d_rows, row_bytes, cudaMemcpyDeviceToHost, st));
+        HEC_CUDA_OK(cudaMemcpyAsync(out_mult, d_mult, n * 8, cudaMemcpyDeviceToHost, st));
+    }
+    HEC_CUDA_OK(cudaStreamSynchronize(st));
+    return HEC_OK;
+}
+
+int hec_curve_map(uint32_t q, uint32_t g, uint32_t d, uint32_t *out_tuples, uint64_t *out_weights, size_t cap, size_t *out_m) {
+    if (!out_m) HEC_FAIL(HEC_ERR_INVALID_ARG, "out_m must not be NULL");
+    *out_m = 0;
+    if (cap > 0 && (!out_tuples || !out_weights)) HEC_FAIL(HEC_ERR_INVALID_ARG, "out_tuples/out_weights must not be NULL when cap > 0");
+    EnumParams E;
+    int rc = build_families(q, g, d, E);
+    if (rc) return rc;
+    int sms = 0;
+    if ((rc = hec_ensure_device(&sms, nullptr))) return rc;
+    cudaStream_t st = hec_current_stream();
+    Scratch gen;
+    if ((rc = upload_generator_powers(q, gen, E))) return rc;
+
+    const size_t chunk = (size_t)std::min<unsigned long long>(E.total, 1ull << 22);
+    Scratch rows, mult, counts, flags, part_t, part_w, acc_t, acc_w, cat_t, cat_w;
+    if ((rc = rows.alloc(chunk * E.ncoef * 2)) || (rc = mult.alloc(chunk * 8)) || (rc = counts.alloc(chunk * g * 4)) ||
+        (rc = flags.alloc(chunk)) || (rc = part_t.alloc(chunk * g * 4)) || (rc = part_w.alloc(chunk * 8))) return rc;
+    size_t acc_m = 0, acc_cap = 0;
+    auto grow = [&](Scratch &t, Scratch &w, size_t &have, size_t need) -> int {
+        if (need <= have) return HEC_OK;
+        Scratch nt, nw;
+        int e;
+        const size_t want = std::max(need, 2 * have);
+        if ((e = nt.alloc(want * g * 4)) || (e = nw.alloc(want * 8))) return e;
+        std::swap(t.p, nt.p); std::swap(w.p, nw.p);      // callers never need the old contents
+        have = want;
+        return HEC_OK;
+    };
+    size_t cat_cap = 0;
+    for (unsigned long long first = 0; first < E.total; first += chunk) {
+        const size_t n = (size_t)std::min<unsigned long long>(chunk, E.total - first);
+        if ((rc = launch_rows(E, first, n, static_cast<uint16_t *>(rows.p), static_cast<unsigned long long *>(mult.p), sms))) return rc;
+        // Algorithm 1 lines 6-18 for the chunk, then the weighted histogram of its squarefree rows (line 20)
+        if ((rc = hec_count(q, g, static_cast<const uint16_t *>(rows.p), n, static_cast<uint32_t *>(counts.p), static_cast<uint8_t *>(flags.p)))) return rc;
+        size_t m = 0;
+        if ((rc = hec_histogram_weighted(static_cast<const uint32_t *>(counts.p), static_cast<const uint8_t *>(flags.p),
+                                         static_cast<const uint64_t *>(mult.p), n, g, static_cast<uint32_t *>(part_t.p),
+                                         static_cast<uint64_t *>(part_w.p), chunk, &m))) return rc;
+        if (m == 0) continue;
+        // running map <- merge(running map, chunk's map)
+        if ((rc = grow(cat_t, cat_w, cat_cap, acc_m + m))) return rc;
+        if (acc_m) {
+            HEC_CUDA_OK(cudaMemcpyAsync(cat_t.p, acc_t.p, acc_m * g * 4, cudaMemcpyDeviceToDevice, st));
+            HEC_CUDA_OK(cudaMemcpyAsync(cat_w.p, acc_w.p, acc_m * 8, cudaMemcpyDeviceToDevice, st));
+        }
+        HEC_CUDA_OK(cudaMemcpyAsync(static_cast<uint32_t *>(cat_t.p) + acc_m * g, part_t.p, m * g * 4, cudaMemcpyDeviceToDevice, st));
+        HEC_CUDA_OK(cudaMemcpyAsync(static_cast<uint64_t *>(cat_w.p) + acc_m, part_w.p, m * 8, cudaMemcpyDeviceToDevice, st));
+        if ((rc = grow(acc_t, acc_w, acc_cap, acc_m + m))) return rc;
+        size_t merged = 0;
+        if ((rc = hec_histogram_weighted(static_cast<const uint32_t *>(cat_t.p), nullptr, static_cast<const uint64_t *>(cat_w.p), acc_m + m, g,
+                                         static_cast<uint32_t *>(acc_t.p), static_cast<uint64_t *>(acc_w.p), acc_cap, &merged))) return rc;
+        acc_m = merged;
+    }
+    if (acc_m == 0) return HEC_OK;
+    // line 21: the same weight at the tuple of the quadratic twist (reading G8)
+    if ((rc = grow(cat_t, cat_w, cat_cap, 2 * acc_m))) return rc;
+    HEC_CUDA_OK(cudaMemcpyAsync(cat_t.p, acc_t.p, acc_m * g * 4, cudaMemcpyDeviceToDevice, st));
+    HEC_CUDA_OK(cudaMemcpyAsync(cat_w.p, acc_w.p, acc_m * 8, cudaMemcpyDeviceToDevice, st));
+    twist_kernel<<<(unsigned)std::min<size_t>((acc_m + 255) / 256, (size_t)sms * 8), 256, 0, st>>>(
+        static_cast<uint32_t *>(cat_t.p), static_cast<unsigned long long *>(cat_w.p), acc_m, g, q);
+    hec_launch_counter::value++;
+    HEC_CUDA_OK(cudaGetLastError());
+    Scratch fin_t, fin_w;
+    if ((rc = fin_t.alloc(2 * acc_m * g * 4)) || (rc = fin_w.alloc(2 * acc_m * 8))) return rc;
+    size_t fin_m = 0;
+    if ((rc = hec_histogram_weighted(static_cast<const uint32_t *>(cat_t.p), nullptr, static_cast<const uint64_t *>(cat_w.p), 2 * acc_m, g,
+                                     static_cast<uint32_t *>(fin_t.p), static_cast<uint64_t *>(fin_w.p), 2 * acc_m, &fin_m))) return rc;
+    *out_m = fin_m;
+    if (cap < fin_m) HEC_FAIL(HEC_ERR_CAPACITY, "hec_curve_map: cap is smaller than the number of distinct tuples");
+    const bool dev = hec_is_device_pointer(out_tuples);
+    if (hec_is_device_pointer(out_weights) != dev) HEC_FAIL(HEC_ERR_INVALID_ARG, "out_tuples/out_weights must both be host or both device pointers");
+    const cudaMemcpyKind kind = dev ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost;
+    HEC_CUDA_OK(cudaMemcpyAsync(out_tuples, fin_t.p, fin_m * g * 4, kind, st));
+    HEC_CUDA_OK(cudaMemcpyAsync(out_weights, fin_w.p, fin_m * 8, kind, st));
+    HEC_CUDA_OK(cudaStreamSynchronize(st));
+    return HEC_OK;
+}
+
+}  // extern "C"

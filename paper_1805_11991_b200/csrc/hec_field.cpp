@@ -4,6 +4,7 @@
 // from FLINT; here the generator is t modulo the lexicographically smallest primitive
 // polynomial (reading G7) and the tables come from one walk through the powers of t.
 #include <algorithm>
+#include <atomic>
 #include <map>
 #include <memory>
 #include <mutex>
@@ -78,6 +79,7 @@ bool walk_powers(const Ring &R, uint32_t Q, std::vector<uint32_t> &antilog) {
 }
 
 std::mutex g_cache_mutex;
+std::atomic<bool> g_device_build{false};
 std::map<std::tuple<uint32_t, uint32_t, uint32_t>, std::unique_ptr<hec_field>> g_cache;
 
 hec_field *build_field_impl(uint32_t p, uint32_t r, uint32_t k) {
@@ -196,7 +198,10 @@ const hec_field *hec_cached_field(uint32_t p, uint32_t r, uint32_t k) {
         auto it = g_cache.find(std::make_tuple(p, r, k));
         if (it != g_cache.end()) return it->second.get();
     }
-    hec_field *F = build_field_impl(p, r, k);      // may recurse into the cache for (p, r, 1)
+    uint64_t Q = 1;
+    for (uint32_t i = 0; i < r * k && Q <= HEC_MAX_FIELD_SIZE; i++) Q *= p;
+    const bool on_device = g_device_build.load() && Q > kDeviceBuildMinQ && Q <= HEC_MAX_FIELD_SIZE && p < 65536;
+    hec_field *F = on_device ? hec_build_field_device_impl(p, r, k) : build_field_impl(p, r, k);   // may recurse into the cache for (p, r, 1)
     if (!F) return nullptr;
     std::lock_guard<std::mutex> lock(g_cache_mutex);
     auto &slot = g_cache[std::make_tuple(p, r, k)];
@@ -204,6 +209,8 @@ const hec_field *hec_cached_field(uint32_t p, uint32_t r, uint32_t k) {
     slot.reset(F);
     return F;
 }
+
+void hec_allow_device_field_build(bool on) { g_device_build.store(on); }
 
 void hec_clear_field_cache() {
     std::lock_guard<std::mutex> lock(g_cache_mutex);

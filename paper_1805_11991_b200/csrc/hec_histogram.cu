@@ -409,6 +409,12 @@ extern "C" int hec_histogram(const uint32_t *counts, const uint8_t *mask, size_t
     return histogram_impl(counts, mask, nullptr, n, g, out_tuples, out_mult, cap, out_m);
 }
 
+// hec_enum.cu: weighted histogram of the rows with a nonzero mask (Algorithm 1 line 20 for one chunk).
+int hec_histogram_weighted(const uint32_t *counts, const uint8_t *mask, const uint64_t *weights, size_t n, uint32_t g,
+                           uint32_t *out_tuples, uint64_t *out_mult, size_t cap, size_t *out_m) {
+    return histogram_impl(counts, mask, weights, n, g, out_tuples, out_mult, cap, out_m);
+}
+
 extern "C" int hec_histogram_merge(const uint32_t *in_tuples, const uint64_t *in_mult, size_t n, uint32_t g,
                                    uint32_t *out_tuples, uint64_t *out_mult, size_t cap, size_t *out_m) {
     if (n > 0 && !in_mult) HEC_FAIL(HEC_ERR_INVALID_ARG, "in_mult must not be NULL");

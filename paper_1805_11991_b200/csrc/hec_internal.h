@@ -30,6 +30,11 @@ bool hec_factor_q(uint32_t q, uint32_t *p, uint32_t *r);
 // Cached, library-owned fields used by hec_count (never freed before hec_shutdown).
 const hec_field *hec_cached_field(uint32_t p, uint32_t r, uint32_t k);
 void hec_clear_field_cache();
+// Tables built on the device (hec_field_device.cu); same result as the host build.
+hec_field *hec_build_field_device_impl(uint32_t p, uint32_t r, uint32_t k);
+// hec_cached_field builds fields above this size on the device once hec_count has initialised one.
+constexpr uint32_t kDeviceBuildMinQ = 1u << 16;
+void hec_allow_device_field_build(bool on);
 
 // ---------------------------------------------------------------------------- device side
 // Geometry of one extended Zech table.  Stored value of a lookup result:

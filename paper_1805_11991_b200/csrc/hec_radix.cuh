@@ -316,14 +316,16 @@ __device__ __forceinline__ bool all_classes_present(const uint32_t nz) {
 // ---------------------------------------------------------------------------------------------------------
 // All x in F_{q^k}^x for one curve, one warp.  lcj: lane j holds the log of c_j in this field (any value when
 // c_j = 0), nz: bit j set iff c_j != 0, scratch: kScratchWords words of shared memory owned by this warp.
-// Returns this lane's share of n_zero = #{x != 0: f(x) = 0} and n_sq = #{x != 0: f(x) a nonzero square}.
+// Returns this lane's share of n_zero = #{x != 0: f(x) = 0} and n_sq = #{x != 0: f(x) a nonzero square}, over the
+// cosets of part `part` of `splits` (splits = 1: all of them; splits > 1 spreads one curve over many warps, the
+// single-curve / small-batch mode of SURVEY.md 8(f) NEXT-2).
 // ALL: the caller guarantees that every residue class mod R holds a nonzero coefficient (the straight-line
 // network); otherwise the network takes warp-uniform branches around the absent classes.
 // ---------------------------------------------------------------------------------------------------------
 template <int D, int R, bool ALL, typename Ar, typename Pol>
 __device__ __forceinline__ void radix_all_x(const Pol pol, const uint32_t M, const uint32_t rcpM, const uint32_t lane,
                                             const uint32_t nz, const uint32_t lcj, volatile uint32_t *scratch,
-                                            uint32_t &n_sq, uint32_t &n_zero) {
+                                            const uint32_t part, const uint32_t splits, uint32_t &n_sq, uint32_t &n_zero) {
     constexpr int L = Ar::LANES;
     constexpr int NT = D + 1 > R ? D + 1 - R : 0;      // terms 0 .. NT-1 can continue a chain
     constexpr int NTA = NT > 0 ? NT : 1;
@@ -334,6 +336,17 @@ __device__ __forceinline__ void radix_all_x(const Pol pol, const uint32_t M, con
         return r >= M ? r - M : r;
     };
 
+    // this warp's share of the cosets: [c_lo, c_hi), part `part` of `splits` equal chunks (a multiple of 32 L cosets)
+    uint32_t c_lo = 0, c_hi = S;
+    if (splits > 1u) {
+        const uint32_t chunk = ((S + splits - 1u) / splits + 32u * L - 1u) / (32u * L) * (32u * L);
+        c_lo = min(S, part * chunk);
+        c_hi = min(S, c_lo + chunk);
+    }
+    n_sq = 0;
+    n_zero = 0;
+    if (c_lo >= c_hi) return;                          // warp-uniform
+
     __syncwarp();
     if (lane <= (uint32_t)D) scratch[lane] = lcj;
     __syncwarp();
@@ -341,7 +354,7 @@ __device__ __forceinline__ void radix_all_x(const Pol pol, const uint32_t M, con
     // ---- per-curve structure (warp-uniform) and this lane's chain offsets for its first cosets
     uint32_t n0[L];
 #pragma unroll
-    for (int c = 0; c < L; c++) n0[c] = lane + 32u * c < S ? lane + 32u * c : 0u;
+    for (int c = 0; c < L; c++) n0[c] = c_lo + lane + 32u * c < c_hi ? c_lo + lane + 32u * c : 0u;
     const uint32_t step = mod(32u * L);
     uint32_t ul[NTA], inc[NTA], kc[R], kinc[R];
     uint32_t cm = 0, present = 0;
@@ -386,7 +399,7 @@ __device__ __forceinline__ void radix_all_x(const Pol pol, const uint32_t M, con
             odd_exact += res & 0xFFFFu;
         }
     };
-    for (uint32_t base = 0; base < S; base += 32u * L) {
+    for (uint32_t base = c_lo; base < c_hi; base += 32u * L) {
         uint32_t v[R];
         uint32_t mn = ar.mn_init();
 #pragma unroll
@@ -412,7 +425,7 @@ __device__ __forceinline__ void radix_all_x(const Pol pol, const uint32_t M, con
         bool any_flag = false;
 #pragma unroll
         for (int c = 0; c < L; c++) {
-            valid[c] = base + lane + 32u * c < S;
+            valid[c] = base + lane + 32u * c < c_hi;
             flag[c] = valid[c] && ar.flagged(mn, c);
             any_flag |= flag[c];
         }
@@ -442,8 +455,8 @@ __device__ __forceinline__ void radix_all_x(const Pol pol, const uint32_t M, con
     uint32_t n_valid = 0;                              // cosets of this lane
 #pragma unroll
     for (int c = 0; c < L; c++) {
-        const uint32_t first = lane + 32u * c;
-        if (first < S) n_valid += (S - first + 32u * L - 1u) / (32u * L);
+        const uint32_t first = c_lo + lane + 32u * c;
+        if (first < c_hi) n_valid += (c_hi - first + 32u * L - 1u) / (32u * L);
     }
     const uint32_t n_nz = (n_valid - pushed) * R + nz_exact;        // every value of an unflagged coset is nonzero
     const uint32_t n_odd = odd_fast + odd_exact;

@@ -30,10 +30,10 @@ MAX_GENUS = 5
 
 # every symbol include/hec.h declares (tests check the library exports all of them)
 SYMBOLS = [
-    "hec_last_error", "hec_last_error_index", "hec_build_field", "hec_free_field", "hec_field_p",
+    "hec_last_error", "hec_last_error_index", "hec_build_field", "hec_build_field_device", "hec_free_field", "hec_field_p",
     "hec_field_degree", "hec_field_q", "hec_field_Q", "hec_field_embed_unit", "hec_field_modulus",
     "hec_field_antilog", "hec_field_log", "hec_field_zech", "hec_field_embed", "hec_count", "hec_histogram",
-    "hec_histogram_merge",
+    "hec_histogram_merge", "hec_reduced_total", "hec_reduced_rows", "hec_curve_map",
     "hec_set_stream", "hec_set_regime", "hec_set_eval", "hec_last_count_stats", "hec_launch_count", "hec_gather_bench",
     "hec_shutdown",
 ]
@@ -49,7 +49,7 @@ class CountStats(ctypes.Structure):
     _fields_ = [("count_kernel_ms", ctypes.c_float), ("squarefree_kernel_ms", ctypes.c_float),
                 ("launches", ctypes.c_uint32), ("regime", ctypes.c_uint32), ("smem_bytes", ctypes.c_uint32),
                 ("grid", ctypes.c_uint32), ("block", ctypes.c_uint32), ("chains_per_lane", ctypes.c_uint32),
-                ("table_mode", ctypes.c_uint32), ("radix_fields", ctypes.c_uint32)]
+                ("table_mode", ctypes.c_uint32), ("radix_fields", ctypes.c_uint32), ("splits", ctypes.c_uint32)]
 
 
 def lib():
@@ -65,6 +65,8 @@ def lib():
         L.hec_last_error_index.restype = sz
         L.hec_build_field.restype = vp
         L.hec_build_field.argtypes = [u32, u32, u32]
+        L.hec_build_field_device.restype = vp
+        L.hec_build_field_device.argtypes = [u32, u32, u32]
         L.hec_free_field.argtypes = [vp]
         for name in ("p", "degree", "q", "Q", "embed_unit"):
             f = getattr(L, f"hec_field_{name}")
@@ -75,6 +77,9 @@ def lib():
         L.hec_count.argtypes = [u32, u32, vp, sz, vp, vp]
         L.hec_histogram.argtypes = [vp, vp, sz, u32, vp, vp, sz, ctypes.POINTER(sz)]
         L.hec_histogram_merge.argtypes = [vp, vp, sz, u32, vp, vp, sz, ctypes.POINTER(sz)]
+        L.hec_reduced_total.argtypes = [u32, u32, u32, ctypes.POINTER(ctypes.c_uint64)]
+        L.hec_reduced_rows.argtypes = [u32, u32, u32, ctypes.c_uint64, sz, vp, vp]
+        L.hec_curve_map.argtypes = [u32, u32, u32, vp, vp, sz, ctypes.POINTER(sz)]
         L.hec_set_stream.argtypes = [vp]
         L.hec_set_regime.argtypes = [ctypes.c_int]
         L.hec_set_eval.argtypes = [ctypes.c_int]
@@ -107,9 +112,9 @@ def _ptr(x):
 class Field:
     """hec_build_field handle with the read-only accessors of hec.h (paper's conventions)."""
 
-    def __init__(self, p: int, r: int, k: int):
+    def __init__(self, p: int, r: int, k: int, device: bool = False):
         L = lib()
-        self._h = L.hec_build_field(p, r, k)
+        self._h = (L.hec_build_field_device if device else L.hec_build_field)(p, r, k)
         if not self._h:
             raise HecError(HEC_ERR_INVALID_FIELD, L.hec_last_error().decode())
         self.p, self.r, self.k = p, r, k
@@ -157,6 +162,11 @@ class Field:
 
 def build_field(p: int, r: int, k: int) -> Field:
     return Field(p, r, k)
+
+
+def build_field_device(p: int, r: int, k: int) -> Field:
+    """hec_build_field_device: same tables, built by CUDA kernels on the current stream (needs a GPU)."""
+    return Field(p, r, k, device=True)
 
 
 def set_stream(cuda_stream: int | None):
@@ -245,6 +255,41 @@ def histogram_merge(tuples, mult):
     if not _is_torch(mult):
         mult = np.ascontiguousarray(mult, dtype=np.uint64)
     return histogram(tuples, None, _weights=mult)
+
+
+def reduced_total(q: int, g: int, d: int) -> int:
+    """hec_reduced_total: number of reduced polynomials of degree d (before the squarefree filter)."""
+    t = ctypes.c_uint64(0)
+    _check(lib().hec_reduced_total(q, g, d, ctypes.byref(t)))
+    return int(t.value)
+
+
+def reduced_rows(q: int, g: int, d: int, first: int, n: int, device=None):
+    """hec_reduced_rows: rows [first, first + n) of the enumeration as (coeffs [n][2g+3], mult [n]); numpy arrays,
+    or torch tensors on `device` when given."""
+    if device is not None:
+        import torch
+        rows = torch.empty((n, 2 * g + 3), dtype=torch.int16, device=device)
+        mult = torch.empty((n,), dtype=torch.int64, device=device)
+    else:
+        rows = np.empty((n, 2 * g + 3), dtype=np.uint16)
+        mult = np.empty((n,), dtype=np.uint64)
+    _check(lib().hec_reduced_rows(q, g, d, ctypes.c_uint64(first), ctypes.c_size_t(n), _ptr(rows), _ptr(mult)))
+    return rows, mult
+
+
+def curve_map(q: int, g: int, d: int):
+    """hec_curve_map (two-call capacity protocol): (tuples [m][g] uint32, weights [m] uint64) on the host."""
+    L = lib()
+    m = ctypes.c_size_t(0)
+    rc = L.hec_curve_map(q, g, d, None, None, ctypes.c_size_t(0), ctypes.byref(m))
+    if rc not in (HEC_OK, HEC_ERR_CAPACITY):
+        _check(rc)
+    tup = np.empty((m.value, g), dtype=np.uint32)
+    w = np.empty((m.value,), dtype=np.uint64)
+    if m.value:
+        _check(L.hec_curve_map(q, g, d, _ptr(tup), _ptr(w), ctypes.c_size_t(m.value), ctypes.byref(m)))
+    return tup[: m.value], w[: m.value]
 
 
 def last_count_stats() -> dict:

@@ -41,9 +41,28 @@ def test_invalid_fields():
             hec.build_field(p, r, k)
 
 
-@pytest.fixture(scope="module", params=FIELDS, ids=lambda f: f"p{f[0]}r{f[1]}k{f[2]}")
+# every invariant below runs on the host-built tables (-m "not gpu") and on the tables built by the CUDA kernels of
+# hec_build_field_device (-m gpu)
+_PARAMS = [pytest.param((f, False), id=f"p{f[0]}r{f[1]}k{f[2]}") for f in FIELDS] + \
+          [pytest.param((f, True), id=f"p{f[0]}r{f[1]}k{f[2]}-device", marks=pytest.mark.gpu) for f in FIELDS]
+
+
+@pytest.fixture(scope="module", params=_PARAMS)
 def field(request):
-    return hec.build_field(*request.param)
+    f, device = request.param
+    return hec.build_field_device(*f) if device else hec.build_field(*f)
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("f", FIELDS + [(1009, 1, 2), (3, 1, 13), (5, 1, 9), (11, 3, 2), (3001, 1, 2)],
+                         ids=lambda f: f"p{f[0]}r{f[1]}k{f[2]}")
+def test_device_build_equals_host_build(f):
+    """hec_build_field_device (order-test modulus search + antilog / log / Zech kernels) against hec_build_field (one
+    walk through the powers of t on the host): same modulus, same tables, entry for entry."""
+    H, D = hec.build_field(*f), hec.build_field_device(*f)
+    assert H.modulus == D.modulus and H.Q == D.Q and H.embed_unit == D.embed_unit
+    for name in ("antilog", "log", "zech", "embed"):
+        assert np.array_equal(getattr(H, name), getattr(D, name)), name
 
 
 def test_modulus_is_smallest_primitive(field):

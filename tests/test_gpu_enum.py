@@ -1,0 +1,123 @@
+"""GPU parity for SURVEY.md 8(f) NEXT-1 (hec_reduced_rows, hec_curve_map) against oracle/hec_enum_oracle.py.
+
+The two sides choose DIFFERENT coset representatives R_m (library: powers of its generator; oracle: smallest
+encodings), so they enumerate different reduced sets; what is unique -- the weighted map N_{g,d} -- must agree
+bit for bit, and the library's rows are checked for validity (reduced form, distinct cosets, multiplicities)."""
+import math
+
+import numpy as np
+import pytest
+
+from oracle import hec_enum_oracle as E
+from paper_1805_11991_b200 import hec
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def cuda():
+    import torch
+    from paper_1805_11991_b200 import build as hb
+    hb.build_lib()
+    assert torch.cuda.is_available()
+    torch.cuda.set_device(0)
+    hec.set_stream(torch.cuda.current_stream().cuda_stream)
+    hec.set_regime(hec.REGIME_AUTO)
+    hec.set_eval(hec.EVAL_AUTO)
+    return torch
+
+
+@pytest.mark.parametrize("q,g,d", [(3, 2, 5), (5, 2, 6), (7, 2, 5), (9, 2, 5), (25, 2, 6), (13, 4, 9), (49, 3, 8)])
+def test_reduced_rows_are_valid(cuda, q, g, d):
+    total = hec.reduced_total(q, g, d)
+    want = 2 * (q - 1) + sum((q - 1) * math.gcd(q - 1, i - j) * q ** j for i in range(1, d - 1) for j in range(i))
+    assert total == want
+    n = min(total, 200000)
+    first = 0 if total == n else total - n                 # the tail holds the large families
+    rows, mult = hec.reduced_rows(q, g, d, first, n)
+    drows, dmult = hec.reduced_rows(q, g, d, first, n, device="cuda")
+    assert (drows.cpu().numpy().view(np.uint16) == rows).all() and (dmult.cpu().numpy().view(np.uint64) == mult).all()
+    # ragged sub-range addressed by index
+    sub, smult = hec.reduced_rows(q, g, d, first + 17, min(n - 17, 1001))
+    assert (sub == rows[17:17 + len(sub)]).all() and (smult == mult[17:17 + len(sub)]).all()
+    assert (rows[:, d] != 0).all() and (rows[:, d - 1] == 0).all() and (rows[:, d + 1:] == 0).all() and (rows < q).all()
+    assert len(np.unique(rows, axis=0)) == n
+    F = E.Fq(q)
+    cosets = {}
+    for c, m in zip(rows[:: max(1, n // 4000)], mult[:: max(1, n // 4000)]):
+        supp = np.flatnonzero(c[:d])
+        i = supp[-1]
+        assert c[i] == 1
+        if len(supp) == 1:
+            assert i in (0, 1) and m == q * (q - 1) // 2
+        else:
+            j = supp[-2]
+            assert m == q * (q - 1) ** 2 // (2 * math.gcd(q - 1, i - j))
+            cosets.setdefault((int(i), int(j)), set()).add(int(c[j]))
+    for (i, j), reps in cosets.items():                      # the c_j seen lie in pairwise different cosets of (i-j)-th powers
+        gam = math.gcd(q - 1, i - j)
+        assert len(reps) <= gam
+        reps = sorted(reps)
+        for a in range(len(reps)):
+            for b in range(a):
+                assert F.pow(F.mul(reps[a], F.inv(reps[b])), (q - 1) // gam) != 1
+
+
+@pytest.mark.parametrize("q,g,d", [(3, 2, 5), (3, 1, 4), (5, 1, 3), (5, 1, 4), (7, 1, 3), (7, 1, 4), (5, 2, 6), (7, 2, 5)])
+def test_curve_map_equals_the_definition(cuda, q, g, d):
+    tup, w = hec.curve_map(q, g, d)
+    otup, ow = E.map_to_arrays(E.brute_force_map(q, g, d), g)
+    assert tup.shape == otup.shape and (tup == otup).all() and (w == ow).all()
+
+
+@pytest.mark.parametrize("q,g,d", [(9, 2, 5), (11, 2, 6), (13, 2, 5), (13, 2, 6), (25, 1, 4), (27, 1, 4), (7, 3, 8)])
+def test_curve_map_equals_algorithm1_oracle(cuda, q, g, d):
+    tup, w = hec.curve_map(q, g, d)
+    otup, ow = E.map_to_arrays(E.reduced_map(q, g, d), g)
+    assert tup.shape == otup.shape and (tup == otup).all() and (w == ow).all()
+    assert int(w.sum()) == (q - 1) * (q ** d - q ** (d - 1))
+
+
+def test_curve_map_multichunk(cuda):
+    """More than one chunk of 2^22 reduced polynomials (q = 13, g = 3, d = 8: 5.66e6, two chunks): the map against the same
+    pipeline assembled by hand with another chunking (hec_reduced_rows -> hec_count -> numpy), the closed-form total
+    and the twist symmetry."""
+    q, g, d = 13, 3, 8
+    total = hec.reduced_total(q, g, d)
+    assert total > (1 << 22)
+    tup, w = hec.curve_map(q, g, d)
+    assert int(w.sum()) == (q - 1) * (q ** d - q ** (d - 1))
+    acc = {}
+    step = 1_500_001
+    for first in range(0, total, step):
+        n = min(step, total - first)
+        rows, mult = hec.reduced_rows(q, g, d, first, n, device="cuda")
+        cnt, sf = hec.count(q, g, rows)
+        cnt = cnt.cpu().numpy().view(np.uint32).astype(np.uint64)
+        keep = sf.cpu().numpy() != 0
+        key = (cnt[:, 0] << np.uint64(44)) | (cnt[:, 1] << np.uint64(22)) | cnt[:, 2]
+        m = mult.cpu().numpy().view(np.uint64)
+        u, inv = np.unique(key[keep], return_inverse=True)
+        s = np.zeros(len(u), dtype=np.uint64)
+        np.add.at(s, inv, m[keep])
+        for k, v in zip(u.tolist(), s.tolist()):
+            acc[k] = acc.get(k, 0) + v
+    full = {}
+    for k, v in acc.items():
+        t = (k >> 44, (k >> 22) & ((1 << 22) - 1), k & ((1 << 22) - 1))
+        for tt in (t, E.twist_tuple(q, t)):
+            full[tt] = full.get(tt, 0) + v
+    otup, ow = E.map_to_arrays(full, g)
+    assert tup.shape == otup.shape and (tup == otup).all() and (w == ow).all()
+
+
+def test_errors(cuda):
+    for q, g, d in [(3, 2, 6), (49, 3, 7), (25, 2, 5)]:         # p | d: reading G19
+        with pytest.raises(hec.HecError) as e:
+            hec.curve_map(q, g, d)
+        assert e.value.code == hec.HEC_ERR_UNSUPPORTED
+    with pytest.raises(hec.HecError) as e:
+        hec.reduced_total(7, 2, 4)
+    assert e.value.code == hec.HEC_ERR_INVALID_ARG
+    with pytest.raises(hec.HecError):
+        hec.reduced_rows(7, 2, 5, hec.reduced_total(7, 2, 5) - 3, 4)

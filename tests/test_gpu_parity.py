@@ -350,3 +350,58 @@ def test_every_radix_against_oracle(torch_cuda, cap):
     finally:
         hec.set_regime(hec.REGIME_AUTO)
         hec.set_eval(hec.EVAL_AUTO)
+
+
+# ------------------------------------------------------------------------------------------ small batches / single curve
+# the workload of the paper's Table 1 is ONE genus-2 curve over F_p and
+# F_{p^2}; hec_count then spreads the curve over the whole GPU (stats["splits"] warps per curve, atomics into the
+# pre-zeroed counts) and, above 2^16 elements, builds the field tables with the kernels of hec_build_field_device.
+
+TABLE1_CURVE = [17, 12, 16, 11, 10, 13, 12]     # Y^2 = 12X^6 + 13X^5 + 10X^4 + 11X^3 + 16X^2 + 12X + 17, c_0 first
+
+
+@pytest.mark.parametrize("p", [101, 211, 503, 1009])
+def test_table1_single_curve(torch_cuda, p):
+    rows = np.array([[c % p for c in TABLE1_CURVE]], dtype=np.uint16)
+    cnt, sf = _assert_parity(torch_cuda, p, 2, rows)
+    st = hec.last_count_stats()
+    if torch_cuda.eval_scheme == "auto":
+        assert st["splits"] > 1, st
+    # Weil bound for a squarefree genus-2 curve
+    if sf[0]:
+        for k in (1, 2):
+            assert abs(int(cnt[0, k - 1]) - (p ** k + 1)) <= 4 * p ** (k / 2)
+
+
+def test_table1_single_curve_p3001(torch_cuda):
+    if torch_cuda.eval_scheme != "auto":
+        pytest.skip("one warp for 9e6 points: the split mode exists for the radix scheme only")
+    p = 3001
+    rows = np.array([[c % p for c in TABLE1_CURVE]], dtype=np.uint16)
+    _assert_parity(torch_cuda, p, 2, rows)
+    assert hec.last_count_stats()["splits"] > 1
+
+
+@pytest.mark.parametrize("cid", [3, 4, 5])
+@pytest.mark.parametrize("n", [1, 2, 7, 33, 300])
+def test_small_batches_use_split_mode_and_agree_with_big_batches(torch_cuda, cid, n):
+    cfg = W.CONFIGS[cid]
+    big = W.generate(cfg, 0, 12000)             # above 2 * 148 * 32 rows: one warp per curve, no atomics
+    cnt_big, sf_big = _gpu_count(torch_cuda, cfg.q, cfg.g, big)
+    if torch_cuda.eval_scheme == "auto":
+        assert hec.last_count_stats()["splits"] == 1
+    cnt, sf = _gpu_count(torch_cuda, cfg.q, cfg.g, big[:n])
+    if torch_cuda.eval_scheme == "auto":
+        assert hec.last_count_stats()["splits"] > 1
+    assert (cnt == cnt_big[:n]).all() and (sf == sf_big[:n]).all()
+    m = min(n, 4 if cid == 3 else 16)
+    ocnt, osf, _ = O.count(cfg.q, cfg.g, big[:m])
+    assert (cnt[:m] == ocnt).all() and (sf[:m] == osf).all()
+
+
+def test_split_mode_edge_rows(torch_cuda):
+    """Degenerate rows (monomials, empty residue classes, zero-heavy) in split mode: few rows of a large field."""
+    q, g = 293, 2
+    rows = W.edge_rows(q, g)
+    for lo in range(0, len(rows), 9):
+        _assert_parity(torch_cuda, q, g, rows[lo:lo + 9])
