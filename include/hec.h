@@ -158,6 +158,32 @@ int hec_histogram_merge(const uint32_t *in_tuples, const uint64_t *in_mult, size
  * #{f squarefree of degree d over F_q with that tuple} (eq. (1.2) without lambda).  Output as for hec_histogram:
  * ascending lexicographic tuples, uint64 weights, two-call capacity protocol (*out_m always set).
  */
+/* ------------------------------------------------------------------------------------------------
+ * lambda(f): SURVEY.md 8(f) NEXT-3 (Algorithm 1 line 18: "compute lambda from r0 if
+ * possible; otherwise by factoring").
+ *
+ * hec_count_ex = hec_count plus two optional outputs (same pointer rules; NULL = not wanted):
+ *   out_roots[n][g]  uint32  r0_k = #{x in F_{q^k} : f(x) = 0}, the affine zeros
+ *   out_lambda[n]    uint8   index (hec_lambda_partitions) of the factorisation type of f over F_q: the partition
+ *                            of 2g+2 into the degrees of the irreducible factors, for degree 2g+1 amended by a summand 1
+ *                            (PAPER.md:61); 0xFF when f is not squarefree.
+ * How: r0_k = sum_{e | k} e n_e (n_e = number of irreducible factors of degree e), so Moebius inversion gives n_e for
+ * e <= g; the rest of the degree is one irreducible factor, except when it is 2g+2 (no factor of degree <= g): then
+ * Stickelberger's theorem decides between "irreducible" and "two factors of degree g+1" by the quadratic character
+ * of disc(f), which the squarefree kernel's Euclid run on (f, f') yields for free -- no factoring is ever needed.
+ *
+ * hec_lambda_partitions: the partitions of 2g+2 as multiplicity vectors (n_1 .. n_{2g+2}), out_parts[count][2g+2],
+ * in ascending lexicographic order of that vector; the row number is the lambda index.  Two-call capacity protocol.
+ * Host pointers only; needs no device.
+ *
+ * hec_curve_map_lambda: hec_curve_map with the full key of the paper's map (1.2), PAPER.md:63-67:
+ * out_keys[m][g+1] = (N_1 .. N_g, lambda index); g <= HEC_MAX_GENUS - 1.
+ */
+int hec_count_ex(uint32_t q, uint32_t g, const uint16_t *coeffs, size_t n, uint32_t *out_counts, uint8_t *out_squarefree,
+                 uint32_t *out_roots, uint8_t *out_lambda);
+int hec_lambda_partitions(uint32_t g, uint8_t *out_parts, size_t cap, size_t *out_count);
+int hec_curve_map_lambda(uint32_t q, uint32_t g, uint32_t d, uint32_t *out_keys, uint64_t *out_weights, size_t cap, size_t *out_m);
+
 int hec_reduced_total(uint32_t q, uint32_t g, uint32_t d, uint64_t *out_total);
 int hec_reduced_rows(uint32_t q, uint32_t g, uint32_t d, uint64_t first, size_t n, uint16_t *out_coeffs, uint64_t *out_mult);
 int hec_curve_map(uint32_t q, uint32_t g, uint32_t d, uint32_t *out_tuples, uint64_t *out_weights, size_t cap, size_t *out_m);

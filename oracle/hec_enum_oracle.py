@@ -143,6 +143,40 @@ def brute_force_map(q: int, g: int, d: int) -> dict:
     return dict(out)
 
 
+def reduced_map_lambda(q: int, g: int, d: int) -> dict:
+    """Algorithm 1 for one d with the full key of (1.2): {((N_1..N_g), lambda): weighted count}, lambda a multiplicity
+    vector (oracle/hec_lambda_oracle.py).  The twist n f has the factorisation type of f."""
+    from oracle import hec_lambda_oracle as LO
+    polys, mults = [], []
+    for c, m in reduced_polynomials(q, d):
+        polys.append(c)
+        mults.append(m)
+    rows = _pad(polys, g)
+    cnt, sf, _ = O.count(q, g, rows)
+    lam = LO.lambda_by_roots(q, g, rows)
+    out: Counter = Counter()
+    for row, flag, m, la in zip(cnt, sf, mults, lam):
+        if not flag:
+            continue
+        t = tuple(int(v) for v in row)
+        out[(t, la)] += m
+        out[(twist_tuple(q, t), la)] += m
+    return dict(out)
+
+
+def brute_force_map_lambda(q: int, g: int, d: int) -> dict:
+    """The definition (1.2): every polynomial of degree d, keyed by ((N_1..N_g), lambda)."""
+    from oracle import hec_lambda_oracle as LO
+    rows = _pad([list(low) + [cd] for cd in range(1, q) for low in itertools.product(range(q), repeat=d)], g)
+    cnt, sf, _ = O.count(q, g, rows)
+    lam = LO.lambda_by_roots(q, g, rows)
+    out: Counter = Counter()
+    for row, flag, la in zip(cnt, sf, lam):
+        if flag:
+            out[(tuple(int(v) for v in row), la)] += 1
+    return dict(out)
+
+
 def map_to_arrays(m: dict, g: int):
     """Sorted (tuples[n][g] uint32, weights[n] uint64), ascending lexicographic order."""
     keys = sorted(m)

@@ -293,6 +293,22 @@ static uint32_t count_points(const ext_field *F, const uint16_t *c, uint32_t nco
     return N;
 }
 
+/* r0_k = #{x in F_{q^k} : f(x) = 0}, the affine zeros only: the input of "compute lambda from r0"
+ * (Algorithm 1 line 18). */
+static uint32_t count_roots(const ext_field *F, const uint16_t *c, uint32_t ncoef) {
+    uint32_t N = 0;
+    for (uint64_t e = 0; e < F->Q; e++) {
+        elt x = elt_from_int(&F->E, e);
+        elt acc = F->iota[c[ncoef - 1]];
+        for (uint32_t i = ncoef - 1; i-- > 0;) {
+            acc = elt_mul(&F->E, &acc, &x);
+            acc = elt_add(&F->E, &acc, &F->iota[c[i]]);
+        }
+        N += (uint32_t)elt_is_zero(&F->E, &acc);
+    }
+    return N;
+}
+
 /* ------------------------------------------------- squarefree: gcd(f, f') over F_q */
 
 typedef struct { int deg; elt c[ORC_MAXDEG + 1]; } fpoly;   /* deg = -1 for the zero polynomial */
@@ -386,6 +402,36 @@ int orc_count_range(uint32_t p, uint32_t r, uint32_t g, const uint16_t *coeffs, 
     }
     for (uint32_t k = k_lo; k <= k_hi; k++) ext_field_free(&F[k]);
     if (threads_used) *threads_used = used;
+    return 0;
+}
+
+/* out_roots[n][width], columns k_lo-1 .. k_hi-1: r0_k of every row (same argument rules as orc_count_range). */
+int orc_roots_range(uint32_t p, uint32_t r, uint32_t g, const uint16_t *coeffs, size_t n,
+                    uint32_t k_lo, uint32_t k_hi, uint32_t width, uint32_t *out_roots, int nthreads) {
+    if (p < 3 || r < 1 || g < 1 || 2 * g + 2 > ORC_MAXDEG) return -10;
+    if (k_lo < 1 || k_hi > width || width >= ORC_MAXDEG || k_lo > k_hi + 1) return -13;
+    uint32_t ncoef = 2 * g + 3;
+    uint32_t q = 1;
+    for (uint32_t i = 0; i < r; i++) q *= p;
+    for (size_t i = 0; i < n; i++) {
+        const uint16_t *c = coeffs + i * ncoef;
+        for (uint32_t j = 0; j < ncoef; j++) if (c[j] >= q) return -11;
+        if (c[ncoef - 1] == 0 && c[ncoef - 2] == 0) return -12;
+    }
+    ext_field F[ORC_MAXDEG];
+    for (uint32_t k = k_lo; k <= k_hi; k++)
+        if (ext_field_init(&F[k], p, r, k)) return -10;
+#ifdef _OPENMP
+    if (nthreads > 0) omp_set_num_threads(nthreads);
+#endif
+    (void)nthreads;
+#pragma omp parallel for schedule(dynamic, 1)
+    for (long long i = 0; i < (long long)n; i++) {
+        const uint16_t *c = coeffs + (size_t)i * ncoef;
+        for (uint32_t k = k_lo; k <= k_hi; k++)
+            out_roots[(size_t)i * width + (k - 1)] = count_roots(&F[k], c, ncoef);
+    }
+    for (uint32_t k = k_lo; k <= k_hi; k++) ext_field_free(&F[k]);
     return 0;
 }
 

@@ -49,6 +49,7 @@ def _load():
         lib.orc_mul_encoded.argtypes = [u32, u32, vp, u64, u64]
         lib.orc_mul_encoded.restype = ctypes.c_int64
         lib.orc_count_range.argtypes = [u32, u32, u32, vp, sz, u32, u32, u32, vp, vp, ctypes.c_int, vp]
+        lib.orc_roots_range.argtypes = [u32, u32, u32, vp, sz, u32, u32, u32, vp, ctypes.c_int]
         _lib = lib
     return _lib
 
@@ -125,6 +126,20 @@ def count(q: int, g: int, coeffs, k_lo: int = 1, k_hi: int | None = None, nthrea
         raise ValueError({-10: "bad field parameters", -11: "coefficient >= q",
                           -12: "degree < 2g+1", -13: "bad k range"}.get(rc, f"error {rc}"))
     return out, sf, used.value
+
+
+def roots(q: int, g: int, coeffs, k_hi: int | None = None, nthreads: int = 0):
+    """r0_k = #{x in F_{q^k}: f(x) = 0} (affine zeros) for k = 1..k_hi (default g): uint32 [n][k_hi]."""
+    p, r = _factor_prime_power(q)
+    c = np.ascontiguousarray(coeffs, dtype=np.uint16)
+    if c.ndim != 2 or c.shape[1] != 2 * g + 3:
+        raise ValueError("coeffs must be [n][2g+3]")
+    k_hi = g if k_hi is None else k_hi
+    out = np.zeros((c.shape[0], k_hi), dtype=np.uint32)
+    rc = _load().orc_roots_range(p, r, g, c.ctypes.data, c.shape[0], 1, k_hi, k_hi, out.ctypes.data, nthreads)
+    if rc:
+        raise ValueError(f"orc_roots_range: error {rc}")
+    return out
 
 
 def histogram(counts, mask=None):

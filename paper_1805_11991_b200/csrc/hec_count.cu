@@ -194,11 +194,11 @@ __global__ void __launch_bounds__(kThreads, 1) hec_count_kernel(const __grid_con
         const bool mine = lane + 1 >= P.k_lo && lane + 1 <= P.k_hi;
         if (bad_range || (nz >> (D - 1)) == 0) {
             if (lane == 0) atomicMin(&P.err[bad_range ? 0 : 1], curve);
-            if (mine) P.out[curve * G + lane] = 0;
+            if (mine) { P.out[curve * G + lane] = 0; if (P.out_r0) P.out_r0[curve * G + lane] = 0; }
             continue;
         }
 
-        uint32_t my_count = 0;   // lane k-1 keeps N_k
+        uint32_t my_count = 0, my_r0 = 0;   // lane k-1 keeps N_k and r0_k
 #pragma unroll
         for (uint32_t k = 1; k <= (uint32_t)G; k++) {
             if (k < P.k_lo || k > P.k_hi) continue;
@@ -258,9 +258,12 @@ __global__ void __launch_bounds__(kThreads, 1) hec_count_kernel(const __grid_con
             const uint32_t x0 = (nz & 1u) == 0 ? 1u : ((lc0 & 1u) ? 0u : 2u);
             const uint32_t inf = ((nz >> D) & 1u) == 0 ? 1u : ((lcD & 1u) ? 0u : 2u);
             const uint32_t Nk = r0 + 2u * rsq + x0 + inf;
-            if (lane + 1 == k) my_count = Nk;
+            if (lane + 1 == k) { my_count = Nk; my_r0 = r0 + ((nz & 1u) ? 0u : 1u); }
         }
-        if (mine) P.out[curve * G + lane] = my_count;
+        if (mine) {
+            P.out[curve * G + lane] = my_count;
+            if (P.out_r0) P.out_r0[curve * G + lane] = my_r0;
+        }
     }
 }
 
@@ -283,7 +286,9 @@ __device__ __forceinline__ void radix_dispatch(const uint32_t R, const Pol pol, 
     else radix_all_x<D, 2, false, Ar>(pol, M, rcpM, lane, nz, lcj, scratch, part, splits, n_sq, n_zero);
 }
 
-template <int G, int TOP>
+// SPLIT = false: one warp per curve (batches; P.splits == 1).  SPLIT = true: a separate instantiation for small batches,
+// so that the batch kernel carries none of the split bookkeeping (measured: 610 -> 685 ms on config 4 when it did).
+template <int G, int TOP, bool SPLIT>
 __global__ void __launch_bounds__(kThreads, 1) hec_count_radix_kernel(const __grid_constant__ HecCountParams P) {
     constexpr int D = 2 * G + 2;
     constexpr int NC = D + 1;
@@ -300,10 +305,11 @@ __global__ void __launch_bounds__(kThreads, 1) hec_count_radix_kernel(const __gr
                                  warp * hec_radix::kScratchWords;
 
     // one work item = (curve, part): part `part` of P.splits slices of the coset range of every field
-    const unsigned long long items = P.n * P.splits;
+    const uint32_t splits = SPLIT ? P.splits : 1u;
+    const unsigned long long items = P.n * splits;
     for (unsigned long long item = (unsigned long long)blockIdx.x * kWarps + warp; item < items; item += stride) {
-        const unsigned long long curve = P.splits == 1u ? item : item / P.splits;
-        const uint32_t part = P.splits == 1u ? 0u : (uint32_t)(item - curve * P.splits);
+        const unsigned long long curve = SPLIT ? item / splits : item;
+        const uint32_t part = SPLIT ? (uint32_t)(item - curve * splits) : 0u;
         // ---- a2: coefficient load (lane j holds c_j) and boundary checks (readings G13, hec.h)
         uint32_t cj = 0;
         if (lane < NC) cj = P.coeffs[curve * NC + lane];
@@ -312,10 +318,10 @@ __global__ void __launch_bounds__(kThreads, 1) hec_count_radix_kernel(const __gr
         const bool mine = lane + 1 >= P.k_lo && lane + 1 <= P.k_hi;
         if (bad_range || (nz >> (D - 1)) == 0) {
             if (lane == 0) atomicMin(&P.err[bad_range ? 0 : 1], curve);
-            if (mine && P.splits == 1u) P.out[curve * G + lane] = 0;
+            if (mine && !SPLIT) { P.out[curve * G + lane] = 0; if (P.out_r0) P.out_r0[curve * G + lane] = 0; }
             continue;
         }
-        uint32_t my_count = 0;   // lane k-1 keeps N_k
+        uint32_t my_count = 0, my_r0 = 0;   // lane k-1 keeps N_k and r0_k
 #pragma unroll 1
         for (uint32_t k = P.k_lo; k <= P.k_hi; k++) {
             const HecFieldDev &F = P.f[k - 1];
@@ -325,16 +331,16 @@ __global__ void __launch_bounds__(kThreads, 1) hec_count_radix_kernel(const __gr
             uint32_t n_zero, n_sq;
             if (TOP == HEC_TAB_PAIR16 || k < P.k_hi) {
                 const hec_radix::PairS16 pol{smem_base + F.smem_off};
-                radix_dispatch<D, hec_radix::ArPacked>(F.radix, pol, M, F.rcpM, lane, nz, lcj, scratch, part, P.splits, n_sq, n_zero);
+                radix_dispatch<D, hec_radix::ArPacked>(F.radix, pol, M, F.rcpM, lane, nz, lcj, scratch, part, splits, n_sq, n_zero);
             } else if constexpr (TOP == HEC_TAB_RHALF32) {
                 const hec_radix::HalfS32 pol{smem_base + F.smem_off, smem_base + F.smem_off + 4u * (M >> 1)};
-                radix_dispatch<D, hec_radix::ArScalar>(F.radix, pol, M, F.rcpM, lane, nz, lcj, scratch, part, P.splits, n_sq, n_zero);
+                radix_dispatch<D, hec_radix::ArScalar>(F.radix, pol, M, F.rcpM, lane, nz, lcj, scratch, part, splits, n_sq, n_zero);
             } else if constexpr (TOP == HEC_TAB_RHALF17) {
                 const hec_radix::HalfS17 pol{smem_base + F.smem_off, smem_base + F.smem_off + 2u * (M >> 1), smem_base + F.smem_off2};
-                radix_dispatch<D, hec_radix::ArScalar>(F.radix, pol, M, F.rcpM, lane, nz, lcj, scratch, part, P.splits, n_sq, n_zero);
+                radix_dispatch<D, hec_radix::ArScalar>(F.radix, pol, M, F.rcpM, lane, nz, lcj, scratch, part, splits, n_sq, n_zero);
             } else if constexpr (TOP == HEC_TAB_GPAIR64) {
                 const hec_radix::PairG64 pol{reinterpret_cast<const uint2 *>(F.gtab)};
-                radix_dispatch<D, hec_radix::ArScalar>(F.radix, pol, M, F.rcpM, lane, nz, lcj, scratch, part, P.splits, n_sq, n_zero);
+                radix_dispatch<D, hec_radix::ArScalar>(F.radix, pol, M, F.rcpM, lane, nz, lcj, scratch, part, splits, n_sq, n_zero);
             }
             const uint32_t r0 = __reduce_add_sync(0xffffffffu, n_zero);
             const uint32_t rsq = __reduce_add_sync(0xffffffffu, n_sq);
@@ -344,11 +350,16 @@ __global__ void __launch_bounds__(kThreads, 1) hec_count_radix_kernel(const __gr
             const uint32_t x0 = (nz & 1u) == 0 ? 1u : ((lc0 & 1u) ? 0u : 2u);
             const uint32_t inf = ((nz >> D) & 1u) == 0 ? 1u : ((lcD & 1u) ? 0u : 2u);
             const uint32_t Nk = r0 + 2u * rsq + (part == 0u ? x0 + inf : 0u);
-            if (lane + 1 == k) my_count = Nk;
+            if (lane + 1 == k) { my_count = Nk; my_r0 = r0 + ((part == 0u && !(nz & 1u)) ? 1u : 0u); }
         }
         if (mine) {
-            if (P.splits == 1u) P.out[curve * G + lane] = my_count;
-            else if (my_count) atomicAdd(&P.out[curve * G + lane], my_count);
+            if (!SPLIT) {
+                P.out[curve * G + lane] = my_count;
+                if (P.out_r0) P.out_r0[curve * G + lane] = my_r0;
+            } else {
+                if (my_count) atomicAdd(&P.out[curve * G + lane], my_count);
+                if (P.out_r0 && my_r0) atomicAdd(&P.out_r0[curve * G + lane], my_r0);
+            }
         }
     }
 }
@@ -408,9 +419,21 @@ __global__ void __launch_bounds__(256) hec_squarefree_kernel(const HecSquarefree
             if (t != ZERO) db = (int)j - 1;
         }
     }
-    if (!ok || da < (int)P.ncoef - 2) { P.out[i] = 0; return; }     // reported by the count kernel
-    // Euclid: gcd(f, 0) = f (reading G14)
+    if (!ok || da < (int)P.ncoef - 2) {                              // reported by the count kernel
+        if (P.out) P.out[i] = 0;
+        if (P.out_lambda) P.out_lambda[i] = 0xFF;
+        return;
+    }
+    // Euclid: gcd(f, 0) = f (reading G14).  Alongside, the parity of log Res(f, f') (the quadratic character of the
+    // resultant: Res(A, B) = (-1)^{deg A deg B} lc(B)^{deg A - deg R} Res(B, R) for R = A mod B, Res(A, b) = b^{deg A}),
+    // needed by lambda below.
+    const int d = da, d1 = db;
+    const uint32_t lcf = a[da];
+    const uint32_t par_m1 = (P.M >> 1) & 1u;                         // -1 = alpha^{M/2}
+    uint32_t par = 0;
     while (db >= 0) {
+        const int m = da, nn = db;
+        const uint32_t lb = b[db];
         // a <- a mod b
         const uint32_t binv = K.inv(b[db]);
         while (da >= db) {
@@ -420,11 +443,44 @@ __global__ void __launch_bounds__(256) hec_squarefree_kernel(const HecSquarefree
             a[da] = ZERO;
             while (da >= 0 && a[da] == ZERO) da--;
         }
+        if (nn == 0) par ^= (uint32_t)m & lb & 1u;
+        else if (da >= 0) par ^= (((uint32_t)(m * nn) & 1u) & par_m1) ^ ((uint32_t)(m - da) & lb & 1u);
         // swap (a, b)
         for (int t = 0; t < (int)kSqMaxCoef; t++) { const uint32_t x = a[t]; a[t] = b[t]; b[t] = x; }
         const int td = da; da = db; db = td;
     }
-    P.out[i] = da == 0 ? 1 : 0;
+    const bool squarefree = da == 0;
+    if (P.out) P.out[i] = squarefree ? 1 : 0;
+    if (!P.out_lambda) return;
+    if (!squarefree) { P.out_lambda[i] = 0xFF; return; }
+    // lambda(f) (Algorithm 1 line 18: "from r0 if possible; otherwise by factoring").  An irreducible factor
+    // of degree e has its e roots in F_{q^k} iff e | k, so r0_k = sum_{e | k} e n_e and Moebius inversion gives n_e for
+    // e <= g.  The rest of the degree is ONE irreducible factor unless it is 2g+2 (no factor of degree <= g at all): then
+    // f is irreducible or a product of two irreducibles of degree g+1, and Stickelberger's theorem decides without
+    // factoring: the number of irreducible factors is congruent to deg f mod 2 iff disc(f) is a square, where
+    // disc(f) = (-1)^{d(d-1)/2} lc(f)^{-(d + deg f')} Res(f, f') up to squares.
+    const uint32_t *r0 = P.roots + i * P.g;
+    int ne[kSqMaxCoef];
+    for (int e = 0; e < (int)kSqMaxCoef; e++) ne[e] = 0;
+    int rest = d;
+    for (int e = 1; e <= (int)P.g; e++) {
+        const int sub = e == 1 ? 0 : (e == 4 ? (int)r0[1] : (int)r0[0]);     // e = 2, 3, 5: r0_e - r0_1; e = 4: r0_4 - r0_2
+        ne[e] = ((int)r0[e - 1] - sub) / e;
+        rest -= e * ne[e];
+    }
+    if (rest == 2 * (int)P.g + 2) {
+        const uint32_t par_disc = par ^ (((uint32_t)(d * (d - 1) / 2) & 1u) & par_m1) ^ ((uint32_t)(d + d1) & lcf & 1u);
+        if (par_disc == 0) ne[P.g + 1] = 2; else ne[rest] = 1;
+    } else if (rest > 0) {
+        ne[rest] = 1;
+    }
+    if (d == 2 * (int)P.g + 1) ne[1]++;                              // an additional summand 1
+    unsigned long long code = 0;
+    for (int e = 1; e <= 2 * (int)P.g + 2; e++) code |= (unsigned long long)ne[e] << (4 * (e - 1));
+    uint32_t idx = 0xFE;                                             // never left: every type is in the table
+    for (uint32_t t = 0; t < P.n_parts; t++)
+        if (P.part_codes[t] == code) { idx = t; break; }
+    P.out_lambda[i] = (uint8_t)idx;
 }
 
 // --------------------------------------------------------------------------------------------
@@ -448,6 +504,8 @@ struct DevicePlan {
     std::vector<LaunchPlan> launches;
     // squarefree
     const uint32_t *sq_zech = nullptr, *sq_emb = nullptr;
+    const unsigned long long *d_part_codes = nullptr;   // lambda: packed partitions of 2g+2 in index order
+    uint32_t n_parts = 0;
     unsigned long long *d_err = nullptr;
     ~DevicePlan() {
         if (d_blob) cudaFree(d_blob);
@@ -732,6 +790,13 @@ int build_plan(LibState &S, uint32_t q, uint32_t g, int regime, int eval, Device
         uint32_t *e = reinterpret_cast<uint32_t *>(host.data() + emb_off[k - 1]);
         for (uint32_t c = 0; c < q; c++) e[c] = fields[k - 1]->embed[c] == t.M ? HEC_LOG_ZERO : fields[k - 1]->embed[c];
     }
+    const std::vector<std::vector<uint8_t>> parts = hec_partitions_of(2 * g + 2);
+    const size_t part_off = reserve(parts.size() * 8u);
+    for (size_t t = 0; t < parts.size(); t++) {
+        unsigned long long code = 0;
+        for (size_t e = 0; e < parts[t].size(); e++) code |= (unsigned long long)parts[t][e] << (4 * e);
+        reinterpret_cast<unsigned long long *>(host.data() + part_off)[t] = code;
+    }
     const size_t sqz_off = reserve((size_t)(q - 1) * 4u);
     std::copy(fields[0]->zech.begin(), fields[0]->zech.end(), reinterpret_cast<uint32_t *>(host.data() + sqz_off));
 
@@ -755,6 +820,8 @@ int build_plan(LibState &S, uint32_t q, uint32_t g, int regime, int eval, Device
     }
     plan->sq_zech = reinterpret_cast<const uint32_t *>(base + sqz_off);
     plan->sq_emb = plan->f[0].emb;
+    plan->d_part_codes = reinterpret_cast<const unsigned long long *>(base + part_off);
+    plan->n_parts = (uint32_t)parts.size();
 
     *out = plan.get();
     S.plans[key] = std::move(plan);
@@ -777,6 +844,12 @@ int launch_kernel(LibState &S, Kern kern, const LaunchPlan &L, const HecCountPar
     return HEC_OK;
 }
 
+template <int G, int TOP>
+int launch_radix(LibState &S, const LaunchPlan &L, const HecCountParams &P, uint32_t chains) {
+    return P.splits > 1u ? launch_kernel(S, hec_count_radix_kernel<G, TOP, true>, L, P, chains)
+                         : launch_kernel(S, hec_count_radix_kernel<G, TOP, false>, L, P, chains);
+}
+
 template <int G, int U>
 int launch_count(LibState &S, const DevicePlan &plan, HecCountParams P) {
     for (const LaunchPlan &L : plan.launches) {
@@ -788,10 +861,10 @@ int launch_count(LibState &S, const DevicePlan &plan, HecCountParams P) {
             case HEC_TAB_HALF32: rc = launch_kernel(S, hec_count_kernel<G, U, HEC_TAB_HALF32>, L, P, U); break;
             case HEC_TAB_HALF24: rc = launch_kernel(S, hec_count_kernel<G, U, HEC_TAB_HALF24>, L, P, U); break;
             case HEC_TAB_EXT16: rc = launch_kernel(S, hec_count_kernel<G, U, HEC_TAB_EXT16>, L, P, U); break;
-            case HEC_TAB_PAIR16: rc = launch_kernel(S, hec_count_radix_kernel<G, HEC_TAB_PAIR16>, L, P, 2); break;
-            case HEC_TAB_RHALF32: rc = launch_kernel(S, hec_count_radix_kernel<G, HEC_TAB_RHALF32>, L, P, 1); break;
-            case HEC_TAB_RHALF17: rc = launch_kernel(S, hec_count_radix_kernel<G, HEC_TAB_RHALF17>, L, P, 1); break;
-            default: rc = launch_kernel(S, hec_count_radix_kernel<G, HEC_TAB_GPAIR64>, L, P, 1); break;
+            case HEC_TAB_PAIR16: rc = launch_radix<G, HEC_TAB_PAIR16>(S, L, P, 2); break;
+            case HEC_TAB_RHALF32: rc = launch_radix<G, HEC_TAB_RHALF32>(S, L, P, 1); break;
+            case HEC_TAB_RHALF17: rc = launch_radix<G, HEC_TAB_RHALF17>(S, L, P, 1); break;
+            default: rc = launch_radix<G, HEC_TAB_GPAIR64>(S, L, P, 1); break;
         }
         if (rc) return rc;
         if (plan.radix)
@@ -809,6 +882,22 @@ bool is_device_pointer(const void *p) {
 }  // namespace
 
 // Shared with the other translation units.
+// Partitions of `total` as multiplicity vectors (n_1 .. n_total) in ascending lexicographic order of that vector: the
+// index order of the lambda codes (hec.h).
+std::vector<std::vector<uint8_t>> hec_partitions_of(uint32_t total) {
+    std::vector<std::vector<uint8_t>> res;
+    std::vector<uint8_t> acc(total, 0);
+    struct Rec {
+        static void go(uint32_t e, uint32_t left, uint32_t total, std::vector<uint8_t> &acc, std::vector<std::vector<uint8_t>> &res) {
+            if (e > total) { if (left == 0) res.push_back(acc); return; }
+            for (uint32_t m = 0; m * e <= left; m++) { acc[e - 1] = (uint8_t)m; go(e + 1, left - m * e, total, acc, res); }
+            acc[e - 1] = 0;
+        }
+    };
+    Rec::go(1, total, total, acc, res);
+    std::sort(res.begin(), res.end());
+    return res;
+}
 cudaStream_t hec_current_stream() { return g_state.stream; }
 int hec_ensure_device(int *sm_count, int *smem_optin) {
     std::lock_guard<std::recursive_mutex> lock(g_state.mu);
@@ -852,6 +941,11 @@ int hec_last_count_stats(hec_count_stats *out) {
 uint64_t hec_launch_count(void) { return hec_launch_counter::value; }
 
 int hec_count(uint32_t q, uint32_t g, const uint16_t *coeffs, size_t n, uint32_t *out_counts, uint8_t *out_squarefree) {
+    return hec_count_ex(q, g, coeffs, n, out_counts, out_squarefree, nullptr, nullptr);
+}
+
+int hec_count_ex(uint32_t q, uint32_t g, const uint16_t *coeffs, size_t n, uint32_t *out_counts, uint8_t *out_squarefree,
+                 uint32_t *out_roots, uint8_t *out_lambda) {
     if (g < 1 || g > HEC_MAX_GENUS) HEC_FAIL(HEC_ERR_INVALID_ARG, "g must be in [1, HEC_MAX_GENUS]");
     uint32_t p, r;
     if (!hec_factor_q(q, &p, &r)) HEC_FAIL(HEC_ERR_INVALID_FIELD, "q must be an odd prime power below 65536");
@@ -868,7 +962,10 @@ int hec_count(uint32_t q, uint32_t g, const uint16_t *coeffs, size_t n, uint32_t
     if (rc) return rc;
     const bool dev_in = is_device_pointer(coeffs), dev_out = is_device_pointer(out_counts);
     const bool dev_sf = out_squarefree ? is_device_pointer(out_squarefree) : dev_out;
-    if (dev_in != dev_out || dev_sf != dev_out) HEC_FAIL(HEC_ERR_INVALID_ARG, "coeffs/out_counts/out_squarefree must all be host or all device pointers");
+    const bool dev_r0 = out_roots ? is_device_pointer(out_roots) : dev_out;
+    const bool dev_lam = out_lambda ? is_device_pointer(out_lambda) : dev_out;
+    if (dev_in != dev_out || dev_sf != dev_out || dev_r0 != dev_out || dev_lam != dev_out)
+        HEC_FAIL(HEC_ERR_INVALID_ARG, "coeffs/out_counts/out_squarefree/out_roots/out_lambda must all be host or all device pointers");
 
     DevicePlan *plan = nullptr;
     rc = build_plan(S, q, g, S.regime, S.eval, &plan);
@@ -879,9 +976,15 @@ int hec_count(uint32_t q, uint32_t g, const uint16_t *coeffs, size_t n, uint32_t
     const uint16_t *d_coeffs = coeffs;
     uint32_t *d_counts = out_counts;
     uint8_t *d_sf = out_squarefree;
-    if (!dev_in) {
-        const size_t a = (in_bytes + 255) & ~(size_t)255, b = (cnt_bytes + 255) & ~(size_t)255;
-        const size_t need = a + b + sf_bytes;
+    uint32_t *d_r0 = out_roots;
+    uint8_t *d_lam = out_lambda;
+    const bool need_r0 = out_roots || out_lambda;              // lambda is computed from r0 (Algorithm 1 line 18)
+    const size_t lam_bytes = out_lambda ? n : 0;
+    if (!dev_in || (need_r0 && !out_roots)) {
+        const size_t a = dev_in ? 0 : (in_bytes + 255) & ~(size_t)255, b = dev_in ? 0 : (cnt_bytes + 255) & ~(size_t)255;
+        const size_t c = dev_in ? 0 : (sf_bytes + 255) & ~(size_t)255;
+        const size_t r0b = (!need_r0 || (dev_in && out_roots)) ? 0 : (cnt_bytes + 255) & ~(size_t)255;
+        const size_t need = a + b + c + r0b + (dev_in ? 0 : lam_bytes);
         if (need > S.stage_bytes) {
             if (S.d_stage) cudaFree(S.d_stage);
             S.d_stage = nullptr; S.stage_bytes = 0;
@@ -889,17 +992,21 @@ int hec_count(uint32_t q, uint32_t g, const uint16_t *coeffs, size_t n, uint32_t
             S.stage_bytes = need;
         }
         uint8_t *base = static_cast<uint8_t *>(S.d_stage);
-        d_coeffs = reinterpret_cast<const uint16_t *>(base);
-        d_counts = reinterpret_cast<uint32_t *>(base + a);
-        d_sf = out_squarefree ? base + a + b : nullptr;
-        HEC_CUDA_OK(cudaMemcpyAsync(base, coeffs, in_bytes, cudaMemcpyHostToDevice, S.stream));
+        if (!dev_in) {
+            d_coeffs = reinterpret_cast<const uint16_t *>(base);
+            d_counts = reinterpret_cast<uint32_t *>(base + a);
+            d_sf = out_squarefree ? base + a + b : nullptr;
+            d_lam = out_lambda ? base + a + b + c + r0b : nullptr;
+            HEC_CUDA_OK(cudaMemcpyAsync(base, coeffs, in_bytes, cudaMemcpyHostToDevice, S.stream));
+        }
+        if (r0b) d_r0 = reinterpret_cast<uint32_t *>(base + a + b + c);
     }
 
     static const unsigned long long kNoErr[2] = {~0ull, ~0ull};
     HEC_CUDA_OK(cudaMemcpyAsync(plan->d_err, kNoErr, sizeof kNoErr, cudaMemcpyHostToDevice, S.stream));
 
     HecCountParams P;
-    P.coeffs = d_coeffs; P.out = d_counts; P.n = n; P.q = q;
+    P.coeffs = d_coeffs; P.out = d_counts; P.out_r0 = need_r0 ? d_r0 : nullptr; P.n = n; P.q = q;
     P.blob = nullptr; P.blob_bytes = 0; P.err = plan->d_err; P.k_lo = 1; P.k_hi = g; P.scratch_off = 0;
     // Small batches (down to the single curve of the paper's Table 1): spread every curve over
     // `splits` warps so that the whole GPU works on it; each warp takes a slice of the cosets of every field.
@@ -912,7 +1019,10 @@ int hec_count(uint32_t q, uint32_t g, const uint16_t *coeffs, size_t n, uint32_t
             P.splits = (uint32_t)std::max<unsigned long long>(1, std::min<unsigned long long>(want, Mtop / 2048u));
         }
     }
-    if (P.splits > 1) HEC_CUDA_OK(cudaMemsetAsync(d_counts, 0, cnt_bytes, S.stream));
+    if (P.splits > 1) {
+        HEC_CUDA_OK(cudaMemsetAsync(d_counts, 0, cnt_bytes, S.stream));
+        if (P.out_r0) HEC_CUDA_OK(cudaMemsetAsync(P.out_r0, 0, cnt_bytes, S.stream));
+    }
     const uint32_t splits_used = P.splits;
     for (uint32_t k = 0; k < HEC_MAX_GENUS; k++) P.f[k] = plan->f[k < g ? k : 0];
 
@@ -931,10 +1041,11 @@ int hec_count(uint32_t q, uint32_t g, const uint16_t *coeffs, size_t n, uint32_t
     }
     if (rc) return rc;
     HEC_CUDA_OK(cudaEventRecord(S.ev[1], S.stream));
-    if (d_sf) {
+    if (d_sf || d_lam) {
         HecSquarefreeParams Q;
         Q.coeffs = d_coeffs; Q.out = d_sf; Q.n = n; Q.p = p; Q.q = q; Q.M = q - 1; Q.ncoef = (uint32_t)ncoef;
         Q.zech = plan->sq_zech; Q.emb = plan->sq_emb;
+        Q.roots = d_lam ? d_r0 : nullptr; Q.out_lambda = d_lam; Q.part_codes = plan->d_part_codes; Q.n_parts = plan->n_parts; Q.g = g;
         const unsigned long long blocks = (n + 255) / 256;
         hec_squarefree_kernel<<<(unsigned)blocks, 256, 0, S.stream>>>(Q);
         hec_launch_counter::value++;
@@ -947,6 +1058,8 @@ int hec_count(uint32_t q, uint32_t g, const uint16_t *coeffs, size_t n, uint32_t
     if (!dev_in) {
         HEC_CUDA_OK(cudaMemcpyAsync(out_counts, d_counts, cnt_bytes, cudaMemcpyDeviceToHost, S.stream));
         if (out_squarefree) HEC_CUDA_OK(cudaMemcpyAsync(out_squarefree, d_sf, sf_bytes, cudaMemcpyDeviceToHost, S.stream));
+        if (out_roots) HEC_CUDA_OK(cudaMemcpyAsync(out_roots, d_r0, cnt_bytes, cudaMemcpyDeviceToHost, S.stream));
+        if (out_lambda) HEC_CUDA_OK(cudaMemcpyAsync(out_lambda, d_lam, lam_bytes, cudaMemcpyDeviceToHost, S.stream));
     }
     HEC_CUDA_OK(cudaStreamSynchronize(S.stream));
     cudaEventElapsedTime(&S.stats.count_kernel_ms, S.ev[0], S.ev[1]);
@@ -959,6 +1072,17 @@ int hec_count(uint32_t q, uint32_t g, const uint16_t *coeffs, size_t n, uint32_t
         hec_set_error(HEC_ERR_DEGREE, "a row has c[2g+2] = c[2g+1] = 0 (degree < 2g+1)", (size_t)err[1]);
         return HEC_ERR_DEGREE;
     }
+    return HEC_OK;
+}
+
+int hec_lambda_partitions(uint32_t g, uint8_t *out_parts, size_t cap, size_t *out_count) {
+    if (g < 1 || g > HEC_MAX_GENUS) HEC_FAIL(HEC_ERR_INVALID_ARG, "g must be in [1, HEC_MAX_GENUS]");
+    if (!out_count) HEC_FAIL(HEC_ERR_INVALID_ARG, "out_count must not be NULL");
+    const std::vector<std::vector<uint8_t>> parts = hec_partitions_of(2 * g + 2);
+    *out_count = parts.size();
+    if (cap < parts.size()) HEC_FAIL(HEC_ERR_CAPACITY, "hec_lambda_partitions: cap is smaller than the number of partitions");
+    if (!out_parts) HEC_FAIL(HEC_ERR_INVALID_ARG, "out_parts must not be NULL");
+    for (size_t t = 0; t < parts.size(); t++) std::copy(parts[t].begin(), parts[t].end(), out_parts + t * (2 * g + 2));
     return HEC_OK;
 }
 

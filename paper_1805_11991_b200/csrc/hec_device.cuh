@@ -55,6 +55,7 @@ struct HecCountParams {
     uint32_t k_lo, k_hi;           // this launch computes N_k for k_lo <= k <= k_hi; only field k_hi may differ from the
                                    // launch's base layout (EXT16 for the Horner kernel, PAIR16 for the radix kernel)
     uint32_t scratch_off;          // radix kernel: byte offset (after the blob) of the per-warp scratch words
+    uint32_t *out_r0;              // [n][g] or NULL: r0_k = #{x in F_{q^k}: f(x) = 0}, the input of lambda
     uint32_t splits;               // radix kernel: warps per curve (>= 1); > 1: out is pre-zeroed and accumulated with atomics
     HecFieldDev f[HEC_MAX_GENUS];
 };
@@ -67,4 +68,9 @@ struct HecSquarefreeParams {
     uint32_t ncoef;                // 2g+3
     const uint32_t *zech;          // M entries, paper's convention (sentinel M)
     const uint32_t *emb;           // q entries: log in F_q or HEC_LOG_ZERO
+    // lambda(f) (Algorithm 1 line 18), all NULL / 0 when not requested
+    const uint32_t *roots;         // [n][g] r0_k from the count kernel
+    uint8_t *out_lambda;           // [n] index of the partition, 0xFF when f is not squarefree
+    const unsigned long long *part_codes;   // n_parts packed multiplicity vectors (4 bits per part size), index order
+    uint32_t n_parts, g;
 };

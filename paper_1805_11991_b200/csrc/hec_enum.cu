@@ -79,16 +79,27 @@ __global__ void __launch_bounds__(256) reduced_rows_kernel(const __grid_constant
     }
 }
 
-// tuples[m + r] = twist of tuples[r] (reading G8), weights copied.
-__global__ void __launch_bounds__(256) twist_kernel(uint32_t *tuples, unsigned long long *w, unsigned long long m, uint32_t g, uint32_t q) {
+// tuples[m + r] = twist of tuples[r] (reading G8), weights copied.  Rows have `cols` >= g columns; columns beyond g
+// (the lambda index: n f factors like f) are copied.
+__global__ void __launch_bounds__(256) twist_kernel(uint32_t *tuples, unsigned long long *w, unsigned long long m, uint32_t g,
+                                                    uint32_t cols, uint32_t q) {
     for (unsigned long long r = blockIdx.x * 256ull + threadIdx.x; r < m; r += gridDim.x * 256ull) {
         unsigned long long qk = 1;
-        for (uint32_t k = 1; k <= g; k++) {
+        for (uint32_t k = 1; k <= cols; k++) {
             qk *= q;
-            const uint32_t v = tuples[r * g + k - 1];
-            tuples[(m + r) * g + k - 1] = (k & 1u) ? (uint32_t)(2 * qk + 2 - v) : v;
+            const uint32_t v = tuples[r * cols + k - 1];
+            tuples[(m + r) * cols + k - 1] = (k <= g && (k & 1u)) ? (uint32_t)(2 * qk + 2 - v) : v;
         }
         w[m + r] = w[r];
+    }
+}
+
+// keys[r] = (N_1 .. N_g, lambda index): the key of the paper's map (1.2).
+__global__ void __launch_bounds__(256) append_lambda_kernel(const uint32_t *counts, const uint8_t *lam, unsigned long long n,
+                                                            uint32_t g, uint32_t *keys) {
+    for (unsigned long long r = blockIdx.x * 256ull + threadIdx.x; r < n; r += gridDim.x * 256ull) {
+        for (uint32_t k = 0; k < g; k++) keys[r * (g + 1) + k] = counts[r * g + k];
+        keys[r * (g + 1) + g] = lam[r];
     }
 }
 
@@ -202,30 +213,34 @@ int hec_reduced_rows(uint32_t q, uint32_t g, uint32_t d, uint64_t first, size_t 
     return HEC_OK;
 }
 
-int hec_curve_map(uint32_t q, uint32_t g, uint32_t d, uint32_t *out_tuples, uint64_t *out_weights, size_t cap, size_t *out_m) {
+static int curve_map_impl(uint32_t q, uint32_t g, uint32_t d, bool with_lambda, uint32_t *out_tuples, uint64_t *out_weights,
+                          size_t cap, size_t *out_m) {
     if (!out_m) HEC_FAIL(HEC_ERR_INVALID_ARG, "out_m must not be NULL");
     *out_m = 0;
     if (cap > 0 && (!out_tuples || !out_weights)) HEC_FAIL(HEC_ERR_INVALID_ARG, "out_tuples/out_weights must not be NULL when cap > 0");
     EnumParams E;
     int rc = build_families(q, g, d, E);
     if (rc) return rc;
+    if (with_lambda && g + 1 > HEC_MAX_GENUS) HEC_FAIL(HEC_ERR_UNSUPPORTED, "hec_curve_map_lambda: g + 1 key columns exceed the histogram's limit");
     int sms = 0;
     if ((rc = hec_ensure_device(&sms, nullptr))) return rc;
     cudaStream_t st = hec_current_stream();
     Scratch gen;
     if ((rc = upload_generator_powers(q, gen, E))) return rc;
+    const uint32_t cols = with_lambda ? g + 1 : g;             // key columns
 
     const size_t chunk = (size_t)std::min<unsigned long long>(E.total, 1ull << 22);
-    Scratch rows, mult, counts, flags, part_t, part_w, acc_t, acc_w, cat_t, cat_w;
+    Scratch rows, mult, counts, flags, lam, keys, part_t, part_w, acc_t, acc_w, cat_t, cat_w;
     if ((rc = rows.alloc(chunk * E.ncoef * 2)) || (rc = mult.alloc(chunk * 8)) || (rc = counts.alloc(chunk * g * 4)) ||
-        (rc = flags.alloc(chunk)) || (rc = part_t.alloc(chunk * g * 4)) || (rc = part_w.alloc(chunk * 8))) return rc;
+        (rc = flags.alloc(chunk)) || (rc = part_t.alloc(chunk * cols * 4)) || (rc = part_w.alloc(chunk * 8))) return rc;
+    if (with_lambda && ((rc = lam.alloc(chunk)) || (rc = keys.alloc(chunk * cols * 4)))) return rc;
     size_t acc_m = 0, acc_cap = 0;
     auto grow = [&](Scratch &t, Scratch &w, size_t &have, size_t need) -> int {
         if (need <= have) return HEC_OK;
         Scratch nt, nw;
         int e;
         const size_t want = std::max(need, 2 * have);
-        if ((e = nt.alloc(want * g * 4)) || (e = nw.alloc(want * 8))) return e;
+        if ((e = nt.alloc(want * cols * 4)) || (e = nw.alloc(want * 8))) return e;
         std::swap(t.p, nt.p); std::swap(w.p, nw.p);      // callers never need the old contents
         have = want;
         return HEC_OK;
@@ -235,49 +250,66 @@ int hec_curve_map(uint32_t q, uint32_t g, uint32_t d, uint32_t *out_tuples, uint
         const size_t n = (size_t)std::min<unsigned long long>(chunk, E.total - first);
         if ((rc = launch_rows(E, first, n, static_cast<uint16_t *>(rows.p), static_cast<unsigned long long *>(mult.p), sms))) return rc;
         // Algorithm 1 lines 6-18 for the chunk, then the weighted histogram of its squarefree rows (line 20)
-        if ((rc = hec_count(q, g, static_cast<const uint16_t *>(rows.p), n, static_cast<uint32_t *>(counts.p), static_cast<uint8_t *>(flags.p)))) return rc;
+        if ((rc = hec_count_ex(q, g, static_cast<const uint16_t *>(rows.p), n, static_cast<uint32_t *>(counts.p),
+                               static_cast<uint8_t *>(flags.p), nullptr, with_lambda ? static_cast<uint8_t *>(lam.p) : nullptr))) return rc;
+        const uint32_t *key_rows = static_cast<const uint32_t *>(counts.p);
+        if (with_lambda) {
+            append_lambda_kernel<<<(unsigned)std::min<size_t>((n + 255) / 256, (size_t)sms * 8), 256, 0, st>>>(
+                static_cast<const uint32_t *>(counts.p), static_cast<const uint8_t *>(lam.p), n, g, static_cast<uint32_t *>(keys.p));
+            hec_launch_counter::value++;
+            HEC_CUDA_OK(cudaGetLastError());
+            key_rows = static_cast<const uint32_t *>(keys.p);
+        }
         size_t m = 0;
-        if ((rc = hec_histogram_weighted(static_cast<const uint32_t *>(counts.p), static_cast<const uint8_t *>(flags.p),
-                                         static_cast<const uint64_t *>(mult.p), n, g, static_cast<uint32_t *>(part_t.p),
+        if ((rc = hec_histogram_weighted(key_rows, static_cast<const uint8_t *>(flags.p),
+                                         static_cast<const uint64_t *>(mult.p), n, cols, static_cast<uint32_t *>(part_t.p),
                                          static_cast<uint64_t *>(part_w.p), chunk, &m))) return rc;
         if (m == 0) continue;
         // running map <- merge(running map, chunk's map)
         if ((rc = grow(cat_t, cat_w, cat_cap, acc_m + m))) return rc;
         if (acc_m) {
-            HEC_CUDA_OK(cudaMemcpyAsync(cat_t.p, acc_t.p, acc_m * g * 4, cudaMemcpyDeviceToDevice, st));
+            HEC_CUDA_OK(cudaMemcpyAsync(cat_t.p, acc_t.p, acc_m * cols * 4, cudaMemcpyDeviceToDevice, st));
             HEC_CUDA_OK(cudaMemcpyAsync(cat_w.p, acc_w.p, acc_m * 8, cudaMemcpyDeviceToDevice, st));
         }
-        HEC_CUDA_OK(cudaMemcpyAsync(static_cast<uint32_t *>(cat_t.p) + acc_m * g, part_t.p, m * g * 4, cudaMemcpyDeviceToDevice, st));
+        HEC_CUDA_OK(cudaMemcpyAsync(static_cast<uint32_t *>(cat_t.p) + acc_m * cols, part_t.p, m * cols * 4, cudaMemcpyDeviceToDevice, st));
         HEC_CUDA_OK(cudaMemcpyAsync(static_cast<uint64_t *>(cat_w.p) + acc_m, part_w.p, m * 8, cudaMemcpyDeviceToDevice, st));
         if ((rc = grow(acc_t, acc_w, acc_cap, acc_m + m))) return rc;
         size_t merged = 0;
-        if ((rc = hec_histogram_weighted(static_cast<const uint32_t *>(cat_t.p), nullptr, static_cast<const uint64_t *>(cat_w.p), acc_m + m, g,
+        if ((rc = hec_histogram_weighted(static_cast<const uint32_t *>(cat_t.p), nullptr, static_cast<const uint64_t *>(cat_w.p), acc_m + m, cols,
                                          static_cast<uint32_t *>(acc_t.p), static_cast<uint64_t *>(acc_w.p), acc_cap, &merged))) return rc;
         acc_m = merged;
     }
     if (acc_m == 0) return HEC_OK;
     // line 21: the same weight at the tuple of the quadratic twist (reading G8)
     if ((rc = grow(cat_t, cat_w, cat_cap, 2 * acc_m))) return rc;
-    HEC_CUDA_OK(cudaMemcpyAsync(cat_t.p, acc_t.p, acc_m * g * 4, cudaMemcpyDeviceToDevice, st));
+    HEC_CUDA_OK(cudaMemcpyAsync(cat_t.p, acc_t.p, acc_m * cols * 4, cudaMemcpyDeviceToDevice, st));
     HEC_CUDA_OK(cudaMemcpyAsync(cat_w.p, acc_w.p, acc_m * 8, cudaMemcpyDeviceToDevice, st));
     twist_kernel<<<(unsigned)std::min<size_t>((acc_m + 255) / 256, (size_t)sms * 8), 256, 0, st>>>(
-        static_cast<uint32_t *>(cat_t.p), static_cast<unsigned long long *>(cat_w.p), acc_m, g, q);
+        static_cast<uint32_t *>(cat_t.p), static_cast<unsigned long long *>(cat_w.p), acc_m, g, cols, q);
     hec_launch_counter::value++;
     HEC_CUDA_OK(cudaGetLastError());
     Scratch fin_t, fin_w;
-    if ((rc = fin_t.alloc(2 * acc_m * g * 4)) || (rc = fin_w.alloc(2 * acc_m * 8))) return rc;
+    if ((rc = fin_t.alloc(2 * acc_m * cols * 4)) || (rc = fin_w.alloc(2 * acc_m * 8))) return rc;
     size_t fin_m = 0;
-    if ((rc = hec_histogram_weighted(static_cast<const uint32_t *>(cat_t.p), nullptr, static_cast<const uint64_t *>(cat_w.p), 2 * acc_m, g,
+    if ((rc = hec_histogram_weighted(static_cast<const uint32_t *>(cat_t.p), nullptr, static_cast<const uint64_t *>(cat_w.p), 2 * acc_m, cols,
                                      static_cast<uint32_t *>(fin_t.p), static_cast<uint64_t *>(fin_w.p), 2 * acc_m, &fin_m))) return rc;
     *out_m = fin_m;
     if (cap < fin_m) HEC_FAIL(HEC_ERR_CAPACITY, "hec_curve_map: cap is smaller than the number of distinct tuples");
     const bool dev = hec_is_device_pointer(out_tuples);
     if (hec_is_device_pointer(out_weights) != dev) HEC_FAIL(HEC_ERR_INVALID_ARG, "out_tuples/out_weights must both be host or both device pointers");
     const cudaMemcpyKind kind = dev ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost;
-    HEC_CUDA_OK(cudaMemcpyAsync(out_tuples, fin_t.p, fin_m * g * 4, kind, st));
+    HEC_CUDA_OK(cudaMemcpyAsync(out_tuples, fin_t.p, fin_m * cols * 4, kind, st));
     HEC_CUDA_OK(cudaMemcpyAsync(out_weights, fin_w.p, fin_m * 8, kind, st));
     HEC_CUDA_OK(cudaStreamSynchronize(st));
     return HEC_OK;
+}
+
+int hec_curve_map(uint32_t q, uint32_t g, uint32_t d, uint32_t *out_tuples, uint64_t *out_weights, size_t cap, size_t *out_m) {
+    return curve_map_impl(q, g, d, false, out_tuples, out_weights, cap, out_m);
+}
+
+int hec_curve_map_lambda(uint32_t q, uint32_t g, uint32_t d, uint32_t *out_keys, uint64_t *out_weights, size_t cap, size_t *out_m) {
+    return curve_map_impl(q, g, d, true, out_keys, out_weights, cap, out_m);
 }
 
 }  // extern "C"

@@ -50,4 +50,6 @@ struct hec_table_geom {
     uint32_t entries;  // 2 * lmax + M
 };
 
+std::vector<std::vector<uint8_t>> hec_partitions_of(uint32_t total);
+
 struct hec_launch_counter { static uint64_t value; };

@@ -34,6 +34,7 @@ SYMBOLS = [
     "hec_field_degree", "hec_field_q", "hec_field_Q", "hec_field_embed_unit", "hec_field_modulus",
     "hec_field_antilog", "hec_field_log", "hec_field_zech", "hec_field_embed", "hec_count", "hec_histogram",
     "hec_histogram_merge", "hec_reduced_total", "hec_reduced_rows", "hec_curve_map",
+    "hec_count_ex", "hec_lambda_partitions", "hec_curve_map_lambda",
     "hec_set_stream", "hec_set_regime", "hec_set_eval", "hec_last_count_stats", "hec_launch_count", "hec_gather_bench",
     "hec_shutdown",
 ]
@@ -80,6 +81,9 @@ def lib():
         L.hec_reduced_total.argtypes = [u32, u32, u32, ctypes.POINTER(ctypes.c_uint64)]
         L.hec_reduced_rows.argtypes = [u32, u32, u32, ctypes.c_uint64, sz, vp, vp]
         L.hec_curve_map.argtypes = [u32, u32, u32, vp, vp, sz, ctypes.POINTER(sz)]
+        L.hec_curve_map_lambda.argtypes = [u32, u32, u32, vp, vp, sz, ctypes.POINTER(sz)]
+        L.hec_count_ex.argtypes = [u32, u32, vp, sz, vp, vp, vp, vp]
+        L.hec_lambda_partitions.argtypes = [u32, vp, sz, ctypes.POINTER(sz)]
         L.hec_set_stream.argtypes = [vp]
         L.hec_set_regime.argtypes = [ctypes.c_int]
         L.hec_set_eval.argtypes = [ctypes.c_int]
@@ -278,18 +282,51 @@ def reduced_rows(q: int, g: int, d: int, first: int, n: int, device=None):
     return rows, mult
 
 
-def curve_map(q: int, g: int, d: int):
-    """hec_curve_map (two-call capacity protocol): (tuples [m][g] uint32, weights [m] uint64) on the host."""
+def curve_map(q: int, g: int, d: int, with_lambda: bool = False):
+    """hec_curve_map / hec_curve_map_lambda (two-call capacity protocol): (keys [m][g (+1)] uint32, weights [m] uint64)
+    on the host; with_lambda appends the lambda index (see lambda_partitions) as the last key column."""
     L = lib()
+    fn = L.hec_curve_map_lambda if with_lambda else L.hec_curve_map
+    cols = g + 1 if with_lambda else g
     m = ctypes.c_size_t(0)
-    rc = L.hec_curve_map(q, g, d, None, None, ctypes.c_size_t(0), ctypes.byref(m))
+    rc = fn(q, g, d, None, None, ctypes.c_size_t(0), ctypes.byref(m))
     if rc not in (HEC_OK, HEC_ERR_CAPACITY):
         _check(rc)
-    tup = np.empty((m.value, g), dtype=np.uint32)
+    tup = np.empty((m.value, cols), dtype=np.uint32)
     w = np.empty((m.value,), dtype=np.uint64)
     if m.value:
-        _check(L.hec_curve_map(q, g, d, _ptr(tup), _ptr(w), ctypes.c_size_t(m.value), ctypes.byref(m)))
+        _check(fn(q, g, d, _ptr(tup), _ptr(w), ctypes.c_size_t(m.value), ctypes.byref(m)))
     return tup[: m.value], w[: m.value]
+
+
+def lambda_partitions(g: int) -> list:
+    """hec_lambda_partitions: list of multiplicity vectors (n_1..n_{2g+2}); the position is the lambda index."""
+    L = lib()
+    m = ctypes.c_size_t(0)
+    rc = L.hec_lambda_partitions(g, None, ctypes.c_size_t(0), ctypes.byref(m))
+    if rc not in (HEC_OK, HEC_ERR_CAPACITY):
+        _check(rc)
+    out = np.empty((m.value, 2 * g + 2), dtype=np.uint8)
+    _check(L.hec_lambda_partitions(g, out.ctypes.data, ctypes.c_size_t(m.value), ctypes.byref(m)))
+    return [tuple(int(v) for v in row) for row in out]
+
+
+def count_ex(q: int, g: int, coeffs):
+    """hec_count_ex with every output: (counts [n][g], squarefree [n], roots [n][g], lambda index [n])."""
+    n = int(coeffs.shape[0])
+    if _is_torch(coeffs):
+        import torch
+        dev = coeffs.device
+        cnt = torch.empty((n, g), dtype=torch.int32, device=dev)
+        sf = torch.empty((n,), dtype=torch.uint8, device=dev)
+        r0 = torch.empty((n, g), dtype=torch.int32, device=dev)
+        lam = torch.empty((n,), dtype=torch.uint8, device=dev)
+    else:
+        coeffs = np.ascontiguousarray(coeffs, dtype=np.uint16)
+        cnt, sf = np.empty((n, g), dtype=np.uint32), np.empty((n,), dtype=np.uint8)
+        r0, lam = np.empty((n, g), dtype=np.uint32), np.empty((n,), dtype=np.uint8)
+    _check(lib().hec_count_ex(q, g, _ptr(coeffs), n, _ptr(cnt), _ptr(sf), _ptr(r0), _ptr(lam)))
+    return cnt, sf, r0, lam
 
 
 def last_count_stats() -> dict:

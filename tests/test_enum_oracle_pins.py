@@ -99,3 +99,9 @@ def test_p_dividing_d_is_rejected():
         list(E.reduced_polynomials(3, 6))
     with pytest.raises(ValueError):
         list(E.reduced_polynomials(49, 7))
+
+
+@pytest.mark.parametrize("q,g,d", [(3, 2, 5), (5, 1, 3), (5, 1, 4), (7, 1, 4), (5, 2, 6)])
+def test_reduced_map_with_lambda_equals_brute_force(q, g, d):
+    """Full key of (1.2): the reduction (shift, scaling, twist) preserves the factorisation type."""
+    assert E.reduced_map_lambda(q, g, d) == E.brute_force_map_lambda(q, g, d)
