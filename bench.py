@@ -32,6 +32,10 @@ if str(ROOT) not in sys.path:
 
 from paper_1805_11991_b200 import workloads as W  # noqa: E402
 
+# dram__bytes_read.sum + dram__bytes_write.sum of the count kernel, per launch at full size, from the committed
+# `ncu --set full` captures (profiles/r01c_ncu_full_c4_radix.md, profiles/r01c_ncu_full_c3_radix.md); None: not captured
+NCU_DRAM_TRAFFIC_BYTES = {"c4_q13_g4": 445.194752e6 + 321.563392e6, "c3_q49_g3": 93.999872e6 + 26.530560e6}
+
 EXPECTED_WAVEFRONTS = 3.53      # E[max bank load], 32 uniformly random 2-byte lookups in 32 banks
 
 
@@ -327,7 +331,8 @@ def run_ours(args, cfg):
         "kernel_share_of_step": k_ms * args.steps / elapsed_ms,
         "hbm": {"achieved_gbs": hbm_bytes / (k_ms * 1e-3) / 1e9, "peak_gbs": hbm_peak,
                 "frac": hbm_bytes / (k_ms * 1e-3) / 1e9 / hbm_peak, "algorithmic_bytes_per_launch": hbm_bytes},
-        "traffic": None,
+        "traffic": NCU_DRAM_TRAFFIC_BYTES.get(cfg.name),
+        "traffic_unit": "bytes per launch (ncu dram read + write, profiles/r01c_*); algorithmic: hbm.algorithmic_bytes_per_launch",
     }
     line = {
         "metric": "curves_per_s", "value": value, "unit": "curves/s", "n_gpus": world, "steps": args.steps,

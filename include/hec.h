@@ -152,7 +152,7 @@ int hec_histogram_merge(const uint32_t *in_tuples, const uint64_t *in_mult, size
  * Errors: HEC_ERR_UNSUPPORTED when p | d (reading G19: the printed set for p | d, misses every
  * polynomial with c_{d-1} = 0 != c_{d-2} and cannot be followed), HEC_ERR_INVALID_ARG (d, index range), HEC_ERR_CUDA.
  *
- * hec_curve_map -- N_{g,d}: for every reduced f (in chunks of 2^22 rows: rows kernel -> hec_count -> weighted
+ * hec_curve_map -- N_{g,d}: for every reduced f (in chunks of 2^24 rows, hec_set_map_chunk_rows: rows kernel -> hec_count -> weighted
  * histogram of the squarefree rows), add mult(f) at (N_1..N_g) and at the tuple of the quadratic twist n f
  * (Algorithm 1 lines 19-21; reading G8: N_k -> 2 q^k + 2 - N_k for odd k, N_k for even k).  The result equals
  * #{f squarefree of degree d over F_q with that tuple} (eq. (1.2) without lambda).  Output as for hec_histogram:
@@ -187,6 +187,8 @@ int hec_curve_map_lambda(uint32_t q, uint32_t g, uint32_t d, uint32_t *out_keys,
 int hec_reduced_total(uint32_t q, uint32_t g, uint32_t d, uint64_t *out_total);
 int hec_reduced_rows(uint32_t q, uint32_t g, uint32_t d, uint64_t first, size_t n, uint16_t *out_coeffs, uint64_t *out_mult);
 int hec_curve_map(uint32_t q, uint32_t g, uint32_t d, uint32_t *out_tuples, uint64_t *out_weights, size_t cap, size_t *out_m);
+/* Rows per chunk of hec_curve_map / hec_curve_map_lambda (default 2^24; device memory per chunk is about 90 B per row). */
+int hec_set_map_chunk_rows(size_t rows);
 
 /* ------------------------------------------------------------------------------------------------
  * Execution control and instrumentation (used by the tests, bench.py and the ncu runs).

@@ -30,6 +30,8 @@ int hec_histogram_weighted(const uint32_t *counts, const uint8_t *mask, const ui
 
 namespace {
 
+unsigned long long g_map_chunk_rows = 1ull << 24;   // hec_set_map_chunk_rows
+
 constexpr int kMaxFamilies = 2 + 12 * 11 / 2;      // d <= 2 HEC_MAX_GENUS + 2 = 12: i <= 10, j < i
 
 struct Family {
@@ -229,7 +231,7 @@ static int curve_map_impl(uint32_t q, uint32_t g, uint32_t d, bool with_lambda, 
     if ((rc = upload_generator_powers(q, gen, E))) return rc;
     const uint32_t cols = with_lambda ? g + 1 : g;             // key columns
 
-    const size_t chunk = (size_t)std::min<unsigned long long>(E.total, 1ull << 22);
+    const size_t chunk = (size_t)std::min<unsigned long long>(E.total, g_map_chunk_rows);
     Scratch rows, mult, counts, flags, lam, keys, part_t, part_w, acc_t, acc_w, cat_t, cat_w;
     if ((rc = rows.alloc(chunk * E.ncoef * 2)) || (rc = mult.alloc(chunk * 8)) || (rc = counts.alloc(chunk * g * 4)) ||
         (rc = flags.alloc(chunk)) || (rc = part_t.alloc(chunk * cols * 4)) || (rc = part_w.alloc(chunk * 8))) return rc;
@@ -301,6 +303,12 @@ static int curve_map_impl(uint32_t q, uint32_t g, uint32_t d, bool with_lambda, 
     HEC_CUDA_OK(cudaMemcpyAsync(out_tuples, fin_t.p, fin_m * cols * 4, kind, st));
     HEC_CUDA_OK(cudaMemcpyAsync(out_weights, fin_w.p, fin_m * 8, kind, st));
     HEC_CUDA_OK(cudaStreamSynchronize(st));
+    return HEC_OK;
+}
+
+int hec_set_map_chunk_rows(size_t rows) {
+    if (rows < 1024 || rows > (1ull << 28)) HEC_FAIL(HEC_ERR_INVALID_ARG, "chunk rows must be in [2^10, 2^28]");
+    g_map_chunk_rows = rows;
     return HEC_OK;
 }
 

@@ -34,7 +34,7 @@ SYMBOLS = [
     "hec_field_degree", "hec_field_q", "hec_field_Q", "hec_field_embed_unit", "hec_field_modulus",
     "hec_field_antilog", "hec_field_log", "hec_field_zech", "hec_field_embed", "hec_count", "hec_histogram",
     "hec_histogram_merge", "hec_reduced_total", "hec_reduced_rows", "hec_curve_map",
-    "hec_count_ex", "hec_lambda_partitions", "hec_curve_map_lambda",
+    "hec_count_ex", "hec_lambda_partitions", "hec_curve_map_lambda", "hec_set_map_chunk_rows",
     "hec_set_stream", "hec_set_regime", "hec_set_eval", "hec_last_count_stats", "hec_launch_count", "hec_gather_bench",
     "hec_shutdown",
 ]
@@ -84,6 +84,7 @@ def lib():
         L.hec_curve_map_lambda.argtypes = [u32, u32, u32, vp, vp, sz, ctypes.POINTER(sz)]
         L.hec_count_ex.argtypes = [u32, u32, vp, sz, vp, vp, vp, vp]
         L.hec_lambda_partitions.argtypes = [u32, vp, sz, ctypes.POINTER(sz)]
+        L.hec_set_map_chunk_rows.argtypes = [sz]
         L.hec_set_stream.argtypes = [vp]
         L.hec_set_regime.argtypes = [ctypes.c_int]
         L.hec_set_eval.argtypes = [ctypes.c_int]
@@ -297,6 +298,10 @@ def curve_map(q: int, g: int, d: int, with_lambda: bool = False):
     if m.value:
         _check(fn(q, g, d, _ptr(tup), _ptr(w), ctypes.c_size_t(m.value), ctypes.byref(m)))
     return tup[: m.value], w[: m.value]
+
+
+def set_map_chunk_rows(rows: int):
+    _check(lib().hec_set_map_chunk_rows(rows))
 
 
 def lambda_partitions(g: int) -> list:

@@ -79,13 +79,17 @@ def test_curve_map_equals_algorithm1_oracle(cuda, q, g, d):
 
 
 def test_curve_map_multichunk(cuda):
-    """More than one chunk of 2^22 reduced polynomials (q = 13, g = 3, d = 8: 5.66e6, two chunks): the map against the same
+    """More than one chunk of reduced polynomials (q = 13, g = 3, d = 8: 5.66e6 rows in chunks of 2^21): the map against the same
     pipeline assembled by hand with another chunking (hec_reduced_rows -> hec_count -> numpy), the closed-form total
     and the twist symmetry."""
     q, g, d = 13, 3, 8
     total = hec.reduced_total(q, g, d)
-    assert total > (1 << 22)
-    tup, w = hec.curve_map(q, g, d)
+    assert total > 2 * (1 << 21)
+    hec.set_map_chunk_rows(1 << 21)
+    try:
+        tup, w = hec.curve_map(q, g, d)
+    finally:
+        hec.set_map_chunk_rows(1 << 24)
     assert int(w.sum()) == (q - 1) * (q ** d - q ** (d - 1))
     acc = {}
     step = 1_500_001
