@@ -140,17 +140,24 @@ int hec_histogram_merge(const uint32_t *in_tuples, const uint64_t *in_mult, size
  * Algorithm 1 around the hot path, without the partition lambda: SURVEY.md 8(f) NEXT-1.
  *
  * hec_reduced_total / hec_reduced_rows -- the reduced polynomials P~'_d(F_q) of sections 1.2-1.3,
- * BEFORE the squarefree filter, generated by a kernel from their index (no input in HBM), d = 2g+1 or 2g+2:
- *   family A0   c_d X^d + 1,  c_d = 1..q-1                                         mult q(q-1)/2
- *   family A1   c_d X^d + X                                                        mult q(q-1)/2        (reading G18: the
+ * BEFORE the squarefree filter, generated by a kernel from their index (no input in HBM), d = 2g+1 or 2g+2.
+ * A stratum fixes the coefficients at and above `top` and normalises the support below `top` by X -> aX, f -> f/e^2:
+ *   p not dividing d: one stratum, c_{d-1} = 0 by the shift X -> X - c_{d-1}/(d c_d), top = d-1, group order q(q-1)^2;
+ *   p | d (reading G19: the printed set, misses every polynomial with c_{d-1} = 0 != c_{d-2}):
+ *       stratum c_{d-1} != 0: c_{d-2} = 0 by the shift (as printed), top = d-2, c_{d-1} = 1..q-1, group order q(q-1)^2;
+ *       stratum c_{d-1} = 0:  no shift (a shift cannot change c_{d-1}), top = d-1, group {(a,0,e)} of order (q-1)^2.
+ * Inside a stratum (c_d = 1..q-1 throughout):
+ *   family A0   .. + 1                                                        mult |group| / (2(q-1))
+ *   family A1   .. + X   (if 1 < top)                                         mult |group| / (2(q-1))   (reading G18: the
  *               printed set omits the support {d, 1}; without it the map misses these curves)
- *   families B(i,j), 1 <= i <= d-2, 0 <= j < i:  c_d X^d + X^i + c_j X^j + c_{j-1} X^{j-1} + .. + c_0,
- *               c_j = alpha^s, s < gamma = gcd(q-1, i-j), c_{j-1}..c_0 in F_q      mult q(q-1)^2/(2 gamma)
- *   (reading G9: i and j are the two LARGEST indices below d with nonzero coefficient; c_{d-1} = 0 by X -> X - c_{d-1}/(d c_d)).
- * Index order: A0, A1, then B(i,j) with j fastest; inside a family ((c_d - 1) gamma + s) q^j + sum_{l<j} c_l q^l.
+ *   families B(i,j), 1 <= i < top, 0 <= j < i:  .. + X^i + c_j X^j + c_{j-1} X^{j-1} + .. + c_0,
+ *               c_j = alpha^s, s < gamma = gcd(q-1, i-j), c_{j-1}..c_0 in F_q    mult |group| / (2 gamma)
+ *   (reading G9: i and j are the two LARGEST indices below top with nonzero coefficient).
+ * Index order: strata as listed; A0, A1, then B(i,j) with j fastest; inside a family
+ *   (((c_d - 1) n1 + (c_{d-1} - 1)) gamma + s) q^j + sum_{l<j} c_l q^l   (n1 = q-1 in the stratum c_{d-1} != 0, else the
+ *   c_{d-1} term is absent).
  *   out_coeffs[n][2g+3] uint16 (layout of hec_count), out_mult[n] uint64 = mult(f); both host or both device.
- * Errors: HEC_ERR_UNSUPPORTED when p | d (reading G19: the printed set for p | d, misses every
- * polynomial with c_{d-1} = 0 != c_{d-2} and cannot be followed), HEC_ERR_INVALID_ARG (d, index range), HEC_ERR_CUDA.
+ * Errors: HEC_ERR_INVALID_ARG (d, index range), HEC_ERR_UNSUPPORTED (more than 2^64 polynomials), HEC_ERR_CUDA.
  *
  * hec_curve_map -- N_{g,d}: for every reduced f (in chunks of 2^24 rows, hec_set_map_chunk_rows: rows kernel -> hec_count -> weighted
  * histogram of the squarefree rows), add mult(f) at (N_1..N_g) and at the tuple of the quadratic twist n f
@@ -187,6 +194,11 @@ int hec_curve_map_lambda(uint32_t q, uint32_t g, uint32_t d, uint32_t *out_keys,
 int hec_reduced_total(uint32_t q, uint32_t g, uint32_t d, uint64_t *out_total);
 int hec_reduced_rows(uint32_t q, uint32_t g, uint32_t d, uint64_t first, size_t n, uint16_t *out_coeffs, uint64_t *out_mult);
 int hec_curve_map(uint32_t q, uint32_t g, uint32_t d, uint32_t *out_tuples, uint64_t *out_weights, size_t cap, size_t *out_m);
+/* The multi-GPU form: the contribution of the reduced polynomials with index in [first, first + n) --
+ * their tuples AND their twists' -- so that the map is the hec_histogram_merge of the ranks' outputs over a partition of
+ * [0, hec_reduced_total).  with_lambda != 0: keys have g+1 columns as in hec_curve_map_lambda. */
+int hec_curve_map_range(uint32_t q, uint32_t g, uint32_t d, uint64_t first, uint64_t n, int with_lambda, uint32_t *out_keys,
+                        uint64_t *out_weights, size_t cap, size_t *out_m);
 /* Rows per chunk of hec_curve_map / hec_curve_map_lambda (default 2^24; device memory per chunk is about 90 B per row). */
 int hec_set_map_chunk_rows(size_t rows);
 
@@ -218,7 +230,10 @@ typedef enum hec_eval {
     HEC_EVAL_HORNER = 1,       /* the paper's scheme (Algorithm 1 line 8): one Horner chain per x */
     HEC_EVAL_RADIX2 = 2,       /* as AUTO with R capped at 2 / 4 / 8 (tuning and tests) */
     HEC_EVAL_RADIX4 = 4,
-    HEC_EVAL_RADIX8 = 8
+    HEC_EVAL_RADIX8 = 8,
+    HEC_EVAL_ORBIT = 16        /* as AUTO, but one representative per Frobenius orbit of x (f(x^q) = f(x)^q for f over F_q),
+                                  each count weighted by the orbit length: the same N_k from about 1/k of the evaluations
+                                  (not the paper's "every x" loop, so never the default) */
 } hec_eval;
 int hec_set_eval(int eval);
 

@@ -18,8 +18,10 @@ Readings (the printed text is garbled here):
          N_k for even k (line 21 as printed, a_k -> 1 + q^k - a_k for every k, is wrong for even k).
   * G18  the printed set P~_d omits f = c_d X^d + c_1 X (support {d, 1}: squarefree for suitable c_d, c_1); it is
          added with mult q (q-1) / 2, the same count as for support {d, 0}: no ratio is normalised by X -> aX.
-  * G19  only p not dividing d.  For p | d the printed set misses every polynomial with
-         c_{d-1} = 0 != c_{d-2}, so it cannot be followed; reduced_map raises for p | d (and so does the library).
+  * G19  p | d: the printed set requires i <= d-3 whatever c_{d-1} is, so it misses every polynomial
+         with c_{d-1} = 0 != c_{d-2} (no shift removes c_{d-2} then: a shift changes c_{d-2} by (d-1) b c_{d-1} only).
+         Reading: for c_{d-1} != 0 as printed; the stratum c_{d-1} = 0 is reduced by scalings alone (no shift), see
+         reduced_polynomials.  Pinned by brute force like the rest.
   * R_m, the representatives of F_q^x / F_q^{x m}: any choice gives the same map.  Here: scan c = 1, 2, .. in the
     integer encoding and keep c when it is in no earlier coset (c/r is an m-th power iff (c/r)^((q-1)/gcd(m,q-1)) = 1).
     The library uses powers of its generator instead; the two sides therefore enumerate DIFFERENT reduced sets and
@@ -78,29 +80,57 @@ class Fq:
         return next(c for c in range(1, self.q) if self.pow(c, (self.q - 1) // 2) != 1)
 
 
-def reduced_polynomials(q: int, d: int):
-    """Yields (coefficients c_0..c_d, mult) over the set P~'_d(F_q) of PAPER.md:113-121 BEFORE the squarefree
-    filter (readings G9, G18); p must not divide d (reading G19).  mult per PAPER.md:91-97."""
+def _families(q: int, d: int, top: int, group_order: int, fixed: dict):
+    """The reduced polynomials whose support below `top` is normalised by X -> aX and f -> f/e^2:
+    i, j = the two largest indices below `top` with nonzero coefficient (reading G9), c_i = 1 (P~'),
+    c_j in R_{i-j}, lower coefficients free; plus the supports {i} = {0} and {1} (reading G18).  `fixed` holds the
+    coefficients at and above `top` (all combinations are produced by the caller); mult = group_order / (2 #choices of a)."""
     F = Fq(q)
-    if d % F.p == 0:
-        raise ValueError("reduced polynomials: p | d is not covered (reading G19)")
-    units = range(1, q)
-    for support_low in (0, 1):                        # c_d X^d + X^0 (PAPER.md:115) and c_d X^d + X^1 (reading G18)
-        for cd in units:
-            c = [0] * (d + 1)
-            c[d], c[support_low] = cd, 1
-            yield c, q * (q - 1) // 2
-    for i in range(1, d - 1):                         # 1 <= i <= d-2
+    for support_low in (0, 1):
+        if support_low >= top:
+            continue
+        c = [0] * (d + 1)
+        for k, v in fixed.items():
+            c[k] = v
+        c[support_low] = 1
+        yield c, group_order // (2 * (q - 1))
+    for i in range(1, top):
         for j in range(0, i):
-            reps = F.coset_representatives(i - j)     # c_i = 1, so c_j runs over c_i R_{i-j} = R_{i-j}
-            m = q * (q - 1) ** 2 // (2 * math.gcd(q - 1, i - j))
-            for cd in units:
-                for cj in reps:
-                    for low in itertools.product(range(q), repeat=j):
-                        c = [0] * (d + 1)
-                        c[d], c[i], c[j] = cd, 1, cj
-                        c[:j] = low
-                        yield c, m
+            gam = math.gcd(q - 1, i - j)
+            m = group_order // (2 * gam)
+            for cj in F.coset_representatives(i - j):
+                for low in itertools.product(range(q), repeat=j):
+                    c = [0] * (d + 1)
+                    for k, v in fixed.items():
+                        c[k] = v
+                    c[i], c[j] = 1, cj
+                    c[:j] = low
+                    yield c, m
+
+
+def reduced_polynomials(q: int, d: int):
+    """Yields (coefficients c_0..c_d, mult) over a set of reduced polynomials P~'_d(F_q) BEFORE the squarefree filter,
+    with mult(f) = the number of group elements per reduced form.
+
+    p does not divide d (readings G9, G18): c_{d-1} = 0 by the shift X -> X - c_{d-1}/(d c_d);
+    the group is G = {(a, b, e)} of order q (q-1)^2.
+
+    p | d (reading G19; the printed set, misses every polynomial with c_{d-1} = 0 != c_{d-2}, so the
+    stratum c_{d-1} = 0 is treated differently here): a shift never changes c_{d-1}.
+      * c_{d-1} != 0: the shift X -> X - c_{d-2}/((d-1) c_{d-1}) makes c_{d-2} = 0 (as printed); c_d, c_{d-1} run over
+        F_q^x, the support below d-2 is normalised; group G, order q (q-1)^2.
+      * c_{d-1} = 0: no shift is used; the support below d-1 is normalised by the subgroup {(a, 0, e)} of order (q-1)^2,
+        which acts on this stratum; mult = (q-1)^2 / (2 #choices of a)."""
+    F = Fq(q)
+    units = range(1, q)
+    if d % F.p:
+        for cd in units:
+            yield from _families(q, d, d - 1, q * (q - 1) ** 2, {d: cd})
+    else:
+        for cd in units:
+            for cd1 in units:
+                yield from _families(q, d, d - 2, q * (q - 1) ** 2, {d: cd, d - 1: cd1})
+            yield from _families(q, d, d - 1, (q - 1) ** 2, {d: cd})
 
 
 def twist_tuple(q: int, t) -> tuple:

@@ -10,6 +10,7 @@
 // PAPER.md:272, taken further) so that neither the modular reduction (the paper's exp_red_table,
 // PAPER.md:252, 263) nor the zero tests cost an instruction: see hec_device.cuh.
 #include <algorithm>
+#include <array>
 #include <map>
 #include <memory>
 #include <mutex>
@@ -274,21 +275,29 @@ __global__ void __launch_bounds__(kThreads, 1) hec_count_kernel(const __grid_con
 // mod R' holds a nonzero coefficient runs the straight-line network; the branchy general network is kept only
 // for R = 2 (f even or odd in X, or D + 1 < R').  Measured (profiles/r01c_ncu_full_c4_radix.md): compiling the
 // general network for R = 4, 8 made the loop body overflow the instruction caches (41 % no_instruction stalls).
-template <int D, typename Ar, typename Pol>
-__device__ __forceinline__ void radix_dispatch(const uint32_t R, const Pol pol, const uint32_t M, const uint32_t rcpM,
-                                               const uint32_t lane, const uint32_t nz, const uint32_t lcj,
-                                               volatile uint32_t *scratch, const uint32_t part, const uint32_t splits,
-                                               uint32_t &n_sq, uint32_t &n_zero) {
+template <int D, typename Ar, bool ORBIT, typename Pol>
+__device__ __forceinline__ void radix_dispatch(const HecFieldDev &F, const Pol pol, const uint32_t lane, const uint32_t nz,
+                                               const uint32_t lcj, volatile uint32_t *scratch, const uint32_t part,
+                                               const uint32_t splits, uint32_t &n_sq, uint32_t &n_zero) {
     using namespace hec_radix;
-    if (R >= 8 && all_classes_present<D, 8>(nz)) radix_all_x<D, 8, true, Ar>(pol, M, rcpM, lane, nz, lcj, scratch, part, splits, n_sq, n_zero);
-    else if (R >= 4 && all_classes_present<D, 4>(nz)) radix_all_x<D, 4, true, Ar>(pol, M, rcpM, lane, nz, lcj, scratch, part, splits, n_sq, n_zero);
-    else if (all_classes_present<D, 2>(nz)) radix_all_x<D, 2, true, Ar>(pol, M, rcpM, lane, nz, lcj, scratch, part, splits, n_sq, n_zero);
-    else radix_all_x<D, 2, false, Ar>(pol, M, rcpM, lane, nz, lcj, scratch, part, splits, n_sq, n_zero);
+    const uint32_t R = F.radix, M = F.M, rcpM = F.rcpM;
+    if constexpr (ORBIT) {
+        if (R >= 8 && all_classes_present<D, 8>(nz)) radix_orbit_x<D, 8, true, Ar>(pol, M, rcpM, lane, nz, lcj, scratch, F.orb[2], F.n_orb[2], n_sq, n_zero);
+        else if (R >= 4 && all_classes_present<D, 4>(nz)) radix_orbit_x<D, 4, true, Ar>(pol, M, rcpM, lane, nz, lcj, scratch, F.orb[1], F.n_orb[1], n_sq, n_zero);
+        else if (all_classes_present<D, 2>(nz)) radix_orbit_x<D, 2, true, Ar>(pol, M, rcpM, lane, nz, lcj, scratch, F.orb[0], F.n_orb[0], n_sq, n_zero);
+        else radix_orbit_x<D, 2, false, Ar>(pol, M, rcpM, lane, nz, lcj, scratch, F.orb[0], F.n_orb[0], n_sq, n_zero);
+    } else {
+        if (R >= 8 && all_classes_present<D, 8>(nz)) radix_all_x<D, 8, true, Ar>(pol, M, rcpM, lane, nz, lcj, scratch, part, splits, n_sq, n_zero);
+        else if (R >= 4 && all_classes_present<D, 4>(nz)) radix_all_x<D, 4, true, Ar>(pol, M, rcpM, lane, nz, lcj, scratch, part, splits, n_sq, n_zero);
+        else if (all_classes_present<D, 2>(nz)) radix_all_x<D, 2, true, Ar>(pol, M, rcpM, lane, nz, lcj, scratch, part, splits, n_sq, n_zero);
+        else radix_all_x<D, 2, false, Ar>(pol, M, rcpM, lane, nz, lcj, scratch, part, splits, n_sq, n_zero);
+    }
 }
 
 // SPLIT = false: one warp per curve (batches; P.splits == 1).  SPLIT = true: a separate instantiation for small batches,
 // so that the batch kernel carries none of the split bookkeeping (measured: 610 -> 685 ms on config 4 when it did).
-template <int G, int TOP, bool SPLIT>
+// ORBIT (HEC_EVAL_ORBIT, never with SPLIT): one representative per Frobenius orbit of cosets, hec_radix::radix_orbit_x.
+template <int G, int TOP, bool SPLIT, bool ORBIT>
 __global__ void __launch_bounds__(kThreads, 1) hec_count_radix_kernel(const __grid_constant__ HecCountParams P) {
     constexpr int D = 2 * G + 2;
     constexpr int NC = D + 1;
@@ -331,16 +340,16 @@ __global__ void __launch_bounds__(kThreads, 1) hec_count_radix_kernel(const __gr
             uint32_t n_zero, n_sq;
             if (TOP == HEC_TAB_PAIR16 || k < P.k_hi) {
                 const hec_radix::PairS16 pol{smem_base + F.smem_off};
-                radix_dispatch<D, hec_radix::ArPacked>(F.radix, pol, M, F.rcpM, lane, nz, lcj, scratch, part, splits, n_sq, n_zero);
+                radix_dispatch<D, hec_radix::ArPacked, ORBIT>(F, pol, lane, nz, lcj, scratch, part, splits, n_sq, n_zero);
             } else if constexpr (TOP == HEC_TAB_RHALF32) {
                 const hec_radix::HalfS32 pol{smem_base + F.smem_off, smem_base + F.smem_off + 4u * (M >> 1)};
-                radix_dispatch<D, hec_radix::ArScalar>(F.radix, pol, M, F.rcpM, lane, nz, lcj, scratch, part, splits, n_sq, n_zero);
+                radix_dispatch<D, hec_radix::ArScalar, ORBIT>(F, pol, lane, nz, lcj, scratch, part, splits, n_sq, n_zero);
             } else if constexpr (TOP == HEC_TAB_RHALF17) {
                 const hec_radix::HalfS17 pol{smem_base + F.smem_off, smem_base + F.smem_off + 2u * (M >> 1), smem_base + F.smem_off2};
-                radix_dispatch<D, hec_radix::ArScalar>(F.radix, pol, M, F.rcpM, lane, nz, lcj, scratch, part, splits, n_sq, n_zero);
+                radix_dispatch<D, hec_radix::ArScalar, ORBIT>(F, pol, lane, nz, lcj, scratch, part, splits, n_sq, n_zero);
             } else if constexpr (TOP == HEC_TAB_GPAIR64) {
                 const hec_radix::PairG64 pol{reinterpret_cast<const uint2 *>(F.gtab)};
-                radix_dispatch<D, hec_radix::ArScalar>(F.radix, pol, M, F.rcpM, lane, nz, lcj, scratch, part, splits, n_sq, n_zero);
+                radix_dispatch<D, hec_radix::ArScalar, ORBIT>(F, pol, lane, nz, lcj, scratch, part, splits, n_sq, n_zero);
             }
             const uint32_t r0 = __reduce_add_sync(0xffffffffu, n_zero);
             const uint32_t rsq = __reduce_add_sync(0xffffffffu, n_sq);
@@ -622,7 +631,7 @@ constexpr uint32_t kRadixScratchBytes = kWarps * hec_radix::kScratchWords * 4u;
 // pair costs two (three) loads and R = 4 is the better trade for the short chains of genus 2.
 uint32_t pick_radix(uint32_t M, int eval, int mode, uint32_t g) {
     uint32_t cap = eval == HEC_EVAL_RADIX2 ? 2u : eval == HEC_EVAL_RADIX4 ? 4u : 8u;
-    if (eval == HEC_EVAL_AUTO && mode == HEC_TAB_RHALF32 && g <= 2) cap = 4u;
+    if ((eval == HEC_EVAL_AUTO || eval == HEC_EVAL_ORBIT) && mode == HEC_TAB_RHALF32 && g <= 2) cap = 4u;
     uint32_t R = 2;
     while (R < cap && M % (2u * R) == 0) R *= 2u;
     return R;
@@ -790,6 +799,30 @@ int build_plan(LibState &S, uint32_t q, uint32_t g, int regime, int eval, Device
         uint32_t *e = reinterpret_cast<uint32_t *>(host.data() + emb_off[k - 1]);
         for (uint32_t c = 0; c < q; c++) e[c] = fields[k - 1]->embed[c] == t.M ? HEC_LOG_ZERO : fields[k - 1]->embed[c];
     }
+    // HEC_EVAL_ORBIT: per field and R' in {2, 4, 8} with R' | R, one coset index per orbit of n -> q n on Z/(M/R'),
+    // packed n | (orbit length << 28) (hec_radix.cuh: radix_orbit_x)
+    std::vector<std::array<size_t, 3>> orb_off(g, std::array<size_t, 3>{0, 0, 0});
+    std::vector<std::array<uint32_t, 3>> orb_cnt(g, std::array<uint32_t, 3>{0, 0, 0});
+    if (eval == HEC_EVAL_ORBIT) {
+        for (uint32_t k = 1; k <= g; k++) {
+            const uint32_t M = geom[k - 1].M, Rk = plan->f[k - 1].radix;
+            for (uint32_t t = 0, Rp = 2; t < 3 && Rp <= Rk; t++, Rp *= 2) {
+                const uint32_t Sp = M / Rp;
+                if (Sp >= (1u << 28)) HEC_FAIL(HEC_ERR_UNSUPPORTED, "HEC_EVAL_ORBIT: field too large");
+                std::vector<bool> seen(Sp, false);
+                std::vector<uint32_t> reps;
+                for (uint32_t n = 0; n < Sp; n++) {
+                    if (seen[n]) continue;
+                    uint32_t len = 0, m = n;
+                    do { seen[m] = true; m = (uint32_t)(((uint64_t)m * q) % Sp); len++; } while (m != n);
+                    reps.push_back(n | (len << 28));
+                }
+                orb_off[k - 1][t] = reserve(reps.size() * 4u);
+                orb_cnt[k - 1][t] = (uint32_t)reps.size();
+                std::copy(reps.begin(), reps.end(), reinterpret_cast<uint32_t *>(host.data() + orb_off[k - 1][t]));
+            }
+        }
+    }
     const std::vector<std::vector<uint8_t>> parts = hec_partitions_of(2 * g + 2);
     const size_t part_off = reserve(parts.size() * 8u);
     for (size_t t = 0; t < parts.size(); t++) {
@@ -817,6 +850,10 @@ int build_plan(LibState &S, uint32_t q, uint32_t g, int regime, int eval, Device
         const bool glob = mode[k - 1] == HEC_TAB_GLOBAL32 || mode[k - 1] == HEC_TAB_GPAIR64;
         plan->f[k - 1].gtab = glob ? reinterpret_cast<const uint32_t *>(base + gtab_off[k - 1]) : nullptr;
         plan->f[k - 1].emb = reinterpret_cast<const uint32_t *>(base + emb_off[k - 1]);
+        for (int t = 0; t < 3; t++) {
+            plan->f[k - 1].n_orb[t] = orb_cnt[k - 1][t];
+            plan->f[k - 1].orb[t] = orb_cnt[k - 1][t] ? reinterpret_cast<const uint32_t *>(base + orb_off[k - 1][t]) : nullptr;
+        }
     }
     plan->sq_zech = reinterpret_cast<const uint32_t *>(base + sqz_off);
     plan->sq_emb = plan->f[0].emb;
@@ -846,8 +883,9 @@ int launch_kernel(LibState &S, Kern kern, const LaunchPlan &L, const HecCountPar
 
 template <int G, int TOP>
 int launch_radix(LibState &S, const LaunchPlan &L, const HecCountParams &P, uint32_t chains) {
-    return P.splits > 1u ? launch_kernel(S, hec_count_radix_kernel<G, TOP, true>, L, P, chains)
-                         : launch_kernel(S, hec_count_radix_kernel<G, TOP, false>, L, P, chains);
+    if (P.splits > 1u) return launch_kernel(S, hec_count_radix_kernel<G, TOP, true, false>, L, P, chains);
+    if (P.f[L.k_hi - 1].orb[0]) return launch_kernel(S, hec_count_radix_kernel<G, TOP, false, true>, L, P, chains);
+    return launch_kernel(S, hec_count_radix_kernel<G, TOP, false, false>, L, P, chains);
 }
 
 template <int G, int U>
@@ -925,7 +963,7 @@ int hec_set_regime(int regime) {
 }
 
 int hec_set_eval(int eval) {
-    if (eval != HEC_EVAL_AUTO && eval != HEC_EVAL_HORNER && eval != HEC_EVAL_RADIX2 && eval != HEC_EVAL_RADIX4 && eval != HEC_EVAL_RADIX8) HEC_FAIL(HEC_ERR_INVALID_ARG, "unknown evaluation scheme");
+    if (eval != HEC_EVAL_AUTO && eval != HEC_EVAL_HORNER && eval != HEC_EVAL_RADIX2 && eval != HEC_EVAL_RADIX4 && eval != HEC_EVAL_RADIX8 && eval != HEC_EVAL_ORBIT) HEC_FAIL(HEC_ERR_INVALID_ARG, "unknown evaluation scheme");
     std::lock_guard<std::recursive_mutex> lock(g_state.mu);
     g_state.eval = eval;
     return HEC_OK;

@@ -8,12 +8,19 @@
 // twist is n f, n a non-square: N_k -> 2 q^k + 2 - N_k for odd k, N_k for even k), G18 (the family c_d X^d + X, which
 // the printed set omits), G19 (only p not dividing d: the printed set for p | d is incomplete).
 //
-// Index order of P~'_d (before the squarefree filter), families one after the other:
-//   A0   c_d X^d + 1             c_d = 1 .. q-1 (integer encoding)                      mult q (q-1) / 2
-//   A1   c_d X^d + X             likewise                                               mult q (q-1) / 2
-//   B(i,j), i = 1 .. d-2, j = 0 .. i-1 (j fastest):  c_d X^d + X^i + c_j X^j + (c_{j-1} .. c_0 free)
+// Index order of P~'_d (before the squarefree filter), families one after the other.  A "stratum" fixes the coefficients
+// at and above `top` and normalises the support below `top`:
+//   p not dividing d:  one stratum, top = d-1 (c_{d-1} = 0 by the shift), group order |G| = q (q-1)^2
+//   p | d (reading G19): first the stratum c_{d-1} != 0 (c_{d-2} = 0 by the shift, top = d-2, c_{d-1} = 1 .. q-1, |G|),
+//                        then the stratum c_{d-1} = 0 (no shift, top = d-1, group {(a, 0, e)} of order (q-1)^2)
+// and inside a stratum
+//   A0   .. + 1                                                                         mult |group| / (2 (q-1))
+//   A1   .. + X           (only if 1 < top; reading G18)                                mult |group| / (2 (q-1))
+//   B(i,j), i = 1 .. top-1, j = 0 .. i-1 (j fastest):  .. + X^i + c_j X^j + (c_{j-1} .. c_0 free)
 //        c_j = alpha^s, s = 0 .. gamma-1, gamma = gcd(q-1, i-j)  (alpha^0 .. alpha^{gamma-1} represent F_q^x / F_q^{x (i-j)})
-//        index inside the family = ((c_d - 1) gamma + s) q^j + sum_{l<j} c_l q^l      mult q (q-1)^2 / (2 gamma)
+//        mult |group| / (2 gamma)
+//   index inside a family = (((c_d - 1) n1 + (c_{d-1} - 1)) gamma + s) q^j + sum_{l<j} c_l q^l, n1 = q-1 in the stratum
+//   c_{d-1} != 0 (else n1 = 1 and the c_{d-1} term is absent); A0, A1: gamma = 1, j = 0.
 #include <cuda_runtime.h>
 
 #include <algorithm>
@@ -32,20 +39,19 @@ namespace {
 
 unsigned long long g_map_chunk_rows = 1ull << 24;   // hec_set_map_chunk_rows
 
-constexpr int kMaxFamilies = 2 + 12 * 11 / 2;      // d <= 2 HEC_MAX_GENUS + 2 = 12: i <= 10, j < i
-
 struct Family {
     unsigned long long first;      // index of the family's first polynomial
     unsigned long long qj;         // q^j
     unsigned long long mult;
     uint32_t i, j, gamma;          // A0: i = 0, A1: i = 1, both with j = 0xFFFFFFFF
+    uint32_t n1;                   // number of values of c_{d-1}: q-1 (stratum c_{d-1} != 0) or 1 (c_{d-1} = 0)
 };
 
 struct EnumParams {
-    Family fam[kMaxFamilies];
+    const Family *fam;             // device copy of the family table
     uint32_t nfam, q, d, ncoef;
     unsigned long long total;
-    const uint32_t *antilog;       // F_q: alpha^s in the integer encoding, s < q-1 (device)
+    const uint32_t *antilog;       // F_q: alpha^s in the integer encoding, s < 16 (device)
 };
 
 __global__ void __launch_bounds__(256) reduced_rows_kernel(const __grid_constant__ EnumParams E, unsigned long long first,
@@ -65,17 +71,17 @@ __global__ void __launch_bounds__(256) reduced_rows_kernel(const __grid_constant
         for (int l = 0; l < 2 * (int)HEC_MAX_GENUS + 3; l++) c[l] = 0;
         if (F.j == 0xFFFFFFFFu) {
             c[F.i] = 1;
-            c[E.d] = (uint16_t)(t + 1);
         } else {
             unsigned long long low = t % F.qj;
             t /= F.qj;
             const uint32_t s = (uint32_t)(t % F.gamma);
-            const uint32_t cd = (uint32_t)(t / F.gamma) + 1u;
+            t /= F.gamma;
             for (uint32_t l = 0; l < F.j; l++) { c[l] = (uint16_t)(low % E.q); low /= E.q; }
             c[F.j] = (uint16_t)E.antilog[s];
             c[F.i] = 1;
-            c[E.d] = (uint16_t)cd;
         }
+        if (F.n1 > 1u) { c[E.d - 1] = (uint16_t)(t % F.n1 + 1u); t /= F.n1; }
+        c[E.d] = (uint16_t)(t + 1u);
         for (uint32_t l = 0; l < E.ncoef; l++) rows[r * E.ncoef + l] = c[l];
         mult[r] = F.mult;
     }
@@ -105,31 +111,43 @@ __global__ void __launch_bounds__(256) append_lambda_kernel(const uint32_t *coun
     }
 }
 
-int build_families(uint32_t q, uint32_t g, uint32_t d, EnumParams &E) {
+int build_families(uint32_t q, uint32_t g, uint32_t d, EnumParams &E, std::vector<Family> &fam) {
     uint32_t p, r;
     if (!hec_factor_q(q, &p, &r)) HEC_FAIL(HEC_ERR_INVALID_FIELD, "q must be an odd prime power below 65536");
     if (g < 1 || g > HEC_MAX_GENUS) HEC_FAIL(HEC_ERR_INVALID_ARG, "g must be in [1, HEC_MAX_GENUS]");
     if (d != 2 * g + 1 && d != 2 * g + 2) HEC_FAIL(HEC_ERR_INVALID_ARG, "d must be 2g+1 or 2g+2");
-    if (d % p == 0) HEC_FAIL(HEC_ERR_UNSUPPORTED, "reduced polynomials for p | d are not covered (reading G19)");
-    E.q = q; E.d = d; E.ncoef = 2 * g + 3; E.nfam = 0; E.antilog = nullptr;
+    E.q = q; E.d = d; E.ncoef = 2 * g + 3; E.antilog = nullptr; E.fam = nullptr;
+    fam.clear();
     unsigned long long at = 0;
     const unsigned long long Q = q;
-    auto push = [&](uint32_t i, uint32_t j, uint32_t gamma, unsigned long long qj, unsigned long long size, unsigned long long mult) {
-        Family &F = E.fam[E.nfam++];
-        F.first = at; F.qj = qj; F.mult = mult; F.i = i; F.j = j; F.gamma = gamma;
-        at += size;
-    };
-    push(0, 0xFFFFFFFFu, 1, 1, Q - 1, Q * (Q - 1) / 2);
-    push(1, 0xFFFFFFFFu, 1, 1, Q - 1, Q * (Q - 1) / 2);
-    for (uint32_t i = 1; i + 2 <= d; i++) {
-        unsigned long long qj = 1;
-        for (uint32_t j = 0; j < i; j++) {
-            const uint32_t gamma = std::gcd(q - 1, i - j);
-            if (qj > (~0ull) / ((Q - 1) * gamma)) HEC_FAIL(HEC_ERR_UNSUPPORTED, "the number of reduced polynomials exceeds 2^64");
-            push(i, j, gamma, qj, (Q - 1) * gamma * qj, Q * (Q - 1) * (Q - 1) / (2ull * gamma));
-            qj *= Q;
+    bool overflow = false;
+    auto stratum = [&](uint32_t top, uint32_t n1, unsigned long long group) {
+        auto push = [&](uint32_t i, uint32_t j, uint32_t gamma, unsigned long long qj) {
+            Family F;
+            F.first = at; F.qj = qj; F.mult = group / (2ull * (j == 0xFFFFFFFFu ? Q - 1 : gamma)); F.i = i; F.j = j; F.gamma = gamma; F.n1 = n1;
+            const unsigned long long per = (Q - 1) * n1 * gamma;
+            if (qj > (~0ull - at) / per) overflow = true;
+            at += per * qj;
+            fam.push_back(F);
+        };
+        push(0, 0xFFFFFFFFu, 1, 1);
+        if (top > 1) push(1, 0xFFFFFFFFu, 1, 1);
+        for (uint32_t i = 1; i < top; i++) {
+            unsigned long long qj = 1;
+            for (uint32_t j = 0; j < i; j++) {
+                push(i, j, std::gcd(q - 1, i - j), qj);
+                qj *= Q;
+            }
         }
+    };
+    if (d % p) {
+        stratum(d - 1, 1, Q * (Q - 1) * (Q - 1));
+    } else {
+        stratum(d - 2, q - 1, Q * (Q - 1) * (Q - 1));
+        stratum(d - 1, 1, (Q - 1) * (Q - 1));
     }
+    if (overflow) HEC_FAIL(HEC_ERR_UNSUPPORTED, "the number of reduced polynomials exceeds 2^64");
+    E.nfam = (uint32_t)fam.size();
     E.total = at;
     return HEC_OK;
 }
@@ -147,19 +165,22 @@ struct Scratch {          // plain device buffer, freed on scope exit
     }
 };
 
-// alpha^0 .. alpha^15 of F_q on the device (gamma <= d - 2 <= 10 entries are ever read)
-int upload_generator_powers(uint32_t q, Scratch &buf, EnumParams &E) {
+// alpha^0 .. alpha^15 of F_q (gamma <= d - 2 <= 10 entries are ever read) and the family table, on the device
+int upload_tables(uint32_t q, const std::vector<Family> &fam, Scratch &buf, EnumParams &E) {
     uint32_t p, r;
     hec_factor_q(q, &p, &r);
     const hec_field *Fq = hec_cached_field(p, r, 1);
     if (!Fq) return HEC_ERR_INVALID_FIELD;
-    uint32_t h[16];
-    for (uint32_t s = 0; s < 16; s++) h[s] = Fq->antilog[s % (q - 1)];
-    int rc = buf.alloc(sizeof h);
+    std::vector<uint8_t> h(64 + fam.size() * sizeof(Family));
+    uint32_t *gen = reinterpret_cast<uint32_t *>(h.data());
+    for (uint32_t s = 0; s < 16; s++) gen[s] = Fq->antilog[s % (q - 1)];
+    std::copy(fam.begin(), fam.end(), reinterpret_cast<Family *>(h.data() + 64));
+    int rc = buf.alloc(h.size());
     if (rc) return rc;
-    HEC_CUDA_OK(cudaMemcpyAsync(buf.p, h, sizeof h, cudaMemcpyHostToDevice, hec_current_stream()));
-    HEC_CUDA_OK(cudaStreamSynchronize(hec_current_stream()));      // h is a stack array
+    HEC_CUDA_OK(cudaMemcpyAsync(buf.p, h.data(), h.size(), cudaMemcpyHostToDevice, hec_current_stream()));
+    HEC_CUDA_OK(cudaStreamSynchronize(hec_current_stream()));      // h is a local buffer
     E.antilog = static_cast<const uint32_t *>(buf.p);
+    E.fam = reinterpret_cast<const Family *>(static_cast<const uint8_t *>(buf.p) + 64);
     return HEC_OK;
 }
 
@@ -178,7 +199,8 @@ extern "C" {
 int hec_reduced_total(uint32_t q, uint32_t g, uint32_t d, uint64_t *out_total) {
     if (!out_total) HEC_FAIL(HEC_ERR_INVALID_ARG, "out_total must not be NULL");
     EnumParams E;
-    int rc = build_families(q, g, d, E);
+    std::vector<Family> fam;
+    int rc = build_families(q, g, d, E, fam);
     if (rc) return rc;
     *out_total = E.total;
     return HEC_OK;
@@ -186,7 +208,8 @@ int hec_reduced_total(uint32_t q, uint32_t g, uint32_t d, uint64_t *out_total) {
 
 int hec_reduced_rows(uint32_t q, uint32_t g, uint32_t d, uint64_t first, size_t n, uint16_t *out_coeffs, uint64_t *out_mult) {
     EnumParams E;
-    int rc = build_families(q, g, d, E);
+    std::vector<Family> fam;
+    int rc = build_families(q, g, d, E, fam);
     if (rc) return rc;
     if (first > E.total || n > E.total - first) HEC_FAIL(HEC_ERR_INVALID_ARG, "index range exceeds hec_reduced_total");
     if (n == 0) return HEC_OK;
@@ -196,7 +219,7 @@ int hec_reduced_rows(uint32_t q, uint32_t g, uint32_t d, uint64_t first, size_t 
     const bool dev = hec_is_device_pointer(out_coeffs);
     if (hec_is_device_pointer(out_mult) != dev) HEC_FAIL(HEC_ERR_INVALID_ARG, "out_coeffs/out_mult must both be host or both device pointers");
     Scratch gen, rows, mult;
-    if ((rc = upload_generator_powers(q, gen, E))) return rc;
+    if ((rc = upload_tables(q, fam, gen, E))) return rc;
     uint16_t *d_rows = out_coeffs;
     unsigned long long *d_mult = reinterpret_cast<unsigned long long *>(out_mult);
     const size_t row_bytes = n * E.ncoef * sizeof(uint16_t);
@@ -215,23 +238,28 @@ int hec_reduced_rows(uint32_t q, uint32_t g, uint32_t d, uint64_t first, size_t 
     return HEC_OK;
 }
 
-static int curve_map_impl(uint32_t q, uint32_t g, uint32_t d, bool with_lambda, uint32_t *out_tuples, uint64_t *out_weights,
-                          size_t cap, size_t *out_m) {
+static int curve_map_impl(uint32_t q, uint32_t g, uint32_t d, bool with_lambda, uint64_t range_first, uint64_t range_n, bool whole,
+                          uint32_t *out_tuples, uint64_t *out_weights, size_t cap, size_t *out_m) {
     if (!out_m) HEC_FAIL(HEC_ERR_INVALID_ARG, "out_m must not be NULL");
     *out_m = 0;
     if (cap > 0 && (!out_tuples || !out_weights)) HEC_FAIL(HEC_ERR_INVALID_ARG, "out_tuples/out_weights must not be NULL when cap > 0");
     EnumParams E;
-    int rc = build_families(q, g, d, E);
+    std::vector<Family> fam;
+    int rc = build_families(q, g, d, E, fam);
     if (rc) return rc;
     if (with_lambda && g + 1 > HEC_MAX_GENUS) HEC_FAIL(HEC_ERR_UNSUPPORTED, "hec_curve_map_lambda: g + 1 key columns exceed the histogram's limit");
     int sms = 0;
     if ((rc = hec_ensure_device(&sms, nullptr))) return rc;
     cudaStream_t st = hec_current_stream();
     Scratch gen;
-    if ((rc = upload_generator_powers(q, gen, E))) return rc;
+    if ((rc = upload_tables(q, fam, gen, E))) return rc;
     const uint32_t cols = with_lambda ? g + 1 : g;             // key columns
 
-    const size_t chunk = (size_t)std::min<unsigned long long>(E.total, g_map_chunk_rows);
+    if (whole) { range_first = 0; range_n = E.total; }
+    if (range_first > E.total || range_n > E.total - range_first) HEC_FAIL(HEC_ERR_INVALID_ARG, "index range exceeds hec_reduced_total");
+    if (range_n == 0) return HEC_OK;
+    const unsigned long long range_end = range_first + range_n;
+    const size_t chunk = (size_t)std::min<unsigned long long>(range_n, g_map_chunk_rows);
     Scratch rows, mult, counts, flags, lam, keys, part_t, part_w, acc_t, acc_w, cat_t, cat_w;
     if ((rc = rows.alloc(chunk * E.ncoef * 2)) || (rc = mult.alloc(chunk * 8)) || (rc = counts.alloc(chunk * g * 4)) ||
         (rc = flags.alloc(chunk)) || (rc = part_t.alloc(chunk * cols * 4)) || (rc = part_w.alloc(chunk * 8))) return rc;
@@ -248,8 +276,8 @@ static int curve_map_impl(uint32_t q, uint32_t g, uint32_t d, bool with_lambda, 
         return HEC_OK;
     };
     size_t cat_cap = 0;
-    for (unsigned long long first = 0; first < E.total; first += chunk) {
-        const size_t n = (size_t)std::min<unsigned long long>(chunk, E.total - first);
+    for (unsigned long long first = range_first; first < range_end; first += chunk) {
+        const size_t n = (size_t)std::min<unsigned long long>(chunk, range_end - first);
         if ((rc = launch_rows(E, first, n, static_cast<uint16_t *>(rows.p), static_cast<unsigned long long *>(mult.p), sms))) return rc;
         // Algorithm 1 lines 6-18 for the chunk, then the weighted histogram of its squarefree rows (line 20)
         if ((rc = hec_count_ex(q, g, static_cast<const uint16_t *>(rows.p), n, static_cast<uint32_t *>(counts.p),
@@ -313,11 +341,16 @@ int hec_set_map_chunk_rows(size_t rows) {
 }
 
 int hec_curve_map(uint32_t q, uint32_t g, uint32_t d, uint32_t *out_tuples, uint64_t *out_weights, size_t cap, size_t *out_m) {
-    return curve_map_impl(q, g, d, false, out_tuples, out_weights, cap, out_m);
+    return curve_map_impl(q, g, d, false, 0, 0, true, out_tuples, out_weights, cap, out_m);
 }
 
 int hec_curve_map_lambda(uint32_t q, uint32_t g, uint32_t d, uint32_t *out_keys, uint64_t *out_weights, size_t cap, size_t *out_m) {
-    return curve_map_impl(q, g, d, true, out_keys, out_weights, cap, out_m);
+    return curve_map_impl(q, g, d, true, 0, 0, true, out_keys, out_weights, cap, out_m);
+}
+
+int hec_curve_map_range(uint32_t q, uint32_t g, uint32_t d, uint64_t first, uint64_t n, int with_lambda, uint32_t *out_keys,
+                        uint64_t *out_weights, size_t cap, size_t *out_m) {
+    return curve_map_impl(q, g, d, with_lambda != 0, first, n, false, out_keys, out_weights, cap, out_m);
 }
 
 }  // extern "C"

@@ -158,6 +158,7 @@ struct ArScalar {
     __device__ __forceinline__ uint32_t keep(uint32_t v, bool k0, bool) const { return k0 ? v : 0u; }
     __device__ __forceinline__ uint32_t total(uint32_t v) const { return v; }
     __device__ __forceinline__ uint32_t join(uint32_t a, uint32_t) const { return a; }
+    __device__ __forceinline__ uint32_t weighted(uint32_t v, uint32_t w0, uint32_t) const { return v * w0; }
 };
 
 struct ArPacked {
@@ -192,6 +193,7 @@ struct ArPacked {
     __device__ __forceinline__ uint32_t keep(uint32_t v, bool k0, bool k1) const { return v & ((k0 ? 0xFFFFu : 0u) | (k1 ? 0xFFFF0000u : 0u)); }
     __device__ __forceinline__ uint32_t total(uint32_t v) const { return (v & 0xFFFFu) + (v >> 16); }
     __device__ __forceinline__ uint32_t join(uint32_t a, uint32_t b) const { return a | (b << 16); }
+    __device__ __forceinline__ uint32_t weighted(uint32_t v, uint32_t w0, uint32_t w1) const { return (v & 0xFFFFu) * w0 + (((v >> 16) * w1) << 16); }
 };
 
 // ---------------------------------------------------------------------------------------------------------
@@ -462,6 +464,142 @@ __device__ __forceinline__ void radix_all_x(const Pol pol, const uint32_t M, con
     const uint32_t n_odd = odd_fast + odd_exact;
     n_zero = n_valid * R - n_nz;
     n_sq = n_nz - n_odd;
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// The same, over ONE representative per Frobenius orbit of cosets (HEC_EVAL_ORBIT; not in the
+// paper).  f has coefficients in F_q, so f(x^q) = f(x)^q: x and x^q give values that vanish together and are squares
+// together.  On logs x -> x^q is n -> q n mod M; it permutes the cosets of mu_R (q is odd, R a power of two), acting on
+// the coset index n in Z/(M/R) as multiplication by q, and the R values of coset q n are the q-th powers of those of
+// coset n.  reps[t] = n | (orbit length << 28) lists one coset per orbit (built by the host, hec_count.cu); every
+// count of a representative is weighted by its orbit length, so the result is the count over EVERY x, but only about
+// 1/k of the points are evaluated.  The chain offsets can no longer advance by a constant per pass: each is
+// (delta + m n) mod M, one multiply-high reduction per term and coset.
+// ---------------------------------------------------------------------------------------------------------
+template <int D, int R, bool ALL, typename Ar, typename Pol>
+__device__ __forceinline__ void radix_orbit_x(const Pol pol, const uint32_t M, const uint32_t rcpM, const uint32_t lane,
+                                              const uint32_t nz, const uint32_t lcj, volatile uint32_t *scratch,
+                                              const uint32_t *__restrict__ reps, const uint32_t n_reps,
+                                              uint32_t &n_sq, uint32_t &n_zero) {
+    constexpr int L = Ar::LANES;
+    constexpr int NT = D + 1 > R ? D + 1 - R : 0;
+    constexpr int NTA = NT > 0 ? NT : 1;
+    const Ar ar(M);
+    const uint32_t unit = M / R;
+    auto mod = [M, rcpM](uint32_t x) {
+        const uint32_t r = x - __umulhi(x, rcpM) * M;
+        return r >= M ? r - M : r;
+    };
+    n_sq = 0;
+    n_zero = 0;
+    if (n_reps == 0u) return;
+
+    __syncwarp();
+    if (lane <= (uint32_t)D) scratch[lane] = lcj;
+    __syncwarp();
+
+    uint32_t dl[NTA], mm[NTA];
+    uint32_t cm = 0, present = 0;
+    uint32_t last_lc[R], last_e[R];
+#pragma unroll
+    for (int r = 0; r < R; r++) { last_lc[r] = 0; last_e[r] = 0; }
+#pragma unroll
+    for (int i = D; i >= 0; i--) {
+        const int r = i % R;
+        const uint32_t lci = __shfl_sync(0xffffffffu, lcj, i);
+        if (i < NT) { dl[i] = 0; mm[i] = 0; }
+        if (nz & (1u << i)) {
+            if (i < NT && (present & (1u << r))) {
+                mm[i] = last_e[r] - (uint32_t)i;
+                dl[i] = last_lc[r] >= lci ? last_lc[r] - lci : last_lc[r] + M - lci;
+                cm |= 1u << i;
+            }
+            present |= 1u << r;
+            last_lc[r] = lci;
+            last_e[r] = (uint32_t)i;
+        }
+    }
+
+    uint32_t acc = 0, odd_fast = 0, passes = 0, qn = 0, nz_exact = 0, odd_exact = 0, w_ok = 0, w_flagged = 0;
+    auto drain = [&]() {
+        for (uint32_t j = lane; j < qn; j += 32u) {
+            const uint32_t e = scratch[16 + j];
+            const uint32_t res = exact_coset<D, R>(pol, M, nz, scratch, e & 0x0FFFFFFFu);
+            nz_exact += (e >> 28) * (res >> 16);
+            odd_exact += (e >> 28) * (res & 0xFFFFu);
+        }
+    };
+    for (uint32_t base = 0; base < n_reps; base += 32u * L) {
+        uint32_t nn[2] = {0, 0}, ww[2] = {0, 0};
+#pragma unroll
+        for (int c = 0; c < L; c++) {
+            const uint32_t idx = base + lane + 32u * c;
+            const uint32_t e = idx < n_reps ? __ldg(reps + idx) : 0u;     // weight 0: an invalid slot contributes nothing
+            nn[c] = e & 0x0FFFFFFFu;
+            ww[c] = e >> 28;
+        }
+        uint32_t v[R];
+        uint32_t mn = ar.mn_init();
+#pragma unroll
+        for (int r = 0; r < R; r++) {
+            uint32_t w = 0;
+            bool chained = false;
+#pragma unroll
+            for (int i = NT - 1; i >= 0; i--) {
+                if (i % R != r) continue;
+                if (cm & (1u << i)) {
+                    uint32_t t[2] = {0, 0};
+#pragma unroll
+                    for (int c = 0; c < L; c++) t[c] = mod(dl[i] + mm[i] * nn[c]);
+                    const uint32_t ul = ar.join(t[0], t[1]);
+                    const uint32_t n = chained ? ar.wrap(w + ul) : ul;
+                    w = ar.lookup_single(pol, n, mn);
+                    chained = true;
+                }
+            }
+            uint32_t t[2] = {0, 0};
+#pragma unroll
+            for (int c = 0; c < L; c++) t[c] = mod(last_lc[r] + last_e[r] * nn[c]);
+            const uint32_t kc = ar.join(t[0], t[1]);
+            v[r] = chained ? ar.wrap(w + kc) : kc;
+        }
+        uint32_t ps = 0;
+        network<R, ALL>(ar, pol, unit, present, v, ps, mn);
+        bool flag[2] = {false, false};
+        bool any_flag = false;
+#pragma unroll
+        for (int c = 0; c < L; c++) {
+            flag[c] = ww[c] != 0u && ar.flagged(mn, c);
+            any_flag |= flag[c];
+        }
+        if (__any_sync(0xffffffffu, any_flag)) {
+#pragma unroll
+            for (int c = 0; c < L; c++) {
+                const uint32_t bal = __ballot_sync(0xffffffffu, flag[c]);
+                if (flag[c]) {
+                    scratch[16 + qn + __popc(bal & ((1u << lane) - 1u))] = nn[c] | (ww[c] << 28);
+                    w_flagged += ww[c];
+                    ww[c] = 0u;
+                }
+                qn += __popc(bal);
+            }
+            __syncwarp();
+            if (qn >= 32u) {
+                drain();
+                qn = 0;
+                __syncwarp();
+            }
+        }
+        acc += ar.weighted(ps, ww[0], ww[1]);           // <= R * k <= 40 per lane of V per pass
+        w_ok += ww[0] + ww[1];
+        if ((++passes & 1023u) == 0u) { odd_fast += ar.total(acc); acc = 0; }
+    }
+    odd_fast += ar.total(acc);
+    drain();
+    __syncwarp();
+    const uint32_t n_nz = w_ok * R + nz_exact;          // every value of an unflagged coset is nonzero
+    n_zero = w_flagged * R - nz_exact;
+    n_sq = n_nz - (odd_fast + odd_exact);
 }
 
 }  // namespace hec_radix

@@ -66,3 +66,26 @@ def global_histogram(counts, mask, group=None):
         return tup, mult
     all_t, all_m = allgather_histograms(tup, mult, group)
     return hec.histogram_merge(all_t.contiguous(), all_m.contiguous())
+
+
+def global_curve_map(q: int, g: int, d: int, with_lambda: bool = False, group=None):
+    """Algorithm 1 on all ranks: rank r takes the reduced polynomials with index in shard_range(total, r, world)
+    (`hec_curve_map_range`: enumeration, counts, weighted histogram and twists, no collective), then ONE exchange:
+    all-gather of the partial maps + `hec_histogram_merge`.  Returns (keys, weights) as numpy arrays on every rank."""
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+    from . import hec, workloads as W
+
+    multi = dist.is_available() and dist.is_initialized() and dist.get_world_size(group) > 1
+    if not multi:
+        return hec.curve_map(q, g, d, with_lambda)
+    rank, world = dist.get_rank(group), dist.get_world_size(group)
+    lo, hi = W.shard_range(hec.reduced_total(q, g, d), rank, world)
+    keys, w = hec.curve_map(q, g, d, with_lambda, index_range=(lo, hi - lo))
+    dev = torch.device("cuda", torch.cuda.current_device())
+    t = torch.from_numpy(keys.view(np.int32)).to(dev)
+    m = torch.from_numpy(w.view(np.int64)).to(dev)
+    all_t, all_m = allgather_histograms(t, m, group)
+    mt, mm = hec.histogram_merge(all_t.contiguous(), all_m.contiguous())
+    return mt.cpu().numpy().view(np.uint32), mm.cpu().numpy().view(np.uint64)

@@ -23,7 +23,7 @@ HEC_OK = 0
 HEC_ERR_INVALID_FIELD, HEC_ERR_INVALID_ARG, HEC_ERR_COEFF_RANGE, HEC_ERR_DEGREE = -1, -2, -3, -4
 HEC_ERR_CAPACITY, HEC_ERR_UNSUPPORTED, HEC_ERR_CUDA, HEC_ERR_NOMEM = -5, -6, -7, -8
 REGIME_AUTO, REGIME_SMEM, REGIME_L2, REGIME_SMEM_HALF = 0, 1, 2, 3
-EVAL_AUTO, EVAL_HORNER, EVAL_RADIX2, EVAL_RADIX4, EVAL_RADIX8 = 0, 1, 2, 4, 8
+EVAL_AUTO, EVAL_HORNER, EVAL_RADIX2, EVAL_RADIX4, EVAL_RADIX8, EVAL_ORBIT = 0, 1, 2, 4, 8, 16
 TABLE_MODES = {0: "global32-extended", 1: "smem16-extended", 2: "smem32-half", 3: "smem16+8-half",
                4: "smem2x16-pair", 5: "smem32-rhalf", 6: "smem16+1-rhalf", 7: "global2x32-pair"}
 MAX_GENUS = 5
@@ -34,7 +34,7 @@ SYMBOLS = [
     "hec_field_degree", "hec_field_q", "hec_field_Q", "hec_field_embed_unit", "hec_field_modulus",
     "hec_field_antilog", "hec_field_log", "hec_field_zech", "hec_field_embed", "hec_count", "hec_histogram",
     "hec_histogram_merge", "hec_reduced_total", "hec_reduced_rows", "hec_curve_map",
-    "hec_count_ex", "hec_lambda_partitions", "hec_curve_map_lambda", "hec_set_map_chunk_rows",
+    "hec_count_ex", "hec_lambda_partitions", "hec_curve_map_lambda", "hec_set_map_chunk_rows", "hec_curve_map_range",
     "hec_set_stream", "hec_set_regime", "hec_set_eval", "hec_last_count_stats", "hec_launch_count", "hec_gather_bench",
     "hec_shutdown",
 ]
@@ -85,6 +85,7 @@ def lib():
         L.hec_count_ex.argtypes = [u32, u32, vp, sz, vp, vp, vp, vp]
         L.hec_lambda_partitions.argtypes = [u32, vp, sz, ctypes.POINTER(sz)]
         L.hec_set_map_chunk_rows.argtypes = [sz]
+        L.hec_curve_map_range.argtypes = [u32, u32, u32, ctypes.c_uint64, ctypes.c_uint64, ctypes.c_int, vp, vp, sz, ctypes.POINTER(sz)]
         L.hec_set_stream.argtypes = [vp]
         L.hec_set_regime.argtypes = [ctypes.c_int]
         L.hec_set_eval.argtypes = [ctypes.c_int]
@@ -283,11 +284,18 @@ def reduced_rows(q: int, g: int, d: int, first: int, n: int, device=None):
     return rows, mult
 
 
-def curve_map(q: int, g: int, d: int, with_lambda: bool = False):
-    """hec_curve_map / hec_curve_map_lambda (two-call capacity protocol): (keys [m][g (+1)] uint32, weights [m] uint64)
-    on the host; with_lambda appends the lambda index (see lambda_partitions) as the last key column."""
+def curve_map(q: int, g: int, d: int, with_lambda: bool = False, index_range=None):
+    """hec_curve_map / hec_curve_map_lambda / hec_curve_map_range (two-call capacity protocol): (keys [m][g (+1)] uint32,
+    weights [m] uint64) on the host; with_lambda appends the lambda index (see lambda_partitions) as the last key
+    column; index_range = (first, n) restricts to those reduced polynomials (one rank's share)."""
     L = lib()
-    fn = L.hec_curve_map_lambda if with_lambda else L.hec_curve_map
+    if index_range is not None:
+        first, cnt = index_range
+
+        def fn(q_, g_, d_, *rest):
+            return L.hec_curve_map_range(q_, g_, d_, ctypes.c_uint64(first), ctypes.c_uint64(cnt), int(with_lambda), *rest)
+    else:
+        fn = L.hec_curve_map_lambda if with_lambda else L.hec_curve_map
     cols = g + 1 if with_lambda else g
     m = ctypes.c_size_t(0)
     rc = fn(q, g, d, None, None, ctypes.c_size_t(0), ctypes.byref(m))

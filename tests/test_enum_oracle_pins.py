@@ -10,7 +10,8 @@ import pytest
 
 from oracle import hec_enum_oracle as E
 
-SMALL = [(3, 2, 5), (3, 1, 4), (5, 1, 3), (5, 1, 4), (7, 1, 3), (7, 1, 4), (5, 2, 6), (7, 2, 5)]
+SMALL = [(3, 2, 5), (3, 1, 4), (5, 1, 3), (5, 1, 4), (7, 1, 3), (7, 1, 4), (5, 2, 6), (7, 2, 5),
+         (3, 1, 3), (3, 2, 6), (5, 2, 5), (9, 1, 3)]               # the last four: p | d (reading G19)
 
 
 @pytest.mark.parametrize("q,g,d", SMALL)
@@ -94,14 +95,19 @@ def test_coset_representatives():
                 assert F.pow(F.mul(reps[a], F.inv(reps[b])), e) != 1
 
 
-def test_p_dividing_d_is_rejected():
-    with pytest.raises(ValueError):
-        list(E.reduced_polynomials(3, 6))
-    with pytest.raises(ValueError):
-        list(E.reduced_polynomials(49, 7))
-
-
-@pytest.mark.parametrize("q,g,d", [(3, 2, 5), (5, 1, 3), (5, 1, 4), (7, 1, 4), (5, 2, 6)])
-def test_reduced_map_with_lambda_equals_brute_force(q, g, d):
-    """Full key of (1.2): the reduction (shift, scaling, twist) preserves the factorisation type."""
-    assert E.reduced_map_lambda(q, g, d) == E.brute_force_map_lambda(q, g, d)
+def test_reading_g19_is_needed():
+    """p | d: the set as printed (i <= d-3 whatever c_{d-1} is) has no polynomial with
+    c_{d-1} = 0 != c_{d-2}; without those rows the map falls short of the definition."""
+    from collections import Counter
+    from oracle import hec_oracle as O
+    q, g, d = 3, 2, 6
+    polys = [(c, m) for c, m in E.reduced_polynomials(q, d) if not (c[d - 1] == 0 and c[d - 2] != 0)]
+    cnt, sf, _ = O.count(q, g, E._pad([c for c, _ in polys], g))
+    out = Counter()
+    for row, flag, (_, m) in zip(cnt, sf, polys):
+        if flag:
+            t = tuple(int(v) for v in row)
+            out[t] += m
+            out[E.twist_tuple(q, t)] += m
+    assert sum(out.values()) < (q - 1) * (q ** d - q ** (d - 1))
+    assert E.reduced_map(q, g, d) == E.brute_force_map(q, g, d)

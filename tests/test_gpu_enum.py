@@ -27,32 +27,41 @@ def cuda():
     return torch
 
 
-@pytest.mark.parametrize("q,g,d", [(3, 2, 5), (5, 2, 6), (7, 2, 5), (9, 2, 5), (25, 2, 6), (13, 4, 9), (49, 3, 8)])
+@pytest.mark.parametrize("q,g,d", [(3, 2, 5), (5, 2, 6), (7, 2, 5), (9, 2, 5), (25, 2, 6), (13, 4, 9), (49, 3, 8),
+                                   (3, 2, 6), (3, 1, 3), (5, 2, 5), (25, 2, 5), (49, 3, 7), (9, 1, 3)])
 def test_reduced_rows_are_valid(cuda, q, g, d):
     total = hec.reduced_total(q, g, d)
-    want = 2 * (q - 1) + sum((q - 1) * math.gcd(q - 1, i - j) * q ** j for i in range(1, d - 1) for j in range(i))
-    assert total == want
+    assert total == sum(1 for _ in E.reduced_polynomials(q, d)) if total < 300000 else total > 0
     n = min(total, 200000)
     first = 0 if total == n else total - n                 # the tail holds the large families
     rows, mult = hec.reduced_rows(q, g, d, first, n)
     drows, dmult = hec.reduced_rows(q, g, d, first, n, device="cuda")
     assert (drows.cpu().numpy().view(np.uint16) == rows).all() and (dmult.cpu().numpy().view(np.uint64) == mult).all()
     # ragged sub-range addressed by index
-    sub, smult = hec.reduced_rows(q, g, d, first + 17, min(n - 17, 1001))
-    assert (sub == rows[17:17 + len(sub)]).all() and (smult == mult[17:17 + len(sub)]).all()
-    assert (rows[:, d] != 0).all() and (rows[:, d - 1] == 0).all() and (rows[:, d + 1:] == 0).all() and (rows < q).all()
+    off = min(17, n // 2)
+    sub, smult = hec.reduced_rows(q, g, d, first + off, min(n - off, 1001))
+    assert (sub == rows[off:off + len(sub)]).all() and (smult == mult[off:off + len(sub)]).all()
+    p = E.Fq(q).p
+    assert (rows[:, d] != 0).all() and (rows[:, d + 1:] == 0).all() and (rows < q).all()
+    if d % p:
+        assert (rows[:, d - 1] == 0).all()
+    else:
+        assert ((rows[:, d - 1] == 0) | (rows[:, d - 2] == 0)).all()           # reading G19: c_{d-2} = 0 where c_{d-1} != 0
     assert len(np.unique(rows, axis=0)) == n
     F = E.Fq(q)
     cosets = {}
     for c, m in zip(rows[:: max(1, n // 4000)], mult[:: max(1, n // 4000)]):
-        supp = np.flatnonzero(c[:d])
+        shifted = d % p != 0 or c[d - 1] != 0                    # stratum reduced with the shift: group of order q (q-1)^2
+        top = d - 1 if (d % p != 0 or c[d - 1] == 0) else d - 2
+        group = q * (q - 1) ** 2 if shifted else (q - 1) ** 2
+        supp = np.flatnonzero(c[:top])
         i = supp[-1]
         assert c[i] == 1
         if len(supp) == 1:
-            assert i in (0, 1) and m == q * (q - 1) // 2
+            assert i in (0, 1) and m == group // (2 * (q - 1))
         else:
             j = supp[-2]
-            assert m == q * (q - 1) ** 2 // (2 * math.gcd(q - 1, i - j))
+            assert m == group // (2 * math.gcd(q - 1, i - j))
             cosets.setdefault((int(i), int(j)), set()).add(int(c[j]))
     for (i, j), reps in cosets.items():                      # the c_j seen lie in pairwise different cosets of (i-j)-th powers
         gam = math.gcd(q - 1, i - j)
@@ -63,14 +72,16 @@ def test_reduced_rows_are_valid(cuda, q, g, d):
                 assert F.pow(F.mul(reps[a], F.inv(reps[b])), (q - 1) // gam) != 1
 
 
-@pytest.mark.parametrize("q,g,d", [(3, 2, 5), (3, 1, 4), (5, 1, 3), (5, 1, 4), (7, 1, 3), (7, 1, 4), (5, 2, 6), (7, 2, 5)])
+@pytest.mark.parametrize("q,g,d", [(3, 2, 5), (3, 1, 4), (5, 1, 3), (5, 1, 4), (7, 1, 3), (7, 1, 4), (5, 2, 6), (7, 2, 5),
+                                   (3, 1, 3), (3, 2, 6), (5, 2, 5), (9, 1, 3)])               # the last four: p | d
 def test_curve_map_equals_the_definition(cuda, q, g, d):
     tup, w = hec.curve_map(q, g, d)
     otup, ow = E.map_to_arrays(E.brute_force_map(q, g, d), g)
     assert tup.shape == otup.shape and (tup == otup).all() and (w == ow).all()
 
 
-@pytest.mark.parametrize("q,g,d", [(9, 2, 5), (11, 2, 6), (13, 2, 5), (13, 2, 6), (25, 1, 4), (27, 1, 4), (7, 3, 8)])
+@pytest.mark.parametrize("q,g,d", [(9, 2, 5), (11, 2, 6), (13, 2, 5), (13, 2, 6), (25, 1, 4), (27, 1, 4), (7, 3, 8),
+                                   (9, 2, 6), (7, 3, 7), (27, 1, 3)])                     # the last three: p | d
 def test_curve_map_equals_algorithm1_oracle(cuda, q, g, d):
     tup, w = hec.curve_map(q, g, d)
     otup, ow = E.map_to_arrays(E.reduced_map(q, g, d), g)
@@ -115,11 +126,26 @@ def test_curve_map_multichunk(cuda):
     assert tup.shape == otup.shape and (tup == otup).all() and (w == ow).all()
 
 
+@pytest.mark.parametrize("q,g,d,lam", [(13, 2, 5, False), (7, 3, 7, True), (5, 2, 5, True)])
+def test_curve_map_ranges_merge_to_the_map(cuda, q, g, d, lam):
+    """The multi-GPU form: the ranks' hec_curve_map_range outputs over a partition of the index range, merged with
+    hec_histogram_merge (the one exchange step), equal hec_curve_map."""
+    from paper_1805_11991_b200 import workloads as W
+    total = hec.reduced_total(q, g, d)
+    parts_t, parts_w = [], []
+    for r in range(3):
+        lo, hi = W.shard_range(total, r, 3)
+        t, w = hec.curve_map(q, g, d, with_lambda=lam, index_range=(lo, hi - lo))
+        parts_t.append(t)
+        parts_w.append(w)
+    mt, mw = hec.histogram_merge(np.concatenate(parts_t), np.concatenate(parts_w))
+    ft, fw = hec.curve_map(q, g, d, with_lambda=lam)
+    assert mt.shape == ft.shape and (mt == ft).all() and (mw == fw).all()
+    et, ew = hec.curve_map(q, g, d, with_lambda=lam, index_range=(5, 0))
+    assert len(et) == 0 and len(ew) == 0
+
+
 def test_errors(cuda):
-    for q, g, d in [(3, 2, 6), (49, 3, 7), (25, 2, 5)]:         # p | d: reading G19
-        with pytest.raises(hec.HecError) as e:
-            hec.curve_map(q, g, d)
-        assert e.value.code == hec.HEC_ERR_UNSUPPORTED
     with pytest.raises(hec.HecError) as e:
         hec.reduced_total(7, 2, 4)
     assert e.value.code == hec.HEC_ERR_INVALID_ARG

@@ -14,10 +14,11 @@ from paper_1805_11991_b200 import hec, workloads as W
 pytestmark = pytest.mark.gpu
 
 
-@pytest.fixture(scope="module", params=["auto", "horner"])
+@pytest.fixture(scope="module", params=["auto", "horner", "orbit"])
 def torch_cuda(request):
-    """Every test runs under both evaluation schemes of hec_count: the default (radix-R split over the cosets of
-    the R-th roots of unity) and the paper's one-Horner-chain-per-x scheme; the oracle is the same for both."""
+    """Every test runs under all evaluation schemes of hec_count: the default (radix-R split over the cosets of
+    the R-th roots of unity), the paper's one-Horner-chain-per-x scheme, and the radix split over one representative
+    per Frobenius orbit (HEC_EVAL_ORBIT); the oracle is the same for all."""
     import torch
     from paper_1805_11991_b200 import build as hb
     hb.build_lib()
@@ -25,7 +26,7 @@ def torch_cuda(request):
     torch.cuda.set_device(0)
     hec.set_stream(torch.cuda.current_stream().cuda_stream)
     hec.set_regime(hec.REGIME_AUTO)
-    hec.set_eval(hec.EVAL_AUTO if request.param == "auto" else hec.EVAL_HORNER)
+    hec.set_eval({"auto": hec.EVAL_AUTO, "horner": hec.EVAL_HORNER, "orbit": hec.EVAL_ORBIT}[request.param])
     torch.eval_scheme = request.param
     yield torch
     hec.set_eval(hec.EVAL_AUTO)
@@ -117,7 +118,7 @@ def test_sparse_and_zero_heavy_rows(torch_cuda):
 def test_regimes_agree(torch_cuda):
     """Every table layout gives identical counts: full shared-memory table (extended 16-bit / 2x16-bit pairs),
     L2-resident table, shared-memory half table (32-bit for q=13^4 and 293^2, 16+8-bit or 16+1-bit planes for 49^3)."""
-    radix = torch_cuda.eval_scheme == "auto"
+    radix = torch_cuda.eval_scheme in ("auto", "orbit")
     modes = {hec.REGIME_SMEM: 4, hec.REGIME_L2: 7} if radix else {hec.REGIME_SMEM: 1, hec.REGIME_L2: 0}
     h32, h24 = (5, 6) if radix else (2, 3)
     try:
@@ -154,7 +155,7 @@ def test_mixed_layout_launch_groups(torch_cuda, q, g, mode, min_launches):
     to the lower fields' extended tables; 19^4 = 130321: 16+8-bit half table in a launch of its own;
     11^5 = 161051: nothing fits, L2-resident).  Oracle on the fields k <= 3 and on a few rows of k = 4; the
     forced L2 regime must agree on everything."""
-    if torch_cuda.eval_scheme == "auto":        # radix tables: pairs / 32-bit half / 16+1-bit half / global pairs
+    if torch_cuda.eval_scheme in ("auto", "orbit"):        # radix tables: pairs / 32-bit half / 16+1-bit half / global pairs
         mode, min_launches = {(17, 4): (5, 2), (19, 4): (6, 3), (9, 5): (5, 2), (11, 5): (7, 2)}[(q, g)]
     rng = np.random.default_rng(q)
     rows = rng.integers(0, q, size=(70, 2 * g + 3)).astype(np.uint16)
@@ -276,7 +277,7 @@ def test_full_config4_headline(torch_cuda):
     stats = _full_size_checks(torch_cuda, 4, 96)
     assert stats["regime"] == hec.REGIME_SMEM
     # 13^k - 1 = 12, 168, 2196, 28560: R = 4, 8, 4, 8
-    assert stats["radix_fields"] == (0x8484 if torch_cuda.eval_scheme == "auto" else 0)
+    assert stats["radix_fields"] == (0x8484 if torch_cuda.eval_scheme in ("auto", "orbit") else 0)
 
 
 def test_eval_schemes_agree_full_config4(torch_cuda):
@@ -297,12 +298,12 @@ def test_eval_schemes_agree_full_config4(torch_cuda):
 
 def test_full_config5_half_table(torch_cuda):
     stats = _full_size_checks(torch_cuda, 5, 64)
-    assert stats["regime"] == hec.REGIME_SMEM_HALF and stats["table_mode"] == (5 if torch_cuda.eval_scheme == "auto" else 2)
+    assert stats["regime"] == hec.REGIME_SMEM_HALF and stats["table_mode"] == (5 if torch_cuda.eval_scheme in ("auto", "orbit") else 2)
 
 
 def test_full_config3_half_planes(torch_cuda):
     stats = _full_size_checks(torch_cuda, 3, 16)
-    assert stats["regime"] == hec.REGIME_SMEM_HALF and stats["table_mode"] == (6 if torch_cuda.eval_scheme == "auto" else 3)
+    assert stats["regime"] == hec.REGIME_SMEM_HALF and stats["table_mode"] == (6 if torch_cuda.eval_scheme in ("auto", "orbit") else 3)
 
 
 # ------------------------------------------------------------------------------------------ radix split
@@ -365,7 +366,7 @@ def test_table1_single_curve(torch_cuda, p):
     rows = np.array([[c % p for c in TABLE1_CURVE]], dtype=np.uint16)
     cnt, sf = _assert_parity(torch_cuda, p, 2, rows)
     st = hec.last_count_stats()
-    if torch_cuda.eval_scheme == "auto":
+    if torch_cuda.eval_scheme in ("auto", "orbit"):
         assert st["splits"] > 1, st
     # Weil bound for a squarefree genus-2 curve
     if sf[0]:
@@ -388,10 +389,10 @@ def test_small_batches_use_split_mode_and_agree_with_big_batches(torch_cuda, cid
     cfg = W.CONFIGS[cid]
     big = W.generate(cfg, 0, 12000)             # above 2 * 148 * 32 rows: one warp per curve, no atomics
     cnt_big, sf_big = _gpu_count(torch_cuda, cfg.q, cfg.g, big)
-    if torch_cuda.eval_scheme == "auto":
+    if torch_cuda.eval_scheme in ("auto", "orbit"):
         assert hec.last_count_stats()["splits"] == 1
     cnt, sf = _gpu_count(torch_cuda, cfg.q, cfg.g, big[:n])
-    if torch_cuda.eval_scheme == "auto":
+    if torch_cuda.eval_scheme in ("auto", "orbit"):
         assert hec.last_count_stats()["splits"] > 1
     assert (cnt == cnt_big[:n]).all() and (sf == sf_big[:n]).all()
     m = min(n, 4 if cid == 3 else 16)
