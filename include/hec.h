@@ -194,6 +194,9 @@ int hec_curve_map_lambda(uint32_t q, uint32_t g, uint32_t d, uint32_t *out_keys,
 int hec_reduced_total(uint32_t q, uint32_t g, uint32_t d, uint64_t *out_total);
 int hec_reduced_rows(uint32_t q, uint32_t g, uint32_t d, uint64_t first, size_t n, uint16_t *out_coeffs, uint64_t *out_mult);
 int hec_curve_map(uint32_t q, uint32_t g, uint32_t d, uint32_t *out_tuples, uint64_t *out_weights, size_t cap, size_t *out_m);
+/* Algorithm 1 in full (line 2: "for d in {2g+1, 2g+2}"): the merge of the maps of both degrees, N_{g,q}.
+ * With lambda the two degrees stay apart where their types differ (degree 2g+1 carries the extra summand 1). */
+int hec_curve_map_all(uint32_t q, uint32_t g, int with_lambda, uint32_t *out_keys, uint64_t *out_weights, size_t cap, size_t *out_m);
 /* The multi-GPU form: the contribution of the reduced polynomials with index in [first, first + n) --
  * their tuples AND their twists' -- so that the map is the hec_histogram_merge of the ranks' outputs over a partition of
  * [0, hec_reduced_total).  with_lambda != 0: keys have g+1 columns as in hec_curve_map_lambda. */

@@ -238,8 +238,10 @@ int hec_reduced_rows(uint32_t q, uint32_t g, uint32_t d, uint64_t first, size_t 
     return HEC_OK;
 }
 
+// keep_t / keep_w (internal callers): hand the final device buffers over instead of copying them out.
 static int curve_map_impl(uint32_t q, uint32_t g, uint32_t d, bool with_lambda, uint64_t range_first, uint64_t range_n, bool whole,
-                          uint32_t *out_tuples, uint64_t *out_weights, size_t cap, size_t *out_m) {
+                          uint32_t *out_tuples, uint64_t *out_weights, size_t cap, size_t *out_m,
+                          Scratch *keep_t = nullptr, Scratch *keep_w = nullptr) {
     if (!out_m) HEC_FAIL(HEC_ERR_INVALID_ARG, "out_m must not be NULL");
     *out_m = 0;
     if (cap > 0 && (!out_tuples || !out_weights)) HEC_FAIL(HEC_ERR_INVALID_ARG, "out_tuples/out_weights must not be NULL when cap > 0");
@@ -324,6 +326,7 @@ static int curve_map_impl(uint32_t q, uint32_t g, uint32_t d, bool with_lambda, 
     if ((rc = hec_histogram_weighted(static_cast<const uint32_t *>(cat_t.p), nullptr, static_cast<const uint64_t *>(cat_w.p), 2 * acc_m, cols,
                                      static_cast<uint32_t *>(fin_t.p), static_cast<uint64_t *>(fin_w.p), 2 * acc_m, &fin_m))) return rc;
     *out_m = fin_m;
+    if (keep_t && keep_w) { std::swap(keep_t->p, fin_t.p); std::swap(keep_w->p, fin_w.p); return HEC_OK; }
     if (cap < fin_m) HEC_FAIL(HEC_ERR_CAPACITY, "hec_curve_map: cap is smaller than the number of distinct tuples");
     const bool dev = hec_is_device_pointer(out_tuples);
     if (hec_is_device_pointer(out_weights) != dev) HEC_FAIL(HEC_ERR_INVALID_ARG, "out_tuples/out_weights must both be host or both device pointers");
@@ -346,6 +349,46 @@ int hec_curve_map(uint32_t q, uint32_t g, uint32_t d, uint32_t *out_tuples, uint
 
 int hec_curve_map_lambda(uint32_t q, uint32_t g, uint32_t d, uint32_t *out_keys, uint64_t *out_weights, size_t cap, size_t *out_m) {
     return curve_map_impl(q, g, d, true, 0, 0, true, out_keys, out_weights, cap, out_m);
+}
+
+// Algorithm 1 in full (line 2: "for d in {2g+1, 2g+2}"): the maps of both degrees merged.
+int hec_curve_map_all(uint32_t q, uint32_t g, int with_lambda, uint32_t *out_keys, uint64_t *out_weights, size_t cap, size_t *out_m) {
+    if (!out_m) HEC_FAIL(HEC_ERR_INVALID_ARG, "out_m must not be NULL");
+    *out_m = 0;
+    if (cap > 0 && (!out_keys || !out_weights)) HEC_FAIL(HEC_ERR_INVALID_ARG, "out_keys/out_weights must not be NULL when cap > 0");
+    if (g < 1 || g > HEC_MAX_GENUS) HEC_FAIL(HEC_ERR_INVALID_ARG, "g must be in [1, HEC_MAX_GENUS]");
+    const uint32_t cols = with_lambda ? g + 1 : g;
+    int rc;
+    size_t m[2] = {0, 0};
+    Scratch t[2], w[2];
+    for (int s = 0; s < 2; s++) {
+        const uint32_t d = 2 * g + 1 + (uint32_t)s;
+        if ((rc = curve_map_impl(q, g, d, with_lambda != 0, 0, 0, true, nullptr, nullptr, 0, &m[s], &t[s], &w[s]))) return rc;
+    }
+    const size_t total = m[0] + m[1];
+    if (total == 0) return HEC_OK;
+    cudaStream_t st = hec_current_stream();
+    Scratch cat_t, cat_w, fin_t, fin_w;
+    if ((rc = cat_t.alloc(total * cols * 4)) || (rc = cat_w.alloc(total * 8)) || (rc = fin_t.alloc(total * cols * 4)) || (rc = fin_w.alloc(total * 8))) return rc;
+    size_t at = 0;
+    for (int s = 0; s < 2; s++) {
+        if (!m[s]) continue;
+        HEC_CUDA_OK(cudaMemcpyAsync(static_cast<uint32_t *>(cat_t.p) + at * cols, t[s].p, m[s] * cols * 4, cudaMemcpyDeviceToDevice, st));
+        HEC_CUDA_OK(cudaMemcpyAsync(static_cast<uint64_t *>(cat_w.p) + at, w[s].p, m[s] * 8, cudaMemcpyDeviceToDevice, st));
+        at += m[s];
+    }
+    size_t fin_m = 0;
+    if ((rc = hec_histogram_weighted(static_cast<const uint32_t *>(cat_t.p), nullptr, static_cast<const uint64_t *>(cat_w.p), total, cols,
+                                     static_cast<uint32_t *>(fin_t.p), static_cast<uint64_t *>(fin_w.p), total, &fin_m))) return rc;
+    *out_m = fin_m;
+    if (cap < fin_m) HEC_FAIL(HEC_ERR_CAPACITY, "hec_curve_map_all: cap is smaller than the number of distinct keys");
+    const bool dev = hec_is_device_pointer(out_keys);
+    if (hec_is_device_pointer(out_weights) != dev) HEC_FAIL(HEC_ERR_INVALID_ARG, "out_keys/out_weights must both be host or both device pointers");
+    const cudaMemcpyKind kind = dev ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost;
+    HEC_CUDA_OK(cudaMemcpyAsync(out_keys, fin_t.p, fin_m * cols * 4, kind, st));
+    HEC_CUDA_OK(cudaMemcpyAsync(out_weights, fin_w.p, fin_m * 8, kind, st));
+    HEC_CUDA_OK(cudaStreamSynchronize(st));
+    return HEC_OK;
 }
 
 int hec_curve_map_range(uint32_t q, uint32_t g, uint32_t d, uint64_t first, uint64_t n, int with_lambda, uint32_t *out_keys,

@@ -34,7 +34,7 @@ SYMBOLS = [
     "hec_field_degree", "hec_field_q", "hec_field_Q", "hec_field_embed_unit", "hec_field_modulus",
     "hec_field_antilog", "hec_field_log", "hec_field_zech", "hec_field_embed", "hec_count", "hec_histogram",
     "hec_histogram_merge", "hec_reduced_total", "hec_reduced_rows", "hec_curve_map",
-    "hec_count_ex", "hec_lambda_partitions", "hec_curve_map_lambda", "hec_set_map_chunk_rows", "hec_curve_map_range",
+    "hec_count_ex", "hec_lambda_partitions", "hec_curve_map_lambda", "hec_set_map_chunk_rows", "hec_curve_map_range", "hec_curve_map_all",
     "hec_set_stream", "hec_set_regime", "hec_set_eval", "hec_last_count_stats", "hec_launch_count", "hec_gather_bench",
     "hec_shutdown",
 ]
@@ -85,6 +85,7 @@ def lib():
         L.hec_count_ex.argtypes = [u32, u32, vp, sz, vp, vp, vp, vp]
         L.hec_lambda_partitions.argtypes = [u32, vp, sz, ctypes.POINTER(sz)]
         L.hec_set_map_chunk_rows.argtypes = [sz]
+        L.hec_curve_map_all.argtypes = [u32, u32, ctypes.c_int, vp, vp, sz, ctypes.POINTER(sz)]
         L.hec_curve_map_range.argtypes = [u32, u32, u32, ctypes.c_uint64, ctypes.c_uint64, ctypes.c_int, vp, vp, sz, ctypes.POINTER(sz)]
         L.hec_set_stream.argtypes = [vp]
         L.hec_set_regime.argtypes = [ctypes.c_int]
@@ -305,6 +306,21 @@ def curve_map(q: int, g: int, d: int, with_lambda: bool = False, index_range=Non
     w = np.empty((m.value,), dtype=np.uint64)
     if m.value:
         _check(fn(q, g, d, _ptr(tup), _ptr(w), ctypes.c_size_t(m.value), ctypes.byref(m)))
+    return tup[: m.value], w[: m.value]
+
+
+def curve_map_all(q: int, g: int, with_lambda: bool = False):
+    """hec_curve_map_all: both degrees 2g+1 and 2g+2 merged (Algorithm 1 in full)."""
+    L = lib()
+    cols = g + 1 if with_lambda else g
+    m = ctypes.c_size_t(0)
+    rc = L.hec_curve_map_all(q, g, int(with_lambda), None, None, ctypes.c_size_t(0), ctypes.byref(m))
+    if rc not in (HEC_OK, HEC_ERR_CAPACITY):
+        _check(rc)
+    tup = np.empty((m.value, cols), dtype=np.uint32)
+    w = np.empty((m.value,), dtype=np.uint64)
+    if m.value:
+        _check(L.hec_curve_map_all(q, g, int(with_lambda), _ptr(tup), _ptr(w), ctypes.c_size_t(m.value), ctypes.byref(m)))
     return tup[: m.value], w[: m.value]
 
 

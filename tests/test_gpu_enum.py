@@ -145,6 +145,26 @@ def test_curve_map_ranges_merge_to_the_map(cuda, q, g, d, lam):
     assert len(et) == 0 and len(ew) == 0
 
 
+@pytest.mark.parametrize("q,g", [(3, 1), (5, 1), (7, 1), (3, 2), (5, 2)])
+def test_curve_map_all_is_the_union_of_both_degrees(cuda, q, g):
+    """Algorithm 1 line 2: N_{g,q} over d = 2g+1 and 2g+2, against the definition (brute force over both degrees)."""
+    want = {}
+    for d in (2 * g + 1, 2 * g + 2):
+        for t, x in E.brute_force_map(q, g, d).items():
+            want[t] = want.get(t, 0) + x
+    tup, w = hec.curve_map_all(q, g)
+    otup, ow = E.map_to_arrays(want, g)
+    assert tup.shape == otup.shape and (tup == otup).all() and (w == ow).all()
+    keys, wl = hec.curve_map_all(q, g, with_lambda=True)
+    parts = hec.lambda_partitions(g)
+    got = {(tuple(int(v) for v in k[:g]), parts[int(k[g])]): int(x) for k, x in zip(keys, wl)}
+    wantl = {}
+    for d in (2 * g + 1, 2 * g + 2):
+        for key, x in E.brute_force_map_lambda(q, g, d).items():
+            wantl[key] = wantl.get(key, 0) + x
+    assert got == wantl
+
+
 def test_errors(cuda):
     with pytest.raises(hec.HecError) as e:
         hec.reduced_total(7, 2, 4)
