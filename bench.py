@@ -258,7 +258,8 @@ def run_ours(args, cfg):
                                        7: (1, 2 * Mtop, 4)}[mode]
     gather_rate, _ = hec.gather_bench(where, max(ceil_entries, 1024), ceil_bytes, 1024, 1, 4,
                                       8192 if where == 0 else 1024)
-    executed = executed_loads(cfg, rows, stats)         # loads the kernel really issues (radix split: far fewer)
+    rows_eval = hec.shift_rows(q, g, rows) if stats["radix_fields"] else rows      # the rows after hec_count's shift pre-pass
+    executed = executed_loads(cfg, rows_eval, stats)    # loads the kernel really issues (radix split: far fewer)
     if args.eval == "orbit":                            # about 1/k of them per field F_{q^k}: one coset per Frobenius orbit
         executed = None
 

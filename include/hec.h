@@ -264,6 +264,18 @@ typedef struct hec_count_stats {
 } hec_count_stats;
 int hec_last_count_stats(hec_count_stats *out);
 
+/* Shift pre-pass of the radix evaluation (on by default; hec_set_shift(0) turns it off -- tests run both).
+ * N_k(f) = N_k(f(X + t)) for every t in F_q: x -> x + t permutes each F_{q^k}, and the leading coefficient (points at
+ * infinity), the root counts and the factorisation type do not change.  The radix-R evaluation takes its straight-line
+ * network only when every residue class of exponents mod R holds a nonzero coefficient; before counting, hec_count
+ * therefore replaces each row that has an empty class mod R (R = the radix of the largest field, when it is 4 or 8 and the
+ * rows have at least R coefficients) by the first f(X + alpha^s), s = 0 .. 7, without one.  The squarefree flag and lambda
+ * are computed from the original rows.
+ * hec_shift_rows exposes that pre-pass: out_coeffs[n][2g+3] = the rows hec_count evaluates (coeffs itself where no
+ * pre-pass applies); both host or both device pointers. */
+int hec_set_shift(int on);
+int hec_shift_rows(uint32_t q, uint32_t g, const uint16_t *coeffs, size_t n, uint16_t *out_coeffs);
+
 /* Total number of kernels launched by this library since load (bench.py's gpu_launches). */
 uint64_t hec_launch_count(void);
 

@@ -493,6 +493,55 @@ __global__ void __launch_bounds__(256) hec_squarefree_kernel(const HecSquarefree
 }
 
 // --------------------------------------------------------------------------------------------
+// Pre-pass of the radix evaluation (not in the paper): N_k(f) = N_k(f(X + t)) for t in F_q -- x -> x + t permutes every
+// F_{q^k}, the leading coefficient and hence the points at infinity are unchanged, and so are the root counts.  A row
+// with an EMPTY residue class mod R (it would fall back to a smaller radix, hec_radix.cuh) is replaced by the first
+// shift f(X + alpha^s), s = 0, 1, .., that has every class non-empty (Taylor shift by repeated synthetic division, O(d^2)
+// Zech additions in F_q); rows that are fine, invalid, or have no such shift among the first kShiftTries are copied.
+// One thread per curve; the squarefree / lambda kernel keeps reading the original rows.
+// --------------------------------------------------------------------------------------------
+constexpr int kShiftTries = 8;
+
+__global__ void __launch_bounds__(256) hec_shift_kernel(const HecShiftParams P) {
+    const unsigned long long i = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= P.n) return;
+    const FqLog K{P.M, P.zech};
+    const uint32_t ZERO = P.M;
+    const uint16_t *row = P.coeffs + i * P.ncoef;
+    uint16_t *out = P.out + i * P.ncoef;
+    uint32_t c[kSqMaxCoef], a[kSqMaxCoef], b[kSqMaxCoef];
+    uint32_t nz = 0;
+    bool ok = true;
+    int d = -1;
+    for (uint32_t j = 0; j < P.ncoef; j++) {
+        c[j] = row[j];
+        if (c[j] >= P.q) ok = false;
+        if (c[j]) { nz |= 1u << j; d = (int)j; }
+    }
+    auto all_present = [&](uint32_t mask) {
+        uint32_t m = mask;
+        for (uint32_t s = P.R; s < P.ncoef; s += P.R) m |= mask >> s;
+        return (m & ((1u << P.R) - 1u)) == (1u << P.R) - 1u;
+    };
+    bool done = !ok || d < (int)P.ncoef - 2 || d + 1 < (int)P.R || all_present(nz);
+    if (!done) {
+        for (int j = 0; j <= d; j++) a[j] = c[j] ? __ldg(P.emb + c[j]) : ZERO;
+        for (int s = 0; s < kShiftTries && s < (int)P.M && !done; s++) {
+            for (int j = 0; j <= d; j++) b[j] = a[j];
+            for (int lo = 0; lo < d; lo++)                     // f(X + t): d rounds of b_j += t b_{j+1}, j = d-1 .. lo
+                for (int j = d - 1; j >= lo; j--) b[j] = K.add(b[j], K.mul((uint32_t)s, b[j + 1]));
+            uint32_t m = 0;
+            for (int j = 0; j <= d; j++) m |= (b[j] != ZERO ? 1u : 0u) << j;
+            if (all_present(m)) {
+                for (int j = 0; j <= d; j++) c[j] = b[j] == ZERO ? 0u : __ldg(P.antilog + b[j]);
+                done = true;
+            }
+        }
+    }
+    for (uint32_t j = 0; j < P.ncoef; j++) out[j] = (uint16_t)c[j];
+}
+
+// --------------------------------------------------------------------------------------------
 // host side: per-(q, g) device plan
 // --------------------------------------------------------------------------------------------
 struct LaunchPlan {
@@ -512,7 +561,8 @@ struct DevicePlan {
     HecFieldDev f[HEC_MAX_GENUS];
     std::vector<LaunchPlan> launches;
     // squarefree
-    const uint32_t *sq_zech = nullptr, *sq_emb = nullptr;
+    const uint32_t *sq_zech = nullptr, *sq_emb = nullptr, *sq_antilog = nullptr;
+    uint32_t shift_R = 0;             // hec_shift_kernel's target radix (0: no pre-pass for this plan)
     const unsigned long long *d_part_codes = nullptr;   // lambda: packed partitions of 2g+2 in index order
     uint32_t n_parts = 0;
     unsigned long long *d_err = nullptr;
@@ -533,6 +583,10 @@ struct LibState {
     // staging buffers for host-pointer calls
     void *d_stage = nullptr;
     size_t stage_bytes = 0;
+    // rows after the shift pre-pass (hec_shift_kernel)
+    void *d_shift = nullptr;
+    size_t shift_bytes = 0;
+    bool shift_enabled = true;
     int sm_count = 0, smem_optin = 0;
     bool device_ready = false;
 };
@@ -830,6 +884,8 @@ int build_plan(LibState &S, uint32_t q, uint32_t g, int regime, int eval, Device
         for (size_t e = 0; e < parts[t].size(); e++) code |= (unsigned long long)parts[t][e] << (4 * e);
         reinterpret_cast<unsigned long long *>(host.data() + part_off)[t] = code;
     }
+    const size_t sqa_off = reserve((size_t)(q - 1) * 4u);
+    std::copy(fields[0]->antilog.begin(), fields[0]->antilog.end(), reinterpret_cast<uint32_t *>(host.data() + sqa_off));
     const size_t sqz_off = reserve((size_t)(q - 1) * 4u);
     std::copy(fields[0]->zech.begin(), fields[0]->zech.end(), reinterpret_cast<uint32_t *>(host.data() + sqz_off));
 
@@ -857,11 +913,38 @@ int build_plan(LibState &S, uint32_t q, uint32_t g, int regime, int eval, Device
     }
     plan->sq_zech = reinterpret_cast<const uint32_t *>(base + sqz_off);
     plan->sq_emb = plan->f[0].emb;
+    plan->sq_antilog = reinterpret_cast<const uint32_t *>(base + sqa_off);
+    // the shift pre-pass pays where the dominant (largest) field has R >= 4 and the rows have at least R coefficients
+    plan->shift_R = (radix && plan->f[g - 1].radix >= 4u && 2 * g + 2 >= plan->f[g - 1].radix) ? plan->f[g - 1].radix : 0u;
     plan->d_part_codes = reinterpret_cast<const unsigned long long *>(base + part_off);
     plan->n_parts = (uint32_t)parts.size();
 
     *out = plan.get();
     S.plans[key] = std::move(plan);
+    return HEC_OK;
+}
+
+// rows -> rows with every residue class mod plan.shift_R non-empty where a shift achieves it; into `out` or S.d_shift
+int run_shift(LibState &S, const DevicePlan &plan, const uint16_t *d_rows, size_t n, uint16_t *d_out) {
+    const uint32_t ncoef = 2 * plan.g + 3;
+    const size_t bytes = n * ncoef * sizeof(uint16_t);
+    if (!d_out) {
+        if (bytes > S.shift_bytes) {
+            if (S.d_shift) cudaFree(S.d_shift);
+            S.d_shift = nullptr; S.shift_bytes = 0;
+            if (cudaMalloc(&S.d_shift, bytes) != cudaSuccess) { cudaGetLastError(); HEC_FAIL(HEC_ERR_NOMEM, "cannot allocate the shifted-row buffer"); }
+            S.shift_bytes = bytes;
+        }
+        d_out = static_cast<uint16_t *>(S.d_shift);
+    }
+    HecShiftParams H;
+    H.coeffs = d_rows; H.out = d_out; H.n = n; H.q = plan.q; H.M = plan.q - 1; H.ncoef = ncoef;
+    H.R = plan.shift_R ? plan.shift_R : 2u;
+    H.zech = plan.sq_zech; H.emb = plan.sq_emb; H.antilog = plan.sq_antilog;
+    hec_shift_kernel<<<(unsigned)((n + 255) / 256), 256, 0, S.stream>>>(H);
+    hec_launch_counter::value++;
+    S.stats.launches++;
+    HEC_CUDA_OK(cudaGetLastError());
     return HEC_OK;
 }
 
@@ -1070,6 +1153,10 @@ int hec_count_ex(uint32_t q, uint32_t g, const uint16_t *coeffs, size_t n, uint3
                      : (plan->top_mode == HEC_TAB_GLOBAL32 || plan->top_mode == HEC_TAB_GPAIR64) ? HEC_REGIME_L2 : HEC_REGIME_SMEM_HALF;
     S.stats.splits = splits_used;
     HEC_CUDA_OK(cudaEventRecord(S.ev[0], S.stream));
+    if (plan->shift_R && S.shift_enabled) {                    // pre-pass: no empty residue class mod R (hec_shift_kernel)
+        if ((rc = run_shift(S, *plan, d_coeffs, n, nullptr))) return rc;
+        P.coeffs = static_cast<const uint16_t *>(S.d_shift);
+    }
     switch (g) {
         case 1: rc = launch_count<1, 4>(S, *plan, P); break;
         case 2: rc = launch_count<2, 4>(S, *plan, P); break;
@@ -1113,6 +1200,44 @@ int hec_count_ex(uint32_t q, uint32_t g, const uint16_t *coeffs, size_t n, uint3
     return HEC_OK;
 }
 
+int hec_set_shift(int on) {
+    std::lock_guard<std::recursive_mutex> lock(g_state.mu);
+    g_state.shift_enabled = on != 0;
+    return HEC_OK;
+}
+
+int hec_shift_rows(uint32_t q, uint32_t g, const uint16_t *coeffs, size_t n, uint16_t *out_coeffs) {
+    if (g < 1 || g > HEC_MAX_GENUS) HEC_FAIL(HEC_ERR_INVALID_ARG, "g must be in [1, HEC_MAX_GENUS]");
+    if (n == 0) return HEC_OK;
+    if (!coeffs || !out_coeffs) HEC_FAIL(HEC_ERR_INVALID_ARG, "coeffs and out_coeffs must not be NULL");
+    std::lock_guard<std::recursive_mutex> lock(g_state.mu);
+    LibState &S = g_state;
+    int rc = ensure_device(S);
+    if (rc) return rc;
+    const bool dev = is_device_pointer(coeffs);
+    if (is_device_pointer(out_coeffs) != dev) HEC_FAIL(HEC_ERR_INVALID_ARG, "coeffs/out_coeffs must both be host or both device pointers");
+    DevicePlan *plan = nullptr;
+    if ((rc = build_plan(S, q, g, S.regime, S.eval, &plan))) return rc;
+    const size_t bytes = n * (2 * (size_t)g + 3) * sizeof(uint16_t);
+    if (!plan->shift_R) {                                      // no pre-pass for this plan: the rows pass through
+        HEC_CUDA_OK(cudaMemcpyAsync(out_coeffs, coeffs, bytes, cudaMemcpyDefault, S.stream));
+        HEC_CUDA_OK(cudaStreamSynchronize(S.stream));
+        return HEC_OK;
+    }
+    void *d_in = nullptr;
+    if (!dev) {
+        if (cudaMalloc(&d_in, bytes) != cudaSuccess) { cudaGetLastError(); HEC_FAIL(HEC_ERR_NOMEM, "cannot allocate device rows"); }
+        cudaMemcpyAsync(d_in, coeffs, bytes, cudaMemcpyHostToDevice, S.stream);
+    }
+    rc = run_shift(S, *plan, dev ? coeffs : static_cast<const uint16_t *>(d_in), n, dev ? out_coeffs : nullptr);
+    if (rc == HEC_OK && !dev) cudaMemcpyAsync(out_coeffs, S.d_shift, bytes, cudaMemcpyDeviceToHost, S.stream);
+    const cudaError_t ce = cudaStreamSynchronize(S.stream);
+    if (d_in) cudaFree(d_in);
+    if (rc) return rc;
+    if (ce != cudaSuccess) { hec_set_error(HEC_ERR_CUDA, cudaGetErrorString(ce)); return HEC_ERR_CUDA; }
+    return HEC_OK;
+}
+
 int hec_lambda_partitions(uint32_t g, uint8_t *out_parts, size_t cap, size_t *out_count) {
     if (g < 1 || g > HEC_MAX_GENUS) HEC_FAIL(HEC_ERR_INVALID_ARG, "g must be in [1, HEC_MAX_GENUS]");
     if (!out_count) HEC_FAIL(HEC_ERR_INVALID_ARG, "out_count must not be NULL");
@@ -1128,6 +1253,7 @@ void hec_shutdown(void) {
     std::lock_guard<std::recursive_mutex> lock(g_state.mu);
     g_state.plans.clear();
     if (g_state.d_stage) { cudaFree(g_state.d_stage); g_state.d_stage = nullptr; g_state.stage_bytes = 0; }
+    if (g_state.d_shift) { cudaFree(g_state.d_shift); g_state.d_shift = nullptr; g_state.shift_bytes = 0; }
     hec_histogram_release_pool();
     hec_clear_field_cache();
 }

@@ -62,6 +62,19 @@ struct HecCountParams {
     HecFieldDev f[HEC_MAX_GENUS];
 };
 
+// hec_shift_kernel (hec_count.cu): rows whose residue classes mod R are not all non-empty are replaced by f(X + t).
+struct HecShiftParams {
+    const uint16_t *coeffs;        // [n][ncoef]
+    uint16_t *out;                 // [n][ncoef]
+    unsigned long long n;
+    uint32_t q, M;                 // M = q - 1
+    uint32_t ncoef;                // 2g+3
+    uint32_t R;                    // target radix (4 or 8)
+    const uint32_t *zech;          // F_q: M entries, paper's convention (sentinel M)
+    const uint32_t *emb;           // q entries: log in F_q or HEC_LOG_ZERO
+    const uint32_t *antilog;       // M entries: alpha^i in the integer encoding
+};
+
 struct HecSquarefreeParams {
     const uint16_t *coeffs;
     uint8_t *out;

@@ -34,7 +34,7 @@ SYMBOLS = [
     "hec_field_degree", "hec_field_q", "hec_field_Q", "hec_field_embed_unit", "hec_field_modulus",
     "hec_field_antilog", "hec_field_log", "hec_field_zech", "hec_field_embed", "hec_count", "hec_histogram",
     "hec_histogram_merge", "hec_reduced_total", "hec_reduced_rows", "hec_curve_map",
-    "hec_count_ex", "hec_lambda_partitions", "hec_curve_map_lambda", "hec_set_map_chunk_rows", "hec_curve_map_range", "hec_curve_map_all",
+    "hec_count_ex", "hec_lambda_partitions", "hec_curve_map_lambda", "hec_set_map_chunk_rows", "hec_curve_map_range", "hec_curve_map_all", "hec_set_shift", "hec_shift_rows",
     "hec_set_stream", "hec_set_regime", "hec_set_eval", "hec_last_count_stats", "hec_launch_count", "hec_gather_bench",
     "hec_shutdown",
 ]
@@ -85,6 +85,8 @@ def lib():
         L.hec_count_ex.argtypes = [u32, u32, vp, sz, vp, vp, vp, vp]
         L.hec_lambda_partitions.argtypes = [u32, vp, sz, ctypes.POINTER(sz)]
         L.hec_set_map_chunk_rows.argtypes = [sz]
+        L.hec_set_shift.argtypes = [ctypes.c_int]
+        L.hec_shift_rows.argtypes = [u32, u32, vp, sz, vp]
         L.hec_curve_map_all.argtypes = [u32, u32, ctypes.c_int, vp, vp, sz, ctypes.POINTER(sz)]
         L.hec_curve_map_range.argtypes = [u32, u32, u32, ctypes.c_uint64, ctypes.c_uint64, ctypes.c_int, vp, vp, sz, ctypes.POINTER(sz)]
         L.hec_set_stream.argtypes = [vp]
@@ -322,6 +324,23 @@ def curve_map_all(q: int, g: int, with_lambda: bool = False):
     if m.value:
         _check(L.hec_curve_map_all(q, g, int(with_lambda), _ptr(tup), _ptr(w), ctypes.c_size_t(m.value), ctypes.byref(m)))
     return tup[: m.value], w[: m.value]
+
+
+def set_shift(on: bool):
+    _check(lib().hec_set_shift(int(on)))
+
+
+def shift_rows(q: int, g: int, coeffs):
+    """hec_shift_rows: the rows hec_count evaluates after its shift pre-pass (same container type as coeffs)."""
+    n = int(coeffs.shape[0])
+    if _is_torch(coeffs):
+        import torch
+        out = torch.empty_like(coeffs)
+    else:
+        coeffs = np.ascontiguousarray(coeffs, dtype=np.uint16)
+        out = np.empty_like(coeffs)
+    _check(lib().hec_shift_rows(q, g, _ptr(coeffs), n, _ptr(out)))
+    return out
 
 
 def set_map_chunk_rows(rows: int):

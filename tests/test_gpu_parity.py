@@ -406,3 +406,62 @@ def test_split_mode_edge_rows(torch_cuda):
     rows = W.edge_rows(q, g)
     for lo in range(0, len(rows), 9):
         _assert_parity(torch_cuda, q, g, rows[lo:lo + 9])
+
+
+# ------------------------------------------------------------------------------------------ shift pre-pass
+
+def _poly_shift_mod_p(c, t, p):
+    """Coefficients of f(X + t) over F_p (plain Horner-style Taylor shift on Python ints)."""
+    b = [int(v) for v in c]
+    d = len(b) - 1
+    for lo in range(d):
+        for j in range(d - 1, lo - 1, -1):
+            b[j] = (b[j] + t * b[j + 1]) % p
+    return b
+
+
+def test_shift_prepass_rows_are_shifts_and_counts_do_not_change(torch_cuda):
+    """hec_count evaluates f(X + t) instead of f when f has an empty residue class mod R (hec.h: hec_set_shift).
+    The rows it evaluates (hec_shift_rows) must be genuine shifts with every class non-empty, and N_k, r0_k, the flag
+    and lambda must equal those without the pre-pass and the oracle's."""
+    if torch_cuda.eval_scheme == "horner":
+        pytest.skip("the pre-pass belongs to the radix evaluation")
+    cfg = W.CONFIGS[4]
+    q, g = cfg.q, cfg.g
+    rows = np.concatenate([W.generate(cfg, 0, 3000), W.edge_rows(q, g)])
+    out = hec.shift_rows(q, g, rows)
+    dev_out = hec.shift_rows(q, g, _dev(torch_cuda, rows)).cpu().numpy().view(np.uint16)
+    assert (out == dev_out).all()
+    changed = (out != rows).any(axis=1)
+    assert 0.2 < changed[:3000].mean() < 0.45               # about a third of the uniform rows have an empty class mod 8
+    nzm = out != 0
+    present = np.stack([nzm[:, r::8].any(axis=1) for r in range(8)], axis=1).all(axis=1)
+    assert present[:3000].mean() > 0.99
+    for c, o in zip(rows[changed][:400], out[changed][:400]):
+        d = int(np.flatnonzero(c)[-1])
+        assert any(_poly_shift_mod_p(c[:d + 1], t, q) == [int(v) for v in o[:d + 1]] for t in range(1, q)), (c, o)
+        assert (o[d + 1:] == 0).all() and o[d] == c[d]
+    try:
+        hec.set_shift(True)
+        on = [t.cpu().numpy() for t in hec.count_ex(q, g, _dev(torch_cuda, rows))]
+        hec.set_shift(False)
+        off = [t.cpu().numpy() for t in hec.count_ex(q, g, _dev(torch_cuda, rows))]
+    finally:
+        hec.set_shift(True)
+    for a, b in zip(on, off):
+        assert (a == b).all()
+    ocnt, osf, _ = O.count(q, g, rows[:64])
+    assert (on[0].view(np.uint32)[:64] == ocnt).all() and (on[1][:64] == osf).all()
+
+
+@pytest.mark.parametrize("cid", [2, 3, 5])
+def test_shift_prepass_off_agrees(torch_cuda, cid):
+    cfg = W.CONFIGS[cid]
+    rows = W.generate(cfg, 0, 2000)
+    try:
+        hec.set_shift(False)
+        off = _gpu_count(torch_cuda, cfg.q, cfg.g, rows)
+    finally:
+        hec.set_shift(True)
+    on = _gpu_count(torch_cuda, cfg.q, cfg.g, rows)
+    assert (on[0] == off[0]).all() and (on[1] == off[1]).all()
