@@ -165,6 +165,15 @@ def test_curve_map_all_is_the_union_of_both_degrees(cuda, q, g):
     assert got == wantl
 
 
+def test_global_curve_map_single_rank(cuda):
+    """distributed.global_curve_map without a process group is hec_curve_map (the N > 1 exchange is all-gather +
+    hec_histogram_merge, covered by test_curve_map_ranges_merge_to_the_map and the gloo tests)."""
+    from paper_1805_11991_b200 import distributed as D
+    a = D.global_curve_map(5, 2, 6, with_lambda=True)
+    b = hec.curve_map(5, 2, 6, with_lambda=True)
+    assert (a[0] == b[0]).all() and (a[1] == b[1]).all()
+
+
 def test_errors(cuda):
     with pytest.raises(hec.HecError) as e:
         hec.reduced_total(7, 2, 4)
