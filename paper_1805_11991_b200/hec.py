@@ -301,14 +301,20 @@ def curve_map(q: int, g: int, d: int, with_lambda: bool = False, index_range=Non
         fn = L.hec_curve_map_lambda if with_lambda else L.hec_curve_map
     cols = g + 1 if with_lambda else g
     m = ctypes.c_size_t(0)
-    rc = fn(q, g, d, None, None, ctypes.c_size_t(0), ctypes.byref(m))
-    if rc not in (HEC_OK, HEC_ERR_CAPACITY):
-        _check(rc)
-    tup = np.empty((m.value, cols), dtype=np.uint32)
-    w = np.empty((m.value,), dtype=np.uint64)
-    if m.value:
-        _check(fn(q, g, d, _ptr(tup), _ptr(w), ctypes.c_size_t(m.value), ctypes.byref(m)))
-    return tup[: m.value], w[: m.value]
+    # Capacity protocol of hec.h.  Every call does the whole computation, so start with a capacity that is almost
+    # always enough (at most two keys per reduced polynomial) instead of asking for the size first.
+    n_red = index_range[1] if index_range is not None else reduced_total(q, g, d)
+    cap = max(1024, min(2 * n_red, 1 << 24))
+    tup = np.empty((cap, cols), dtype=np.uint32)
+    w = np.empty((cap,), dtype=np.uint64)
+    rc = fn(q, g, d, _ptr(tup), _ptr(w), ctypes.c_size_t(cap), ctypes.byref(m))
+    if rc == HEC_ERR_CAPACITY:
+        cap = m.value
+        tup = np.empty((cap, cols), dtype=np.uint32)
+        w = np.empty((cap,), dtype=np.uint64)
+        rc = fn(q, g, d, _ptr(tup), _ptr(w), ctypes.c_size_t(cap), ctypes.byref(m))
+    _check(rc)
+    return tup[: m.value].copy(), w[: m.value].copy()
 
 
 def curve_map_all(q: int, g: int, with_lambda: bool = False):
@@ -316,14 +322,17 @@ def curve_map_all(q: int, g: int, with_lambda: bool = False):
     L = lib()
     cols = g + 1 if with_lambda else g
     m = ctypes.c_size_t(0)
-    rc = L.hec_curve_map_all(q, g, int(with_lambda), None, None, ctypes.c_size_t(0), ctypes.byref(m))
-    if rc not in (HEC_OK, HEC_ERR_CAPACITY):
-        _check(rc)
-    tup = np.empty((m.value, cols), dtype=np.uint32)
-    w = np.empty((m.value,), dtype=np.uint64)
-    if m.value:
-        _check(L.hec_curve_map_all(q, g, int(with_lambda), _ptr(tup), _ptr(w), ctypes.c_size_t(m.value), ctypes.byref(m)))
-    return tup[: m.value], w[: m.value]
+    cap = max(1024, min(2 * (reduced_total(q, g, 2 * g + 1) + reduced_total(q, g, 2 * g + 2)), 1 << 24))
+    tup = np.empty((cap, cols), dtype=np.uint32)
+    w = np.empty((cap,), dtype=np.uint64)
+    rc = L.hec_curve_map_all(q, g, int(with_lambda), _ptr(tup), _ptr(w), ctypes.c_size_t(cap), ctypes.byref(m))
+    if rc == HEC_ERR_CAPACITY:
+        cap = m.value
+        tup = np.empty((cap, cols), dtype=np.uint32)
+        w = np.empty((cap,), dtype=np.uint64)
+        rc = L.hec_curve_map_all(q, g, int(with_lambda), _ptr(tup), _ptr(w), ctypes.c_size_t(cap), ctypes.byref(m))
+    _check(rc)
+    return tup[: m.value].copy(), w[: m.value].copy()
 
 
 def set_shift(on: bool):
