@@ -111,3 +111,22 @@ def test_reading_g19_is_needed():
             out[E.twist_tuple(q, t)] += m
     assert sum(out.values()) < (q - 1) * (q ** d - q ** (d - 1))
     assert E.reduced_map(q, g, d) == E.brute_force_map(q, g, d)
+
+
+@pytest.mark.parametrize("q,g,d", [(3, 2, 5), (5, 1, 3), (5, 1, 4), (7, 1, 4), (5, 2, 6),
+                                   (3, 1, 3), (3, 2, 6), (5, 2, 5)])         # the last three: p | d (reading G19)
+def test_reduced_map_with_lambda_equals_brute_force(q, g, d):
+    """Full key of (1.2): Algorithm 1 with lambda (lines 18-21) over the reduced
+    polynomials equals the definition over EVERY polynomial of degree d -- the reduction (shift, scaling: PAPER.md:73-121)
+    and the twist n f (reading G8) preserve the factorisation type, in both strata of p | d."""
+    assert E.reduced_map_lambda(q, g, d) == E.brute_force_map_lambda(q, g, d)
+
+
+@pytest.mark.parametrize("q,g,d", [(5, 2, 6), (3, 2, 6), (7, 1, 4)])
+def test_lambda_map_projects_onto_the_map_without_lambda(q, g, d):
+    """Summing the full-key map over lambda gives the map without it (two functions, one Algorithm 1)."""
+    from collections import Counter
+    proj = Counter()
+    for (t, lam), w in E.reduced_map_lambda(q, g, d).items():
+        proj[t] += w
+    assert dict(proj) == E.reduced_map(q, g, d)

@@ -332,6 +332,12 @@ def test_weil_bound_and_parity(q, g, kmax, n):
     cnt, _, _ = O.count(q, g, rows, k_lo=kmax, k_hi=kmax)
     nk = cnt[:, kmax - 1].astype(np.float64)
     assert (np.abs(nk - (q ** kmax + 1)) <= 2 * g * q ** (kmax / 2) + 1e-9).all()
+    # parity: N_k = r0 + 2 r_sq + inf-term, so N_k - r0 - inf-term is even; the infinity term decided
+    # here without the oracle: 1 for odd degree; for even degree 2 or 0, hence irrelevant mod 2
+    r0 = O.roots(q, g, rows, k_hi=kmax)[:, kmax - 1].astype(np.int64)
+    inf = np.where(rows[:, 2 * g + 2] == 0, 1, 0)
+    assert ((cnt[:, kmax - 1].astype(np.int64) - r0 - inf) % 2 == 0).all()
+    assert (r0 <= 2 * g + 2).all()                                           # a nonzero polynomial has at most deg f roots
 
 
 def test_zero_sum_over_constant_term_orbit():
