@@ -261,6 +261,7 @@ typedef struct hec_count_stats {
     uint32_t radix_fields;     /* nibble k-1: radix R used for N_k (0: one Horner chain per x) */
     uint32_t splits;           /* warps per curve: 1 for batches; > 1 when a small batch (down to a single curve) is spread
                                   over the whole GPU, each warp taking a slice of the x range of every field */
+    uint32_t fast_fields;      /* bit k-1: field k carried fast tables (hec_set_fast_tables) */
 } hec_count_stats;
 int hec_last_count_stats(hec_count_stats *out);
 
@@ -275,6 +276,16 @@ int hec_last_count_stats(hec_count_stats *out);
  * pre-pass applies); both host or both device pointers. */
 int hec_set_shift(int on);
 int hec_shift_rows(uint32_t q, uint32_t g, const uint16_t *coeffs, size_t n, uint16_t *out_coeffs);
+
+/* Fast tables of the radix evaluation (on by default; hec_set_fast_tables(0) turns them off -- tests run both, the counts
+ * are identical).  A shared-memory field stored as pairs (Z[n], Z[n + M/2]) also gets, when the launch's shared memory has
+ * room, (i) a copy of Z transposed by residue mod R, T[c][j] = Z[c + R j], which serves the first lookup of every
+ * residue-class chain of Algorithm 1 line 8 -- there lane l reads Z[delta + R (n0 + l)], R words apart in the
+ * plain table (an R-way bank conflict) and consecutive entries of one row of T -- and (ii) e n mod M for the lanes' first
+ * cosets and the step 64 e mod M, e = 0 .. 2g+2, so that the per-curve set-up needs no modular reduction.
+ * hec_count_stats.fast_fields: bit k-1 set iff field k carried them in the last call.  Takes effect on the next plan build
+ * for a (q, g) (the setting is part of the plan key). */
+int hec_set_fast_tables(int on);
 
 /* Total number of kernels launched by this library since load (bench.py's gpu_launches). */
 uint64_t hec_launch_count(void);

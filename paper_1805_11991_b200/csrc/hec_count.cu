@@ -260,6 +260,25 @@ void fill_rhalf17(const hec_field &F, uint32_t M, uint16_t *lo, uint8_t *bits) {
     }
 }
 
+// Fast tables of a PAIR16 field (hec_radix.cuh: radix_fast_x): lanepow[e][lane] = (e lane mod M) | (e (lane + 32) mod M) << 16
+// and stepe[e] = (64 e mod M) in both halves for e = 0 .. D, then the transposed Zech table, R rows of S + 64 16-bit
+// entries, T[c][j] = Z[c + R (j mod S)], S = M / R, each row padded to a multiple of 4 bytes.
+uint32_t fast_row_bytes(uint32_t M, uint32_t R) { return (2u * (M / R + 64u) + 3u) & ~3u; }
+uint32_t fast_head_bytes(uint32_t D) { return (D + 1u) * 128u + (((D + 1u) * 4u + 15u) & ~15u); }
+uint32_t fast_bytes(uint32_t M, uint32_t R, uint32_t D) { return align16(fast_head_bytes(D) + R * fast_row_bytes(M, R)); }
+void fill_fast_tables(const hec_field &F, uint32_t M, uint32_t R, uint32_t D, uint8_t *out) {
+    uint32_t *lanepow = reinterpret_cast<uint32_t *>(out), *stepe = lanepow + (D + 1u) * 32u;
+    for (uint32_t e = 0; e <= D; e++) {
+        for (uint32_t l = 0; l < 32u; l++) lanepow[e * 32u + l] = (e * l) % M | ((e * (l + 32u)) % M) << 16;
+        stepe[e] = ((64u * e) % M) * 0x10001u;
+    }
+    const uint32_t S = M / R, rowB = fast_row_bytes(M, R);
+    for (uint32_t c = 0; c < R; c++) {
+        uint16_t *row = reinterpret_cast<uint16_t *>(out + fast_head_bytes(D) + c * rowB);
+        for (uint32_t j = 0; j < S + 64u; j++) row[j] = (uint16_t)zech0(F, M, c + R * (j % S));
+    }
+}
+
 // Smallest field for which the half-table step is valid: the lane term must stay below h (kernel comment).
 constexpr uint32_t kHalfMinM = 1u << 13;
 constexpr uint32_t kHalf24MaxM = 1u << 22;      // |Z - h| < 127 * 65536
@@ -278,7 +297,7 @@ uint32_t pick_radix(uint32_t M, int eval, int mode, uint32_t g) {
 
 int build_plan(LibState &S, uint32_t q, uint32_t g, int regime, int eval, DevicePlan **out) {
     const bool radix = eval != HEC_EVAL_HORNER;
-    auto key = std::make_tuple(q, g, regime, eval);
+    auto key = std::make_tuple(q, g, regime, eval | (S.fast_enabled ? 0x100 : 0));
     auto it = S.plans.find(key);
     if (it != S.plans.end()) { *out = it->second.get(); return HEC_OK; }
 
@@ -365,14 +384,28 @@ int build_plan(LibState &S, uint32_t q, uint32_t g, int regime, int eval, Device
         bytes[k - 1] = b;
     }
     plan->top_mode = mode[g - 1];
+    // fast tables (radix_fast_x) for the PAIR16 fields, the largest field first, as long as one launch still holds everything
+    std::vector<uint32_t> radix_of(g, 0), fastb(g, 0);
+    for (uint32_t k = 1; k <= g; k++) radix_of[k - 1] = radix ? pick_radix(geom[k - 1].M, eval, mode[k - 1], g) : 0u;
+    if (radix && S.fast_enabled) {
+        uint64_t total = 0;
+        for (uint32_t k = 1; k <= g; k++) total += bytes[k - 1];
+        for (uint32_t k = g; k >= 1; k--) {
+            if (mode[k - 1] != HEC_TAB_PAIR16) continue;
+            const uint32_t fb = fast_bytes(geom[k - 1].M, radix_of[k - 1], D);
+            if (total + fb > budget) continue;
+            total += fb;
+            fastb[k - 1] = fb;
+        }
+    }
     struct Group { uint32_t k_lo, k_hi, smem; };
     std::vector<Group> groups;
     {
         Group cur{1, 0, 0};
         for (uint32_t k = 1; k <= g; k++) {
-            if (cur.k_hi >= cur.k_lo && cur.smem + bytes[k - 1] > budget) { groups.push_back(cur); cur = Group{k, 0, 0}; }
+            if (cur.k_hi >= cur.k_lo && cur.smem + bytes[k - 1] + fastb[k - 1] > budget) { groups.push_back(cur); cur = Group{k, 0, 0}; }
             cur.k_hi = k;
-            cur.smem += bytes[k - 1];
+            cur.smem += bytes[k - 1] + fastb[k - 1];
             if (mode[k - 1] != base_mode) { groups.push_back(cur); cur = Group{k + 1, 0, 0}; }   // only the top of a launch may differ
         }
         if (cur.k_hi >= cur.k_lo) groups.push_back(cur);
@@ -392,7 +425,8 @@ int build_plan(LibState &S, uint32_t q, uint32_t g, int regime, int eval, Device
             fd.M = t.M; fd.mode = (uint32_t)mode[k - 1]; fd.z0 = t.M + t.lmax; fd.rcpM = (uint32_t)((1ull << 32) / t.M);
             fd.lane_cap = std::min<uint32_t>(32u * U, t.M);
             fd.smem_off = so; fd.smem_off2 = 0; fd.gtab = nullptr;
-            fd.radix = radix ? pick_radix(t.M, eval, mode[k - 1], g) : 0u;
+            fd.radix = radix_of[k - 1];
+            fd.fast_off = 0; fd.fast_row = 0;
             uint8_t *dst = host.data() + blob_off[gi] + so;
             switch (mode[k - 1]) {
                 case HEC_TAB_EXT16:
@@ -409,6 +443,11 @@ int build_plan(LibState &S, uint32_t q, uint32_t g, int regime, int eval, Device
                 }
                 case HEC_TAB_PAIR16:
                     fill_pair16(*fields[k - 1], t.M, reinterpret_cast<uint32_t *>(dst));
+                    if (fastb[k - 1]) {
+                        fd.fast_off = so + bytes[k - 1];
+                        fd.fast_row = fast_row_bytes(t.M, fd.radix);
+                        fill_fast_tables(*fields[k - 1], t.M, fd.radix, D, dst + bytes[k - 1]);
+                    }
                     break;
                 case HEC_TAB_RHALF32:
                     fill_rhalf32(*fields[k - 1], t.M, reinterpret_cast<uint32_t *>(dst));
@@ -422,7 +461,7 @@ int build_plan(LibState &S, uint32_t q, uint32_t g, int regime, int eval, Device
                 default:
                     break;
             }
-            so += bytes[k - 1];
+            so += bytes[k - 1] + fastb[k - 1];
         }
     }
     for (uint32_t k = 1; k <= g; k++) {
@@ -736,6 +775,12 @@ int hec_count_ex(uint32_t q, uint32_t g, const uint16_t *coeffs, size_t n, uint3
         hec_set_error(HEC_ERR_DEGREE, "a row has c[2g+2] = c[2g+1] = 0 (degree < 2g+1)", (size_t)err[1]);
         return HEC_ERR_DEGREE;
     }
+    return HEC_OK;
+}
+
+int hec_set_fast_tables(int on) {
+    std::lock_guard<std::recursive_mutex> lock(g_state.mu);
+    g_state.fast_enabled = on != 0;
     return HEC_OK;
 }
 

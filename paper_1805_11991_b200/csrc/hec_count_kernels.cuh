@@ -25,7 +25,10 @@
 #include "hec_device.cuh"
 #include "hec_radix.cuh"
 
-constexpr int kThreads = 1024;        // one CTA per SM, 32 warps, one curve per warp
+#ifndef HEC_THREADS
+#define HEC_THREADS 1024
+#endif
+constexpr int kThreads = HEC_THREADS;  // one CTA per SM, 32 warps, one curve per warp
 constexpr int kWarps = kThreads / 32;
 
 // --------------------------------------------------------------------------------------------
@@ -74,6 +77,7 @@ struct LibState {
     void *d_shift = nullptr;
     size_t shift_bytes = 0;
     bool shift_enabled = true;
+    bool fast_enabled = true;  // fast tables of the PAIR16 fields (radix_fast_x); part of the plan key
     int sm_count = 0, smem_optin = 0;
     bool device_ready = false;
 };
@@ -337,12 +341,22 @@ __global__ void __launch_bounds__(kThreads, 1) hec_count_kernel(const __grid_con
 // mod R' holds a nonzero coefficient runs the straight-line network; the branchy general network is kept only
 // for R = 2 (f even or odd in X, or D + 1 < R').  Measured (profiles/r01c_ncu_full_c4_radix.md): compiling the
 // general network for R = 4, 8 made the loop body overflow the instruction caches (41 % no_instruction stalls).
-template <int D, typename Ar, bool ORBIT, typename Pol>
-__device__ __forceinline__ void radix_dispatch(const HecFieldDev &F, const Pol pol, const uint32_t lane, const uint32_t nz,
-                                               const uint32_t lcj, volatile uint32_t *scratch, const uint32_t part,
+// FAST (PAIR16 fields of the batch kernel): a field that carries fast tables runs radix_fast_x when every class mod its full
+// radix is non-empty, which the shift pre-pass arranges for all but a few rows.
+template <int D, typename Ar, bool ORBIT, bool FAST, typename Pol>
+__device__ __forceinline__ void radix_dispatch(const HecFieldDev &F, const Pol pol, const uint32_t smem_base, const uint32_t lane,
+                                               const uint32_t nz, const uint32_t lcj, volatile uint32_t *scratch, const uint32_t part,
                                                const uint32_t splits, uint32_t &n_sq, uint32_t &n_zero) {
     using namespace hec_radix;
     const uint32_t R = F.radix, M = F.M, rcpM = F.rcpM;
+    if constexpr (FAST) {
+        if (F.fast_off) {
+            const uint32_t ft = smem_base + F.fast_off;
+            if (R == 8) { if (all_classes_present<D, 8>(nz)) { radix_fast_x<D, 8>(pol, ft, F.fast_row, M, lane, nz, lcj, scratch, n_sq, n_zero); return; } }
+            else if (R == 4) { if (all_classes_present<D, 4>(nz)) { radix_fast_x<D, 4>(pol, ft, F.fast_row, M, lane, nz, lcj, scratch, n_sq, n_zero); return; } }
+            else if (all_classes_present<D, 2>(nz)) { radix_fast_x<D, 2>(pol, ft, F.fast_row, M, lane, nz, lcj, scratch, n_sq, n_zero); return; }
+        }
+    }
     if constexpr (ORBIT) {
         if (R >= 8 && all_classes_present<D, 8>(nz)) radix_orbit_x<D, 8, true, Ar>(pol, M, rcpM, lane, nz, lcj, scratch, F.orb[2], F.n_orb[2], n_sq, n_zero);
         else if (R >= 4 && all_classes_present<D, 4>(nz)) radix_orbit_x<D, 4, true, Ar>(pol, M, rcpM, lane, nz, lcj, scratch, F.orb[1], F.n_orb[1], n_sq, n_zero);
@@ -402,16 +416,16 @@ __global__ void __launch_bounds__(kThreads, 1) hec_count_radix_kernel(const __gr
             uint32_t n_zero, n_sq;
             if (TOP == HEC_TAB_PAIR16 || k < P.k_hi) {
                 const hec_radix::PairS16 pol{smem_base + F.smem_off};
-                radix_dispatch<D, hec_radix::ArPacked, ORBIT>(F, pol, lane, nz, lcj, scratch, part, splits, n_sq, n_zero);
+                radix_dispatch<D, hec_radix::ArPacked, ORBIT, !SPLIT && !ORBIT>(F, pol, smem_base, lane, nz, lcj, scratch, part, splits, n_sq, n_zero);
             } else if constexpr (TOP == HEC_TAB_RHALF32) {
                 const hec_radix::HalfS32 pol{smem_base + F.smem_off, smem_base + F.smem_off + 4u * (M >> 1)};
-                radix_dispatch<D, hec_radix::ArScalar, ORBIT>(F, pol, lane, nz, lcj, scratch, part, splits, n_sq, n_zero);
+                radix_dispatch<D, hec_radix::ArScalar, ORBIT, false>(F, pol, smem_base, lane, nz, lcj, scratch, part, splits, n_sq, n_zero);
             } else if constexpr (TOP == HEC_TAB_RHALF17) {
                 const hec_radix::HalfS17 pol{smem_base + F.smem_off, smem_base + F.smem_off + 2u * (M >> 1), smem_base + F.smem_off2};
-                radix_dispatch<D, hec_radix::ArScalar, ORBIT>(F, pol, lane, nz, lcj, scratch, part, splits, n_sq, n_zero);
+                radix_dispatch<D, hec_radix::ArScalar, ORBIT, false>(F, pol, smem_base, lane, nz, lcj, scratch, part, splits, n_sq, n_zero);
             } else if constexpr (TOP == HEC_TAB_GPAIR64) {
                 const hec_radix::PairG64 pol{reinterpret_cast<const uint2 *>(F.gtab)};
-                radix_dispatch<D, hec_radix::ArScalar, ORBIT>(F, pol, lane, nz, lcj, scratch, part, splits, n_sq, n_zero);
+                radix_dispatch<D, hec_radix::ArScalar, ORBIT, false>(F, pol, smem_base, lane, nz, lcj, scratch, part, splits, n_sq, n_zero);
             }
             const uint32_t r0 = __reduce_add_sync(0xffffffffu, n_zero);
             const uint32_t rsq = __reduce_add_sync(0xffffffffu, n_sq);
@@ -476,7 +490,10 @@ int launch_count(LibState &S, const DevicePlan &plan, HecCountParams P) {
         }
         if (rc) return rc;
         if (plan.radix)
-            for (uint32_t k = L.k_lo; k <= L.k_hi; k++) S.stats.radix_fields |= plan.f[k - 1].radix << (4u * (k - 1));
+            for (uint32_t k = L.k_lo; k <= L.k_hi; k++) {
+                S.stats.radix_fields |= plan.f[k - 1].radix << (4u * (k - 1));
+                if (plan.f[k - 1].fast_off && P.splits == 1u && !plan.f[k - 1].orb[0]) S.stats.fast_fields |= 1u << (k - 1);
+            }
     }
     return HEC_OK;
 }

@@ -40,6 +40,8 @@ struct HecFieldDev {
     uint32_t smem_off2;  // HALF24: byte offset of the high plane
     uint32_t lane_cap;   // lanes with lane + 32u >= lane_cap use lane term 0 (they are masked out anyway)
     uint32_t radix;      // radix evaluation: R in {2, 4, 8}, the largest with R | M; 0 for the Horner tables
+    uint32_t fast_off;   // PAIR16: byte offset inside the blob of the field's fast tables (hec_radix.cuh: radix_fast_x), 0: none
+    uint32_t fast_row;   // bytes per row of the transposed Zech table inside them
     const uint32_t *orb[3]; // HEC_EVAL_ORBIT: Frobenius-orbit representatives of the cosets of mu_R, R = 2, 4, 8 (hec_radix.cuh)
     uint32_t n_orb[3];
     const uint32_t *gtab;   // GLOBAL32: extended table in global memory; GPAIR64: the pair table

@@ -467,6 +467,154 @@ __device__ __forceinline__ void radix_all_x(const Pol pol, const uint32_t M, con
 }
 
 // ---------------------------------------------------------------------------------------------------------
+// The batch loop for PAIR16 fields (packed arithmetic, one warp per curve, every coset of the field, every residue
+// class mod R non-empty with R the field's radix): radix_all_x<D, R, true, ArPacked> with three changes, all measured
+// on config 4 (profiles/r01f_ncu_full_c4_radix_first1M.md -> profiles/r02*):
+//  * Chain-start lookups.  The first link of the class-r chain reads Z[delta + R n] (the two top terms of the class
+//    are R apart): lanes hold consecutive n, so in the pair table the 32 addresses are R words apart -- an R-way bank
+//    conflict on every such load (4.04 wavefronts per request against 3.53 for a random gather).  R | M, so
+//    delta + R n = c + R ((a + n) mod S) with c = delta mod R, a = delta div R warp-uniform: a transposed copy of Z,
+//    T[c][j] = Z[c + R (j mod S)] for j < S + 64 (16-bit entries, rows padded by one pass so that a row never wraps
+//    inside a pass), turns them into two conflict-free loads of consecutive entries at a warp-uniform offset.
+//    Links that are not of this kind (later links of a chain, top terms 2R or more apart) keep the pair table.
+//  * Per-curve set-up without modular reductions: e n mod M for the lane's first cosets (n = lane, lane + 32) and the
+//    per-pass step 64 e mod M depend on the field only, so the host tabulates them (lanepow, stepe) for e = 0 .. D.
+//  * Validity of the lane's cosets and the zero queue are only looked at in the last pass or after a zero was seen.
+// Layout of the field's fast tables at shared byte address ft: [lanepow: (D+1) x 32 words][stepe: D+1 words, padded to
+// 16 bytes][T: R rows of rowB bytes]; built by the host (hec_count.cu: fill_fast_tables).
+// ---------------------------------------------------------------------------------------------------------
+template <int D>
+__host__ __device__ constexpr uint32_t fast_tables_head_bytes() { return (uint32_t)(D + 1) * 128u + (((uint32_t)(D + 1) * 4u + 15u) & ~15u); }
+
+template <int D, int R>
+__device__ __forceinline__ void radix_fast_x(const PairS16 pol, const uint32_t ft, const uint32_t rowB, const uint32_t M,
+                                             const uint32_t lane, const uint32_t nz, const uint32_t lcj,
+                                             volatile uint32_t *scratch, uint32_t &n_sq, uint32_t &n_zero) {
+    constexpr int NT = D + 1 > R ? D + 1 - R : 0;
+    constexpr int NTA = NT > 0 ? NT : 1;
+    constexpr uint32_t LG = R == 8 ? 3u : R == 4 ? 2u : 1u;
+    const ArPacked ar(M);
+    const uint32_t S = M >> LG, unit = S;
+    const uint32_t tLP = ft + 4u * lane, tSE = ft + (uint32_t)(D + 1) * 128u, tT = ft + fast_tables_head_bytes<D>() + 2u * lane;
+
+    __syncwarp();
+    if (lane <= (uint32_t)D) scratch[lane] = lcj;
+    __syncwarp();
+
+    // ---- per-curve structure (warp-uniform masks; per-lane offsets from the field's tables)
+    // link i (a nonzero term that continues the chain of its class):
+    //   ct bit i: transposed kind, ca[i] = byte offset 2 ((a + base) mod S) (uniform), cb[i] = T + row c + 2 lane
+    //   cm bit i: pair-table kind, ca[i] = packed index offsets of the lane's two cosets, cb[i] = their step per pass
+    uint32_t ca[NTA], cb[NTA], kc[R], kinc[R];
+    uint32_t cm = 0, ct = 0, present = 0, linked = 0;
+    uint32_t last_lc[R], last_e[R];
+#pragma unroll
+    for (int r = 0; r < R; r++) { last_lc[r] = 0; last_e[r] = 0; }
+#pragma unroll
+    for (int i = D; i >= 0; i--) {
+        const int r = i % R;
+        const uint32_t lci = __shfl_sync(0xffffffffu, lcj, i);
+        if (i < NT) { ca[i] = 0; cb[i] = 0; }
+        if (nz & (1u << i)) {
+            if (i < NT && (present & (1u << r))) {
+                const uint32_t m = last_e[r] - (uint32_t)i;
+                const uint32_t delta = last_lc[r] >= lci ? last_lc[r] - lci : last_lc[r] + M - lci;
+                if (m == (uint32_t)R && !(linked & (1u << r))) {
+                    ca[i] = 2u * (delta >> LG);
+                    cb[i] = tT + (delta & (uint32_t)(R - 1)) * rowB;
+                    ct |= 1u << i;
+                } else {
+                    ca[i] = ar.wrap(ar.rep(delta) + lds_u32(tLP + m * 128u));
+                    cb[i] = lds_u32(tSE + 4u * m);
+                    cm |= 1u << i;
+                }
+                linked |= 1u << r;
+            }
+            present |= 1u << r;
+            last_lc[r] = lci;
+            last_e[r] = (uint32_t)i;
+        }
+    }
+#pragma unroll
+    for (int r = 0; r < R; r++) {                      // log G_r = W_r + K_r(n), K_r(n) = log c_{e_T} + e_T n
+        kc[r] = ar.wrap(ar.rep(last_lc[r]) + lds_u32(tLP + last_e[r] * 128u));
+        kinc[r] = lds_u32(tSE + 4u * last_e[r]);
+    }
+
+    uint32_t acc = 0, pushed = 0, qn = 0, nz_exact = 0, odd_exact = 0;
+    auto drain = [&]() {
+        for (uint32_t j = lane; j < qn; j += 32u) {
+            const uint32_t res = exact_coset<D, R>(pol, M, nz, scratch, scratch[16 + j]);
+            nz_exact += res >> 16;
+            odd_exact += res & 0xFFFFu;
+        }
+    };
+    const uint32_t twoS = 2u * S;
+    for (uint32_t base = 0; base < S; base += 64u) {
+        uint32_t v[R];
+        uint32_t mn = ar.mn_init();
+#pragma unroll
+        for (int r = 0; r < R; r++) {
+            uint32_t w = 0;
+            bool chained = false;
+#pragma unroll
+            for (int i = NT - 1; i >= 0; i--) {
+                if (i % R != r) continue;
+                if (ct & (1u << i)) {                  // always the first link of its chain
+                    const uint32_t a0 = cb[i] + ca[i];
+                    const uint32_t z0 = lds_u16(a0), z1 = lds_u16(a0 + 64u);
+                    w = __byte_perm(z0, z1, 0x5410);
+                    mn = __vminu2(mn, w);
+                    const uint32_t nx = ca[i] + 128u;
+                    ca[i] = min(nx, nx - twoS);
+                    chained = true;
+                } else if (cm & (1u << i)) {
+                    const uint32_t n = chained ? ar.wrap(w + ca[i]) : ca[i];
+                    w = ar.lookup_single(pol, n, mn);
+                    ca[i] = ar.wrap(ca[i] + cb[i]);
+                    chained = true;
+                }
+            }
+            v[r] = chained ? ar.wrap(w + kc[r]) : kc[r];
+            kc[r] = ar.wrap(kc[r] + kinc[r]);
+        }
+        uint32_t ps = 0;
+        network<R, true>(ar, pol, unit, present, v, ps, mn);
+        const bool z0 = (mn & 0xFFFFu) == 0u, z1 = (mn >> 16) == 0u;
+        if (__any_sync(0xffffffffu, z0 || z1) || base + 64u > S) {       // rare: a zero somewhere, or the ragged last pass
+            const bool valid0 = base + lane < S, valid1 = base + lane + 32u < S;
+            const bool flag0 = valid0 && z0, flag1 = valid1 && z1;
+            if (__any_sync(0xffffffffu, flag0 || flag1)) {               // queue the flagged cosets for exact evaluation
+                uint32_t bal = __ballot_sync(0xffffffffu, flag0);
+                if (flag0) { scratch[16 + qn + __popc(bal & ((1u << lane) - 1u))] = base + lane; pushed++; }
+                qn += __popc(bal);
+                bal = __ballot_sync(0xffffffffu, flag1);
+                if (flag1) { scratch[16 + qn + __popc(bal & ((1u << lane) - 1u))] = base + lane + 32u; pushed++; }
+                qn += __popc(bal);
+                __syncwarp();
+                if (qn >= 32u) {
+                    drain();
+                    qn = 0;
+                    __syncwarp();
+                }
+            }
+            ps = ar.keep(ps, valid0 && !flag0, valid1 && !flag1);
+        }
+        acc += ps;                                     // <= R per half and pass, at most S / 64 + 1 <= 257 passes: no carry
+    }
+    const uint32_t odd_fast = ar.total(acc);
+    drain();
+    __syncwarp();
+    uint32_t n_valid = 0;                              // cosets of this lane
+    if (lane < S) n_valid += (S - lane + 63u) / 64u;
+    if (lane + 32u < S) n_valid += (S - lane - 32u + 63u) / 64u;
+    const uint32_t n_nz = (n_valid - pushed) * R + nz_exact;            // every value of an unflagged coset is nonzero
+    const uint32_t n_odd = odd_fast + odd_exact;
+    n_zero = n_valid * R - n_nz;
+    n_sq = n_nz - n_odd;
+}
+
+// ---------------------------------------------------------------------------------------------------------
 // The same, over ONE representative per Frobenius orbit of cosets (HEC_EVAL_ORBIT; not in the
 // paper).  f has coefficients in F_q, so f(x^q) = f(x)^q: x and x^q give values that vanish together and are squares
 // together.  On logs x -> x^q is n -> q n mod M; it permutes the cosets of mu_R (q is odd, R a power of two), acting on
