@@ -352,22 +352,25 @@ __device__ __forceinline__ void radix_dispatch(const HecFieldDev &F, const Pol p
     if constexpr (FAST) {
         if (F.fast_off) {
             const uint32_t ft = smem_base + F.fast_off;
-            if (R == 8) { if (all_classes_present<D, 8>(nz)) { radix_fast_x<D, 8>(pol, ft, F.fast_row, M, lane, nz, lcj, scratch, n_sq, n_zero); return; } }
-            else if (R == 4) { if (all_classes_present<D, 4>(nz)) { radix_fast_x<D, 4>(pol, ft, F.fast_row, M, lane, nz, lcj, scratch, n_sq, n_zero); return; } }
-            else if (all_classes_present<D, 2>(nz)) { radix_fast_x<D, 2>(pol, ft, F.fast_row, M, lane, nz, lcj, scratch, n_sq, n_zero); return; }
+            if (R == 8) { if (all_classes_present<D, 8>(nz)) { const uint2 res = radix_fast_x<D, 8>(pol, ft, F.fast_row, M, lane, nz, lcj, scratch); n_sq = res.x; n_zero = res.y; return; } }
+            else if (R == 4) { if (all_classes_present<D, 4>(nz)) { const uint2 res = radix_fast_x<D, 4>(pol, ft, F.fast_row, M, lane, nz, lcj, scratch); n_sq = res.x; n_zero = res.y; return; } }
+            else if (all_classes_present<D, 2>(nz)) { const uint2 res = radix_fast_x<D, 2>(pol, ft, F.fast_row, M, lane, nz, lcj, scratch); n_sq = res.x; n_zero = res.y; return; }
         }
     }
+    uint2 res;
     if constexpr (ORBIT) {
-        if (R >= 8 && all_classes_present<D, 8>(nz)) radix_orbit_x<D, 8, true, Ar>(pol, M, rcpM, lane, nz, lcj, scratch, F.orb[2], F.n_orb[2], n_sq, n_zero);
-        else if (R >= 4 && all_classes_present<D, 4>(nz)) radix_orbit_x<D, 4, true, Ar>(pol, M, rcpM, lane, nz, lcj, scratch, F.orb[1], F.n_orb[1], n_sq, n_zero);
-        else if (all_classes_present<D, 2>(nz)) radix_orbit_x<D, 2, true, Ar>(pol, M, rcpM, lane, nz, lcj, scratch, F.orb[0], F.n_orb[0], n_sq, n_zero);
-        else radix_orbit_x<D, 2, false, Ar>(pol, M, rcpM, lane, nz, lcj, scratch, F.orb[0], F.n_orb[0], n_sq, n_zero);
+        if (R >= 8 && all_classes_present<D, 8>(nz)) res = radix_orbit_x<D, 8, true, Ar>(pol, M, rcpM, lane, nz, lcj, scratch, F.orb[2], F.n_orb[2]);
+        else if (R >= 4 && all_classes_present<D, 4>(nz)) res = radix_orbit_x<D, 4, true, Ar>(pol, M, rcpM, lane, nz, lcj, scratch, F.orb[1], F.n_orb[1]);
+        else if (all_classes_present<D, 2>(nz)) res = radix_orbit_x<D, 2, true, Ar>(pol, M, rcpM, lane, nz, lcj, scratch, F.orb[0], F.n_orb[0]);
+        else res = radix_orbit_x<D, 2, false, Ar>(pol, M, rcpM, lane, nz, lcj, scratch, F.orb[0], F.n_orb[0]);
     } else {
-        if (R >= 8 && all_classes_present<D, 8>(nz)) radix_all_x<D, 8, true, Ar>(pol, M, rcpM, lane, nz, lcj, scratch, part, splits, n_sq, n_zero);
-        else if (R >= 4 && all_classes_present<D, 4>(nz)) radix_all_x<D, 4, true, Ar>(pol, M, rcpM, lane, nz, lcj, scratch, part, splits, n_sq, n_zero);
-        else if (all_classes_present<D, 2>(nz)) radix_all_x<D, 2, true, Ar>(pol, M, rcpM, lane, nz, lcj, scratch, part, splits, n_sq, n_zero);
-        else radix_all_x<D, 2, false, Ar>(pol, M, rcpM, lane, nz, lcj, scratch, part, splits, n_sq, n_zero);
+        if (R >= 8 && all_classes_present<D, 8>(nz)) res = radix_all_x<D, 8, true, Ar>(pol, M, rcpM, lane, nz, lcj, scratch, part, splits);
+        else if (R >= 4 && all_classes_present<D, 4>(nz)) res = radix_all_x<D, 4, true, Ar>(pol, M, rcpM, lane, nz, lcj, scratch, part, splits);
+        else if (all_classes_present<D, 2>(nz)) res = radix_all_x<D, 2, true, Ar>(pol, M, rcpM, lane, nz, lcj, scratch, part, splits);
+        else res = radix_all_x<D, 2, false, Ar>(pol, M, rcpM, lane, nz, lcj, scratch, part, splits);
     }
+    n_sq = res.x;
+    n_zero = res.y;
 }
 
 // SPLIT = false: one warp per curve (batches; P.splits == 1).  SPLIT = true: a separate instantiation for small batches,

@@ -256,6 +256,42 @@ __device__ __noinline__ uint32_t exact_coset(const Pol pol, const uint32_t M, co
 }
 
 // ---------------------------------------------------------------------------------------------------------
+// Exact evaluation of the queued cosets, one POINT per lane (radix_all_x / radix_fast_x; the orbit scheme keeps
+// exact_coset for its weights).  Each group of R lanes takes one queued coset n and lane j of the group evaluates f at
+// x = zeta^j alpha^n by the plain Horner rule of Algorithm 1 line 8 in Zech form with the zero element
+// handled explicitly: 32 / R cosets per round with every lane busy, where exact_coset walked the
+// whole butterfly network in one lane per coset (measured on config 4: 10 % of all issued instructions, with
+// 3 of 32 lanes active).  Adds to this lane's nz_exact / odd_exact (the caller sums over the warp anyway).
+// ---------------------------------------------------------------------------------------------------------
+template <int D, int R, typename Pol>
+__device__ __noinline__ void exact_queue(const Pol pol, const uint32_t M, const uint32_t nz, const volatile uint32_t *sc,
+                                         const uint32_t qn, const uint32_t lane, uint32_t &nz_exact, uint32_t &odd_exact) {
+    constexpr uint32_t LG = R == 8 ? 3u : R == 4 ? 2u : 1u;
+    const uint32_t h = M >> 1, S = M >> LG;
+    auto wrap = [M](uint32_t x) { return min(x, x - M); };
+    const uint32_t j = lane & (uint32_t)(R - 1), slot = lane >> LG;
+    for (uint32_t q0 = 0; q0 < qn; q0 += 32u / R) {
+        if (q0 + slot >= qn) continue;
+        const uint32_t lx = sc[16 + q0 + slot] + j * S;                    // log x < M
+        uint32_t acc = kZero;
+#pragma unroll 1
+        for (int i = D; i >= 0; i--) {
+            if (acc < M) acc = wrap(acc + lx);                             // acc * x
+            if ((nz >> i) & 1u) {                                          // acc + c_i
+                const uint32_t b = sc[i];
+                if (acc >= M) {
+                    acc = b;
+                } else {
+                    const uint32_t dd = wrap(b + M - acc);
+                    acc = dd == h ? kZero : wrap(acc + pol.single(dd, M, h));
+                }
+            }
+        }
+        if (acc < M) { nz_exact++; odd_exact += acc & 1u; }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------------
 // The butterfly network of the fast path on LANES cosets at once.  present: bit r set iff G_r is not
 // identically zero (warp-uniform; some G_r is present because the leading coefficient is nonzero, so no final
 // value is identically zero).  Adds to ps the number of odd logs among the values (per lane of V) and folds the
@@ -324,10 +360,12 @@ __device__ __forceinline__ bool all_classes_present(const uint32_t nz) {
 // ALL: the caller guarantees that every residue class mod R holds a nonzero coefficient (the straight-line
 // network); otherwise the network takes warp-uniform branches around the absent classes.
 // ---------------------------------------------------------------------------------------------------------
+// Not inlined (as radix_fast_x): the loop wants all 64 registers; the kernel's per-curve state is saved around the call.
 template <int D, int R, bool ALL, typename Ar, typename Pol>
-__device__ __forceinline__ void radix_all_x(const Pol pol, const uint32_t M, const uint32_t rcpM, const uint32_t lane,
-                                            const uint32_t nz, const uint32_t lcj, volatile uint32_t *scratch,
-                                            const uint32_t part, const uint32_t splits, uint32_t &n_sq, uint32_t &n_zero) {
+__device__ __noinline__ uint2 radix_all_x(const Pol pol, const uint32_t M, const uint32_t rcpM, const uint32_t lane,
+                                          const uint32_t nz, const uint32_t lcj, volatile uint32_t *scratch,
+                                          const uint32_t part, const uint32_t splits) {
+    uint32_t n_sq, n_zero;
     constexpr int L = Ar::LANES;
     constexpr int NT = D + 1 > R ? D + 1 - R : 0;      // terms 0 .. NT-1 can continue a chain
     constexpr int NTA = NT > 0 ? NT : 1;
@@ -345,9 +383,7 @@ __device__ __forceinline__ void radix_all_x(const Pol pol, const uint32_t M, con
         c_lo = min(S, part * chunk);
         c_hi = min(S, c_lo + chunk);
     }
-    n_sq = 0;
-    n_zero = 0;
-    if (c_lo >= c_hi) return;                          // warp-uniform
+    if (c_lo >= c_hi) return make_uint2(0u, 0u);       // warp-uniform
 
     __syncwarp();
     if (lane <= (uint32_t)D) scratch[lane] = lcj;
@@ -394,13 +430,7 @@ __device__ __forceinline__ void radix_all_x(const Pol pol, const uint32_t M, con
     }
 
     uint32_t acc = 0, odd_fast = 0, passes = 0, pushed = 0, qn = 0, nz_exact = 0, odd_exact = 0;
-    auto drain = [&]() {
-        for (uint32_t j = lane; j < qn; j += 32u) {
-            const uint32_t res = exact_coset<D, R>(pol, M, nz, scratch, scratch[16 + j]);
-            nz_exact += res >> 16;
-            odd_exact += res & 0xFFFFu;
-        }
-    };
+    auto drain = [&]() { exact_queue<D, R>(pol, M, nz, scratch, qn, lane, nz_exact, odd_exact); };
     for (uint32_t base = c_lo; base < c_hi; base += 32u * L) {
         uint32_t v[R];
         uint32_t mn = ar.mn_init();
@@ -464,6 +494,7 @@ __device__ __forceinline__ void radix_all_x(const Pol pol, const uint32_t M, con
     const uint32_t n_odd = odd_fast + odd_exact;
     n_zero = n_valid * R - n_nz;
     n_sq = n_nz - n_odd;
+    return make_uint2(n_sq, n_zero);
 }
 
 // ---------------------------------------------------------------------------------------------------------
@@ -486,10 +517,14 @@ __device__ __forceinline__ void radix_all_x(const Pol pol, const uint32_t M, con
 template <int D>
 __host__ __device__ constexpr uint32_t fast_tables_head_bytes() { return (uint32_t)(D + 1) * 128u + (((uint32_t)(D + 1) * 4u + 15u) & ~15u); }
 
+// Not inlined on purpose: the loop needs every one of the 64 registers a thread of a 1024-thread CTA can have (8 values,
+// 8 + 8 class offsets and steps, the chain state); as a function of its own the kernel's per-curve state is saved around
+// the call once per field instead of competing with the loop (inlined, ptxas re-derived constants inside the loop).
 template <int D, int R>
-__device__ __forceinline__ void radix_fast_x(const PairS16 pol, const uint32_t ft, const uint32_t rowB, const uint32_t M,
-                                             const uint32_t lane, const uint32_t nz, const uint32_t lcj,
-                                             volatile uint32_t *scratch, uint32_t &n_sq, uint32_t &n_zero) {
+__device__ __noinline__ uint2 radix_fast_x(const PairS16 pol, const uint32_t ft, const uint32_t rowB, const uint32_t M,
+                                           const uint32_t lane, const uint32_t nz, const uint32_t lcj,
+                                           volatile uint32_t *scratch) {
+    uint32_t n_sq, n_zero;
     constexpr int NT = D + 1 > R ? D + 1 - R : 0;
     constexpr int NTA = NT > 0 ? NT : 1;
     constexpr uint32_t LG = R == 8 ? 3u : R == 4 ? 2u : 1u;
@@ -542,13 +577,7 @@ __device__ __forceinline__ void radix_fast_x(const PairS16 pol, const uint32_t f
     }
 
     uint32_t acc = 0, pushed = 0, qn = 0, nz_exact = 0, odd_exact = 0;
-    auto drain = [&]() {
-        for (uint32_t j = lane; j < qn; j += 32u) {
-            const uint32_t res = exact_coset<D, R>(pol, M, nz, scratch, scratch[16 + j]);
-            nz_exact += res >> 16;
-            odd_exact += res & 0xFFFFu;
-        }
-    };
+    auto drain = [&]() { exact_queue<D, R>(pol, M, nz, scratch, qn, lane, nz_exact, odd_exact); };
     const uint32_t twoS = 2u * S;
     for (uint32_t base = 0; base < S; base += 64u) {
         uint32_t v[R];
@@ -560,6 +589,8 @@ __device__ __forceinline__ void radix_fast_x(const PairS16 pol, const uint32_t f
 #pragma unroll
             for (int i = NT - 1; i >= 0; i--) {
                 if (i % R != r) continue;
+                // a term with no second term of its class above it (i + 2R > D) can only be a first link, R below the top term
+                const bool only_t = i + 2 * R > D;
                 if (ct & (1u << i)) {                  // always the first link of its chain
                     const uint32_t a0 = cb[i] + ca[i];
                     const uint32_t z0 = lds_u16(a0), z1 = lds_u16(a0 + 64u);
@@ -568,7 +599,7 @@ __device__ __forceinline__ void radix_fast_x(const PairS16 pol, const uint32_t f
                     const uint32_t nx = ca[i] + 128u;
                     ca[i] = min(nx, nx - twoS);
                     chained = true;
-                } else if (cm & (1u << i)) {
+                } else if (!only_t && (cm & (1u << i))) {
                     const uint32_t n = chained ? ar.wrap(w + ca[i]) : ca[i];
                     w = ar.lookup_single(pol, n, mn);
                     ca[i] = ar.wrap(ca[i] + cb[i]);
@@ -580,8 +611,9 @@ __device__ __forceinline__ void radix_fast_x(const PairS16 pol, const uint32_t f
         }
         uint32_t ps = 0;
         network<R, true>(ar, pol, unit, present, v, ps, mn);
-        const bool z0 = (mn & 0xFFFFu) == 0u, z1 = (mn >> 16) == 0u;
-        if (__any_sync(0xffffffffu, z0 || z1) || base + 64u > S) {       // rare: a zero somewhere, or the ragged last pass
+        const bool zany = ((mn - 0x10001u) & ~mn & 0x80008000u) != 0u;   // some half of mn is 0 (halves are < 2^15 or 0xFFFF)
+        if (__any_sync(0xffffffffu, zany) || base + 64u > S) {           // rare: a zero somewhere, or the ragged last pass
+            const bool z0 = (mn & 0xFFFFu) == 0u, z1 = (mn >> 16) == 0u;
             const bool valid0 = base + lane < S, valid1 = base + lane + 32u < S;
             const bool flag0 = valid0 && z0, flag1 = valid1 && z1;
             if (__any_sync(0xffffffffu, flag0 || flag1)) {               // queue the flagged cosets for exact evaluation
@@ -612,6 +644,7 @@ __device__ __forceinline__ void radix_fast_x(const PairS16 pol, const uint32_t f
     const uint32_t n_odd = odd_fast + odd_exact;
     n_zero = n_valid * R - n_nz;
     n_sq = n_nz - n_odd;
+    return make_uint2(n_sq, n_zero);
 }
 
 // ---------------------------------------------------------------------------------------------------------
@@ -625,10 +658,10 @@ __device__ __forceinline__ void radix_fast_x(const PairS16 pol, const uint32_t f
 // (delta + m n) mod M, one multiply-high reduction per term and coset.
 // ---------------------------------------------------------------------------------------------------------
 template <int D, int R, bool ALL, typename Ar, typename Pol>
-__device__ __forceinline__ void radix_orbit_x(const Pol pol, const uint32_t M, const uint32_t rcpM, const uint32_t lane,
-                                              const uint32_t nz, const uint32_t lcj, volatile uint32_t *scratch,
-                                              const uint32_t *__restrict__ reps, const uint32_t n_reps,
-                                              uint32_t &n_sq, uint32_t &n_zero) {
+__device__ __noinline__ uint2 radix_orbit_x(const Pol pol, const uint32_t M, const uint32_t rcpM, const uint32_t lane,
+                                            const uint32_t nz, const uint32_t lcj, volatile uint32_t *scratch,
+                                            const uint32_t *__restrict__ reps, const uint32_t n_reps) {
+    uint32_t n_sq, n_zero;
     constexpr int L = Ar::LANES;
     constexpr int NT = D + 1 > R ? D + 1 - R : 0;
     constexpr int NTA = NT > 0 ? NT : 1;
@@ -638,9 +671,7 @@ __device__ __forceinline__ void radix_orbit_x(const Pol pol, const uint32_t M, c
         const uint32_t r = x - __umulhi(x, rcpM) * M;
         return r >= M ? r - M : r;
     };
-    n_sq = 0;
-    n_zero = 0;
-    if (n_reps == 0u) return;
+    if (n_reps == 0u) return make_uint2(0u, 0u);
 
     __syncwarp();
     if (lane <= (uint32_t)D) scratch[lane] = lcj;
@@ -748,6 +779,7 @@ __device__ __forceinline__ void radix_orbit_x(const Pol pol, const uint32_t M, c
     const uint32_t n_nz = w_ok * R + nz_exact;          // every value of an unflagged coset is nonzero
     n_zero = w_flagged * R - nz_exact;
     n_sq = n_nz - (odd_fast + odd_exact);
+    return make_uint2(n_sq, n_zero);
 }
 
 }  // namespace hec_radix
