@@ -20,6 +20,7 @@
 #include <memory>
 #include <mutex>
 #include <tuple>
+#include <type_traits>
 #include <vector>
 
 #include "hec_device.cuh"
@@ -30,6 +31,7 @@
 #endif
 constexpr int kThreads = HEC_THREADS;  // one CTA per SM, 32 warps, one curve per warp
 constexpr int kWarps = kThreads / 32;
+constexpr uint32_t kDirectMaxM = 64;   // fields with at most this many nonzero elements skip the coset split (hec_radix.cuh: direct_all_x)
 
 // --------------------------------------------------------------------------------------------
 // host side: per-(q, g) device plan and the library state (one per process and device, hec.h)
@@ -349,6 +351,14 @@ __device__ __forceinline__ void radix_dispatch(const HecFieldDev &F, const Pol p
                                                const uint32_t splits, uint32_t &n_sq, uint32_t &n_zero) {
     using namespace hec_radix;
     const uint32_t R = F.radix, M = F.M, rcpM = F.rcpM;
+    if constexpr (!ORBIT && std::is_same<Pol, PairS16>::value) {
+        if (M <= kDirectMaxM) {                       // tiny field: every point directly (splits: part 0 takes them all)
+            uint2 res = make_uint2(0u, 0u);
+            if (part == 0u) res = direct_all_x<D>(pol, M, lane, nz, lcj, scratch);
+            n_sq = res.x; n_zero = res.y;
+            return;
+        }
+    }
     if constexpr (FAST) {
         if (F.fast_off) {
             const uint32_t ft = smem_base + F.fast_off;

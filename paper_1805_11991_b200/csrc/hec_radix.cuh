@@ -263,32 +263,63 @@ __device__ __noinline__ uint32_t exact_coset(const Pol pol, const uint32_t M, co
 // whole butterfly network in one lane per coset (measured on config 4: 10 % of all issued instructions, with
 // 3 of 32 lanes active).  Adds to this lane's nz_exact / odd_exact (the caller sums over the warp anyway).
 // ---------------------------------------------------------------------------------------------------------
+// f(x) at ONE point x = alpha^lx, lx < M, by the Horner rule in Zech form; returns the log of the value or kZero.
+// Straight-line: the term tests are warp-uniform, the zero element is carried as a predicate.
+template <int D, typename Pol>
+__device__ __forceinline__ uint32_t horner_point(const Pol &pol, const uint32_t M, const uint32_t nz, const volatile uint32_t *sc,
+                                                 const uint32_t lx) {
+    const uint32_t h = M >> 1;
+    auto wrap = [M](uint32_t x) { return min(x, x - M); };
+    uint32_t acc = 0;
+    bool zero = true;
+#pragma unroll
+    for (int i = D; i >= 0; i--) {
+        acc = wrap(acc + lx);                                              // acc * x (kept in range also while zero)
+        if ((nz >> i) & 1u) {                                              // acc + c_i
+            const uint32_t b = sc[i];
+            const uint32_t dd = wrap(b + M - acc);
+            const uint32_t s = wrap(acc + pol.single(dd, M, h));
+            const bool cancel = !zero && dd == h;
+            acc = zero ? b : s;
+            zero = cancel;
+        }
+    }
+    return zero ? kZero : acc;
+}
+
 template <int D, int R, typename Pol>
 __device__ __noinline__ void exact_queue(const Pol pol, const uint32_t M, const uint32_t nz, const volatile uint32_t *sc,
                                          const uint32_t qn, const uint32_t lane, uint32_t &nz_exact, uint32_t &odd_exact) {
     constexpr uint32_t LG = R == 8 ? 3u : R == 4 ? 2u : 1u;
-    const uint32_t h = M >> 1, S = M >> LG;
-    auto wrap = [M](uint32_t x) { return min(x, x - M); };
+    const uint32_t S = M >> LG;
     const uint32_t j = lane & (uint32_t)(R - 1), slot = lane >> LG;
     for (uint32_t q0 = 0; q0 < qn; q0 += 32u / R) {
-        if (q0 + slot >= qn) continue;
-        const uint32_t lx = sc[16 + q0 + slot] + j * S;                    // log x < M
-        uint32_t acc = kZero;
-#pragma unroll 1
-        for (int i = D; i >= 0; i--) {
-            if (acc < M) acc = wrap(acc + lx);                             // acc * x
-            if ((nz >> i) & 1u) {                                          // acc + c_i
-                const uint32_t b = sc[i];
-                if (acc >= M) {
-                    acc = b;
-                } else {
-                    const uint32_t dd = wrap(b + M - acc);
-                    acc = dd == h ? kZero : wrap(acc + pol.single(dd, M, h));
-                }
-            }
-        }
-        if (acc < M) { nz_exact++; odd_exact += acc & 1u; }
+        const uint32_t qi = min(q0 + slot, qn - 1u);                       // idle slots repeat the last coset (not counted)
+        const uint32_t acc = horner_point<D>(pol, M, nz, sc, sc[16 + qi] + j * S);     // log x < M
+        if (q0 + slot < qn && acc < M) { nz_exact++; odd_exact += acc & 1u; }
     }
+}
+
+// Every x != 0 of a tiny field (M <= 64) by horner_point, one point per lane: there the coset machinery costs more than
+// it saves (for q = 13, k = 1 every coset holds an intermediate zero and is re-evaluated anyway).  Returns this lane's
+// (#{x: f(x) a nonzero square}, #{x: f(x) = 0}).
+template <int D, typename Pol>
+__device__ __noinline__ uint2 direct_all_x(const Pol pol, const uint32_t M, const uint32_t lane, const uint32_t nz, const uint32_t lcj,
+                                           volatile uint32_t *scratch) {
+    __syncwarp();
+    if (lane <= (uint32_t)D) scratch[lane] = lcj;
+    __syncwarp();
+    uint32_t n_sq = 0, n_zero = 0;
+    for (uint32_t base = 0; base < M; base += 32u) {
+        const uint32_t lx = min(base + lane, M - 1u);
+        const uint32_t acc = horner_point<D>(pol, M, nz, scratch, lx);
+        if (base + lane < M) {
+            n_zero += acc >= M ? 1u : 0u;
+            n_sq += (acc < M && !(acc & 1u)) ? 1u : 0u;
+        }
+    }
+    __syncwarp();
+    return make_uint2(n_sq, n_zero);
 }
 
 // ---------------------------------------------------------------------------------------------------------
