@@ -289,11 +289,20 @@ def reduced_rows(q: int, g: int, d: int, first: int, n: int, device=None):
     return rows, mult
 
 
-def curve_map(q: int, g: int, d: int, with_lambda: bool = False, index_range=None):
+def curve_map(q: int, g: int, d: int, with_lambda: bool = False, index_range=None, device: bool = False):
     """hec_curve_map / hec_curve_map_lambda / hec_curve_map_range (two-call capacity protocol): (keys [m][g (+1)] uint32,
     weights [m] uint64) on the host; with_lambda appends the lambda index (see lambda_partitions) as the last key
-    column; index_range = (first, n) restricts to those reduced polynomials (one rank's share)."""
+    column; index_range = (first, n) restricts to those reduced polynomials (one rank's share).
+    device=True: the outputs stay on the current CUDA device (int32 / int64 torch tensors holding the same bits)."""
     L = lib()
+    if device:
+        import torch
+
+        def alloc(cap, cols):
+            return (torch.empty((cap, cols), dtype=torch.int32, device="cuda"), torch.empty((cap,), dtype=torch.int64, device="cuda"))
+    else:
+        def alloc(cap, cols):
+            return np.empty((cap, cols), dtype=np.uint32), np.empty((cap,), dtype=np.uint64)
     if index_range is not None:
         first, cnt = index_range
 
@@ -307,15 +316,15 @@ def curve_map(q: int, g: int, d: int, with_lambda: bool = False, index_range=Non
     # always enough (at most two keys per reduced polynomial) instead of asking for the size first.
     n_red = index_range[1] if index_range is not None else reduced_total(q, g, d)
     cap = max(1024, min(2 * n_red, 1 << 24))
-    tup = np.empty((cap, cols), dtype=np.uint32)
-    w = np.empty((cap,), dtype=np.uint64)
+    tup, w = alloc(cap, cols)
     rc = fn(q, g, d, _ptr(tup), _ptr(w), ctypes.c_size_t(cap), ctypes.byref(m))
     if rc == HEC_ERR_CAPACITY:
         cap = m.value
-        tup = np.empty((cap, cols), dtype=np.uint32)
-        w = np.empty((cap,), dtype=np.uint64)
+        tup, w = alloc(cap, cols)
         rc = fn(q, g, d, _ptr(tup), _ptr(w), ctypes.c_size_t(cap), ctypes.byref(m))
     _check(rc)
+    if device:
+        return tup[: m.value].clone(), w[: m.value].clone()
     return tup[: m.value].copy(), w[: m.value].copy()
 
 
