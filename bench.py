@@ -107,7 +107,7 @@ def executed_loads(cfg: W.Workload, rows: np.ndarray, stats: dict) -> dict:
             if fast and R == Rf:
                 full = pr.all(axis=1)                        # R' = 2 without every class present takes the general loop
                 sub = nzm[sel][full]
-                for r in range(R):
+                for r in range(R if len(sub) else 0):
                     cls = sub[:, r::R][:, ::-1]              # class r, top exponent first
                     first = cls.argmax(axis=1)
                     idx = np.arange(len(cls))
@@ -408,9 +408,14 @@ def run_ours(args, cfg):
     h_sf = torch.empty((n,), dtype=torch.uint8).pin_memory()
     np_rows, np_cnt, np_sf = h_rows.numpy().view(np.uint16), h_cnt.numpy().view(np.uint32), h_sf.numpy()
 
-    def e2e_step():
-        hec.count(q, g, np_rows, np_cnt, np_sf)
-        return hec.histogram(np_cnt, np_sf)
+    cap = min(n, m["distinct_tuples"] + m["distinct_tuples"] // 8 + 1024)     # pinned result buffers, sized from the warm-up
+    h_tup = torch.empty((cap, g), dtype=torch.int32).pin_memory()
+    h_mult = torch.empty((cap,), dtype=torch.int64).pin_memory()
+    np_tup, np_mult = h_tup.numpy().view(np.uint32), h_mult.numpy().view(np.uint64)
+
+    def e2e_step():                                                # the call a user makes for one pass of the hot path
+        _, _, tup_, mult_ = hec.count_histogram(q, g, np_rows, np_cnt, np_sf, out_tuples=np_tup, out_mult=np_mult)
+        return tup_, mult_
 
     e2e_step()
     sync_all()
@@ -423,7 +428,7 @@ def run_ours(args, cfg):
     if world > 1:
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
     e2e_s = float(t.item())
-    h2d = np_rows.nbytes + np_cnt.nbytes + np_sf.nbytes            # rows for hec_count; counts + mask for hec_histogram
+    h2d = np_rows.nbytes                                           # the rows; the histogram reads the device copy of the counts
     d2h = np_cnt.nbytes + np_sf.nbytes + e_tup.nbytes + e_mult.nbytes
 
     if rank != 0:
@@ -466,7 +471,7 @@ def run_ours(args, cfg):
         line["cpu_baseline"]["parity_rows_checked"] = int(len(idx))
         line["cpu_baseline"]["parity_ok"] = bool(
             (np_cnt[idx] == o_cnt).all() and (np_sf[idx] == o_sf).all())
-    del m, h_rows, h_cnt, h_sf
+    del m, h_rows, h_cnt, h_sf, h_tup, h_mult
     if world == 1 and args.sub_configs and args.config == 4 and args.eval == "auto" and not args.curves:
         line["configs"] = sub_config_records(torch, hec, D, args, local_rank, counters)
     print(json.dumps(line), flush=True)

@@ -15,6 +15,11 @@
  *     the stream, because the status code depends on device-side validation).
  *   - The caller owns every buffer it passes in; the library owns hec_field handles
  *     and its internal per-(q,g) device plans (released by hec_shutdown).
+ *   - ONE GPU PER PROCESS: the library's state (table plans, staging buffers, the
+ *     histogram pool) lives on the CUDA device that is current at the first call that
+ *     touches the device.  A later call with another current device fails with
+ *     HEC_ERR_INVALID_ARG; hec_shutdown() releases everything, after which the next
+ *     call binds to the device current then.
  *   - An F_q element (q = p^r, p an odd prime) is the integer sum a_i p^i, which
  *     stands for sum a_i T^i in F_p[T]/(R_q) (little-endian base-p digits,
  *     PAPER.md:199); R_q is the lexicographically smallest monic primitive
@@ -102,7 +107,9 @@ void hec_field_embed(const hec_field *F, uint32_t *out);       /* q entries */
  *   out_squarefree[n] uint8 in {0,1}: deg gcd(f, f') = 0 over F_q; may be NULL
  * N_k is computed by the same formula whether or not f is squarefree (reading G12).
  * Pointers: all host or all device.  Host pointers: the library stages the batch through its own
- * device buffers (H2D, kernels, D2H) on the current stream.  n = 0 is a no-op.
+ * device buffers; from 2^20 rows on, in four chunks through two internal copy streams, so that the H2D copy of
+ * chunk i+1 and the D2H copies of chunk i-1 run under the kernels of chunk i (pinned host memory overlaps;
+ * pageable memory is staged by the driver and is merely slower).  n = 0 is a no-op.
  * Errors: HEC_ERR_INVALID_FIELD (q not an odd prime power below 65536, q^g too large),
  * HEC_ERR_INVALID_ARG, HEC_ERR_COEFF_RANGE, HEC_ERR_DEGREE (outputs are unspecified after these
  * two), HEC_ERR_CUDA, HEC_ERR_NOMEM.
@@ -125,6 +132,17 @@ int hec_count(uint32_t q, uint32_t g, const uint16_t *coeffs, size_t n,
  */
 int hec_histogram(const uint32_t *counts, const uint8_t *mask, size_t n, uint32_t g,
                   uint32_t *out_tuples, uint64_t *out_mult, size_t cap, size_t *out_m);
+
+/*
+ * hec_count_histogram -- one pass of the whole hot path in ONE call: hec_count followed by hec_histogram of the rows
+ * with a nonzero squarefree flag (of every row when out_squarefree is NULL).  Arguments as in hec_count and
+ * hec_histogram (same capacity protocol: on HEC_ERR_CAPACITY out_counts / out_squarefree are complete and only the
+ * histogram has to be repeated, e.g. with hec_histogram).  All array pointers host or all device.  With host
+ * pointers the counts never make the round trip: the histogram runs on the device copies while the last D2H copies
+ * of the counts are still in flight, and only the distinct tuples come back.
+ */
+int hec_count_histogram(uint32_t q, uint32_t g, const uint16_t *coeffs, size_t n, uint32_t *out_counts,
+                        uint8_t *out_squarefree, uint32_t *out_tuples, uint64_t *out_mult, size_t cap, size_t *out_m);
 
 /*
  * hec_histogram_merge -- the one exchange step of the multi-GPU path: merges partial
@@ -262,6 +280,7 @@ typedef struct hec_count_stats {
     uint32_t splits;           /* warps per curve: 1 for batches; > 1 when a small batch (down to a single curve) is spread
                                   over the whole GPU, each warp taking a slice of the x range of every field */
     uint32_t fast_fields;      /* bit k-1: field k carried fast tables (hec_set_fast_tables) */
+    uint32_t chunks;           /* host-pointer calls: number of row chunks pipelined through the copy streams (1: none) */
 } hec_count_stats;
 int hec_last_count_stats(hec_count_stats *out);
 

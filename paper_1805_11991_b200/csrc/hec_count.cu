@@ -178,7 +178,15 @@ __global__ void __launch_bounds__(256) hec_shift_kernel(const HecShiftParams P) 
 LibState g_state;
 
 int ensure_device(LibState &S) {
-    if (S.device_ready) return HEC_OK;
+    if (S.device_ready) {                         // one GPU per process (hec.h): plans, staging buffers and pools live on S.device
+        int cur = -1;
+        if (cudaGetDevice(&cur) != cudaSuccess || cur != S.device) {
+            cudaGetLastError();
+            HEC_FAIL(HEC_ERR_INVALID_ARG, "libhec is bound to the CUDA device that was current at its first call (one GPU per process); "
+                                          "call hec_shutdown() before switching devices");
+        }
+        return HEC_OK;
+    }
     int dev = 0, cnt = 0;
     if (cudaGetDeviceCount(&cnt) != cudaSuccess || cnt == 0) {
         cudaGetLastError();
@@ -188,6 +196,10 @@ int ensure_device(LibState &S) {
     HEC_CUDA_OK(cudaDeviceGetAttribute(&S.sm_count, cudaDevAttrMultiProcessorCount, dev));
     HEC_CUDA_OK(cudaDeviceGetAttribute(&S.smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
     for (auto &e : S.ev) HEC_CUDA_OK(cudaEventCreate(&e));
+    for (auto &e : S.ev_chunk) HEC_CUDA_OK(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+    HEC_CUDA_OK(cudaStreamCreateWithFlags(&S.copy_in, cudaStreamNonBlocking));
+    HEC_CUDA_OK(cudaStreamCreateWithFlags(&S.copy_out, cudaStreamNonBlocking));
+    S.device = dev;
     S.device_ready = true;
     hec_allow_device_field_build(true);          // fields above 2^16 elements are now built by hec_field_device.cu
     return HEC_OK;
@@ -643,22 +655,49 @@ int hec_count(uint32_t q, uint32_t g, const uint16_t *coeffs, size_t n, uint32_t
     return hec_count_ex(q, g, coeffs, n, out_counts, out_squarefree, nullptr, nullptr);
 }
 
-int hec_count_ex(uint32_t q, uint32_t g, const uint16_t *coeffs, size_t n, uint32_t *out_counts, uint8_t *out_squarefree,
-                 uint32_t *out_roots, uint8_t *out_lambda) {
-    if (g < 1 || g > HEC_MAX_GENUS) HEC_FAIL(HEC_ERR_INVALID_ARG, "g must be in [1, HEC_MAX_GENUS]");
-    uint32_t p, r;
-    if (!hec_factor_q(q, &p, &r)) HEC_FAIL(HEC_ERR_INVALID_FIELD, "q must be an odd prime power below 65536");
-    {
-        uint64_t Qg = 1;
-        for (uint32_t i = 0; i < g; i++) { Qg *= q; if (Qg > HEC_MAX_FIELD_SIZE) HEC_FAIL(HEC_ERR_INVALID_FIELD, "q^g exceeds HEC_MAX_FIELD_SIZE (2^26)"); }
-    }
-    if (n == 0) return HEC_OK;
-    if (!coeffs || !out_counts) HEC_FAIL(HEC_ERR_INVALID_ARG, "coeffs and out_counts must not be NULL");
+}  // extern "C"
 
-    std::lock_guard<std::recursive_mutex> lock(g_state.mu);
-    LibState &S = g_state;
-    int rc = ensure_device(S);
-    if (rc) return rc;
+namespace {
+
+// Host buffers: rows in chunks through three streams -- H2D of chunk i+1 and D2H of chunk i-1 run under the kernels of
+// chunk i (pinned host memory; pageable memory is staged by the driver and still correct).  Below this many rows one chunk.
+constexpr size_t kPipelineMinRows = (size_t)1 << 20;
+constexpr int kPipelineChunks = 4;
+
+// hec_count_ex.  keep_device (host-pointer calls of hec_count_histogram): do not wait for the D2H copies; return the device
+// copies of the counts and the flags (valid until the next call) so that the histogram can start under those copies, and
+// leave the status check to finish_count().
+struct CountTail {
+    DevicePlan *plan = nullptr;
+    unsigned long long err[2] = {~0ull, ~0ull};
+    bool pending = false;          // D2H copies in flight on S.copy_out
+    const uint32_t *d_counts = nullptr;
+    const uint8_t *d_sf = nullptr;
+};
+
+int finish_count(LibState &S, CountTail &T) {
+    if (T.pending) {
+        HEC_CUDA_OK(cudaStreamSynchronize(S.copy_out));
+        T.pending = false;
+    }
+    HEC_CUDA_OK(cudaStreamSynchronize(S.stream));
+    cudaEventElapsedTime(&S.stats.count_kernel_ms, S.ev[0], S.ev[1]);
+    cudaEventElapsedTime(&S.stats.squarefree_kernel_ms, S.ev[1], S.ev[2]);
+    if (T.err[0] != ~0ull) {
+        hec_set_error(HEC_ERR_COEFF_RANGE, "a coefficient is >= q", (size_t)T.err[0]);
+        return HEC_ERR_COEFF_RANGE;
+    }
+    if (T.err[1] != ~0ull) {
+        hec_set_error(HEC_ERR_DEGREE, "a row has c[2g+2] = c[2g+1] = 0 (degree < 2g+1)", (size_t)T.err[1]);
+        return HEC_ERR_DEGREE;
+    }
+    return HEC_OK;
+}
+
+int count_impl(LibState &S, uint32_t q, uint32_t g, const uint16_t *coeffs, size_t n, uint32_t *out_counts, uint8_t *out_squarefree,
+               uint32_t *out_roots, uint8_t *out_lambda, bool keep_device, CountTail &T) {
+    uint32_t p, r;
+    hec_factor_q(q, &p, &r);
     const bool dev_in = is_device_pointer(coeffs), dev_out = is_device_pointer(out_counts);
     const bool dev_sf = out_squarefree ? is_device_pointer(out_squarefree) : dev_out;
     const bool dev_r0 = out_roots ? is_device_pointer(out_roots) : dev_out;
@@ -667,8 +706,9 @@ int hec_count_ex(uint32_t q, uint32_t g, const uint16_t *coeffs, size_t n, uint3
         HEC_FAIL(HEC_ERR_INVALID_ARG, "coeffs/out_counts/out_squarefree/out_roots/out_lambda must all be host or all device pointers");
 
     DevicePlan *plan = nullptr;
-    rc = build_plan(S, q, g, S.regime, S.eval, &plan);
+    int rc = build_plan(S, q, g, S.regime, S.eval, &plan);
     if (rc) return rc;
+    T.plan = plan;
 
     const size_t ncoef = 2 * (size_t)g + 3;
     const size_t in_bytes = n * ncoef * sizeof(uint16_t), cnt_bytes = n * g * sizeof(uint32_t), sf_bytes = out_squarefree ? n : 0;
@@ -696,17 +736,17 @@ int hec_count_ex(uint32_t q, uint32_t g, const uint16_t *coeffs, size_t n, uint3
             d_counts = reinterpret_cast<uint32_t *>(base + a);
             d_sf = out_squarefree ? base + a + b : nullptr;
             d_lam = out_lambda ? base + a + b + c + r0b : nullptr;
-            HEC_CUDA_OK(cudaMemcpyAsync(base, coeffs, in_bytes, cudaMemcpyHostToDevice, S.stream));
         }
         if (r0b) d_r0 = reinterpret_cast<uint32_t *>(base + a + b + c);
     }
+    T.d_counts = d_counts;
+    T.d_sf = d_sf;
 
     static const unsigned long long kNoErr[2] = {~0ull, ~0ull};
     HEC_CUDA_OK(cudaMemcpyAsync(plan->d_err, kNoErr, sizeof kNoErr, cudaMemcpyHostToDevice, S.stream));
 
     HecCountParams P;
-    P.coeffs = d_coeffs; P.out = d_counts; P.out_r0 = need_r0 ? d_r0 : nullptr; P.n = n; P.q = q;
-    P.blob = nullptr; P.blob_bytes = 0; P.err = plan->d_err; P.k_lo = 1; P.k_hi = g; P.scratch_off = 0;
+    P.q = q; P.blob = nullptr; P.blob_bytes = 0; P.err = plan->d_err; P.k_lo = 1; P.k_hi = g; P.scratch_off = 0;
     // Small batches (down to the single curve of the paper's Table 1): spread every curve over
     // `splits` warps so that the whole GPU works on it; each warp takes a slice of the cosets of every field.
     P.splits = 1;
@@ -720,62 +760,142 @@ int hec_count_ex(uint32_t q, uint32_t g, const uint16_t *coeffs, size_t n, uint3
     }
     if (P.splits > 1) {
         HEC_CUDA_OK(cudaMemsetAsync(d_counts, 0, cnt_bytes, S.stream));
-        if (P.out_r0) HEC_CUDA_OK(cudaMemsetAsync(P.out_r0, 0, cnt_bytes, S.stream));
+        if (need_r0) HEC_CUDA_OK(cudaMemsetAsync(d_r0, 0, cnt_bytes, S.stream));
     }
-    const uint32_t splits_used = P.splits;
     for (uint32_t k = 0; k < HEC_MAX_GENUS; k++) P.f[k] = plan->f[k < g ? k : 0];
 
     S.stats = hec_count_stats{};
     S.stats.table_mode = (uint32_t)plan->top_mode;
     S.stats.regime = (plan->top_mode == HEC_TAB_EXT16 || plan->top_mode == HEC_TAB_PAIR16) ? HEC_REGIME_SMEM
                      : (plan->top_mode == HEC_TAB_GLOBAL32 || plan->top_mode == HEC_TAB_GPAIR64) ? HEC_REGIME_L2 : HEC_REGIME_SMEM_HALF;
-    S.stats.splits = splits_used;
+    S.stats.splits = P.splits;
+
+    const bool shift = plan->shift_R && S.shift_enabled;
+    if (shift) {                                               // the whole batch's shifted rows live in S.d_shift
+        if (in_bytes > S.shift_bytes) {
+            if (S.d_shift) cudaFree(S.d_shift);
+            S.d_shift = nullptr; S.shift_bytes = 0;
+            if (cudaMalloc(&S.d_shift, in_bytes) != cudaSuccess) { cudaGetLastError(); HEC_FAIL(HEC_ERR_NOMEM, "cannot allocate the shifted-row buffer"); }
+            S.shift_bytes = in_bytes;
+        }
+    }
+    const int chunks = (!dev_in && n >= kPipelineMinRows) ? kPipelineChunks : 1;
+    S.stats.chunks = (uint32_t)chunks;
+    if (chunks > 1) {                                          // the copy streams start after whatever precedes on S.stream
+        HEC_CUDA_OK(cudaEventRecord(S.ev_chunk[0], S.stream));
+        HEC_CUDA_OK(cudaStreamWaitEvent(S.copy_in, S.ev_chunk[0], 0));
+        HEC_CUDA_OK(cudaStreamWaitEvent(S.copy_out, S.ev_chunk[0], 0));
+    }
     HEC_CUDA_OK(cudaEventRecord(S.ev[0], S.stream));
-    if (plan->shift_R && S.shift_enabled) {                    // pre-pass: no empty residue class mod R (hec_shift_kernel)
-        if ((rc = run_shift(S, *plan, d_coeffs, n, nullptr))) return rc;
-        P.coeffs = static_cast<const uint16_t *>(S.d_shift);
-    }
-    switch (g) {
-        case 1: rc = hec_launch_count_g1(S, *plan, P); break;
-        case 2: rc = hec_launch_count_g2(S, *plan, P); break;
-        case 3: rc = hec_launch_count_g3(S, *plan, P); break;
-        case 4: rc = hec_launch_count_g4(S, *plan, P); break;
-        default: rc = hec_launch_count_g5(S, *plan, P); break;
-    }
-    if (rc) return rc;
-    HEC_CUDA_OK(cudaEventRecord(S.ev[1], S.stream));
-    if (d_sf || d_lam) {
-        HecSquarefreeParams Q;
-        Q.coeffs = d_coeffs; Q.out = d_sf; Q.n = n; Q.p = p; Q.q = q; Q.M = q - 1; Q.ncoef = (uint32_t)ncoef;
-        Q.zech = plan->sq_zech; Q.emb = plan->sq_emb;
-        Q.roots = d_lam ? d_r0 : nullptr; Q.out_lambda = d_lam; Q.part_codes = plan->d_part_codes; Q.n_parts = plan->n_parts; Q.g = g;
-        const unsigned long long blocks = (n + 255) / 256;
-        hec_squarefree_kernel<<<(unsigned)blocks, 256, 0, S.stream>>>(Q);
-        hec_launch_counter::value++;
-        S.stats.launches++;
-        HEC_CUDA_OK(cudaGetLastError());
+    for (int c = 0; c < chunks; c++) {
+        const size_t lo = n * (size_t)c / chunks, hi = n * (size_t)(c + 1) / chunks, nc = hi - lo;
+        if (nc == 0) continue;
+        cudaStream_t s_in = chunks > 1 ? S.copy_in : S.stream, s_out = chunks > 1 ? S.copy_out : S.stream;
+        if (!dev_in) {
+            HEC_CUDA_OK(cudaMemcpyAsync(const_cast<uint16_t *>(d_coeffs) + lo * ncoef, coeffs + lo * ncoef, nc * ncoef * sizeof(uint16_t),
+                                        cudaMemcpyHostToDevice, s_in));
+            if (chunks > 1) {
+                HEC_CUDA_OK(cudaEventRecord(S.ev_chunk[1 + 2 * c], s_in));
+                HEC_CUDA_OK(cudaStreamWaitEvent(S.stream, S.ev_chunk[1 + 2 * c], 0));
+            }
+        }
+        P.coeffs = d_coeffs + lo * ncoef; P.out = d_counts + lo * g; P.out_r0 = need_r0 ? d_r0 + lo * g : nullptr; P.n = nc; P.row0 = lo;
+        if (shift) {                                           // pre-pass: no empty residue class mod R (hec_shift_kernel)
+            uint16_t *d_sh = static_cast<uint16_t *>(S.d_shift) + lo * ncoef;
+            if ((rc = run_shift(S, *plan, P.coeffs, nc, d_sh))) return rc;
+            P.coeffs = d_sh;
+        }
+        switch (g) {
+            case 1: rc = hec_launch_count_g1(S, *plan, P); break;
+            case 2: rc = hec_launch_count_g2(S, *plan, P); break;
+            case 3: rc = hec_launch_count_g3(S, *plan, P); break;
+            case 4: rc = hec_launch_count_g4(S, *plan, P); break;
+            default: rc = hec_launch_count_g5(S, *plan, P); break;
+        }
+        if (rc) return rc;
+        if (c == chunks - 1) HEC_CUDA_OK(cudaEventRecord(S.ev[1], S.stream));
+        if (d_sf || d_lam) {
+            HecSquarefreeParams Q;
+            Q.coeffs = d_coeffs + lo * ncoef; Q.out = d_sf ? d_sf + lo : nullptr; Q.n = nc; Q.p = p; Q.q = q; Q.M = q - 1; Q.ncoef = (uint32_t)ncoef;
+            Q.zech = plan->sq_zech; Q.emb = plan->sq_emb;
+            Q.roots = d_lam ? d_r0 + lo * g : nullptr; Q.out_lambda = d_lam ? d_lam + lo : nullptr;
+            Q.part_codes = plan->d_part_codes; Q.n_parts = plan->n_parts; Q.g = g;
+            const unsigned long long blocks = (nc + 255) / 256;
+            hec_squarefree_kernel<<<(unsigned)blocks, 256, 0, S.stream>>>(Q);
+            hec_launch_counter::value++;
+            S.stats.launches++;
+            HEC_CUDA_OK(cudaGetLastError());
+        }
+        if (!dev_in) {
+            if (chunks > 1) {
+                HEC_CUDA_OK(cudaEventRecord(S.ev_chunk[2 + 2 * c], S.stream));
+                HEC_CUDA_OK(cudaStreamWaitEvent(s_out, S.ev_chunk[2 + 2 * c], 0));
+            }
+            HEC_CUDA_OK(cudaMemcpyAsync(out_counts + lo * g, d_counts + lo * g, nc * g * sizeof(uint32_t), cudaMemcpyDeviceToHost, s_out));
+            if (out_squarefree) HEC_CUDA_OK(cudaMemcpyAsync(out_squarefree + lo, d_sf + lo, nc, cudaMemcpyDeviceToHost, s_out));
+            if (out_roots) HEC_CUDA_OK(cudaMemcpyAsync(out_roots + lo * g, d_r0 + lo * g, nc * g * sizeof(uint32_t), cudaMemcpyDeviceToHost, s_out));
+            if (out_lambda) HEC_CUDA_OK(cudaMemcpyAsync(out_lambda + lo, d_lam + lo, nc, cudaMemcpyDeviceToHost, s_out));
+        }
     }
     HEC_CUDA_OK(cudaEventRecord(S.ev[2], S.stream));
-    unsigned long long err[2];
-    HEC_CUDA_OK(cudaMemcpyAsync(err, plan->d_err, sizeof err, cudaMemcpyDeviceToHost, S.stream));
-    if (!dev_in) {
-        HEC_CUDA_OK(cudaMemcpyAsync(out_counts, d_counts, cnt_bytes, cudaMemcpyDeviceToHost, S.stream));
-        if (out_squarefree) HEC_CUDA_OK(cudaMemcpyAsync(out_squarefree, d_sf, sf_bytes, cudaMemcpyDeviceToHost, S.stream));
-        if (out_roots) HEC_CUDA_OK(cudaMemcpyAsync(out_roots, d_r0, cnt_bytes, cudaMemcpyDeviceToHost, S.stream));
-        if (out_lambda) HEC_CUDA_OK(cudaMemcpyAsync(out_lambda, d_lam, lam_bytes, cudaMemcpyDeviceToHost, S.stream));
-    }
-    HEC_CUDA_OK(cudaStreamSynchronize(S.stream));
-    cudaEventElapsedTime(&S.stats.count_kernel_ms, S.ev[0], S.ev[1]);
-    cudaEventElapsedTime(&S.stats.squarefree_kernel_ms, S.ev[1], S.ev[2]);
-    if (err[0] != ~0ull) {
-        hec_set_error(HEC_ERR_COEFF_RANGE, "a coefficient is >= q", (size_t)err[0]);
-        return HEC_ERR_COEFF_RANGE;
-    }
-    if (err[1] != ~0ull) {
-        hec_set_error(HEC_ERR_DEGREE, "a row has c[2g+2] = c[2g+1] = 0 (degree < 2g+1)", (size_t)err[1]);
-        return HEC_ERR_DEGREE;
-    }
+    HEC_CUDA_OK(cudaMemcpyAsync(T.err, plan->d_err, sizeof T.err, cudaMemcpyDeviceToHost, S.stream));
+    T.pending = chunks > 1;
+    if (keep_device) return HEC_OK;
+    return finish_count(S, T);
+}
+
+int check_count_args(uint32_t q, uint32_t g) {
+    if (g < 1 || g > HEC_MAX_GENUS) HEC_FAIL(HEC_ERR_INVALID_ARG, "g must be in [1, HEC_MAX_GENUS]");
+    uint32_t p, r;
+    if (!hec_factor_q(q, &p, &r)) HEC_FAIL(HEC_ERR_INVALID_FIELD, "q must be an odd prime power below 65536");
+    uint64_t Qg = 1;
+    for (uint32_t i = 0; i < g; i++) { Qg *= q; if (Qg > HEC_MAX_FIELD_SIZE) HEC_FAIL(HEC_ERR_INVALID_FIELD, "q^g exceeds HEC_MAX_FIELD_SIZE (2^26)"); }
     return HEC_OK;
+}
+
+}  // namespace
+
+int hec_histogram_mixed(const uint32_t *counts, const uint8_t *mask, size_t n, uint32_t g, uint32_t *out_tuples, uint64_t *out_mult,
+                        size_t cap, size_t *out_m);
+
+extern "C" {
+
+int hec_count_ex(uint32_t q, uint32_t g, const uint16_t *coeffs, size_t n, uint32_t *out_counts, uint8_t *out_squarefree,
+                 uint32_t *out_roots, uint8_t *out_lambda) {
+    int rc = check_count_args(q, g);
+    if (rc) return rc;
+    if (n == 0) return HEC_OK;
+    if (!coeffs || !out_counts) HEC_FAIL(HEC_ERR_INVALID_ARG, "coeffs and out_counts must not be NULL");
+    std::lock_guard<std::recursive_mutex> lock(g_state.mu);
+    LibState &S = g_state;
+    if ((rc = ensure_device(S))) return rc;
+    CountTail T;
+    return count_impl(S, q, g, coeffs, n, out_counts, out_squarefree, out_roots, out_lambda, false, T);
+}
+
+int hec_count_histogram(uint32_t q, uint32_t g, const uint16_t *coeffs, size_t n, uint32_t *out_counts, uint8_t *out_squarefree,
+                        uint32_t *out_tuples, uint64_t *out_mult, size_t cap, size_t *out_m) {
+    int rc = check_count_args(q, g);
+    if (rc) return rc;
+    if (!out_m) HEC_FAIL(HEC_ERR_INVALID_ARG, "out_m must not be NULL");
+    *out_m = 0;
+    if (n == 0) return HEC_OK;
+    if (!coeffs || !out_counts) HEC_FAIL(HEC_ERR_INVALID_ARG, "coeffs and out_counts must not be NULL");
+    if (cap > 0 && (!out_tuples || !out_mult)) HEC_FAIL(HEC_ERR_INVALID_ARG, "out_tuples/out_mult must not be NULL when cap > 0");
+    std::lock_guard<std::recursive_mutex> lock(g_state.mu);
+    LibState &S = g_state;
+    if ((rc = ensure_device(S))) return rc;
+    const bool dev = is_device_pointer(coeffs);
+    if (cap > 0 && (is_device_pointer(out_tuples) != dev || is_device_pointer(out_mult) != dev))
+        HEC_FAIL(HEC_ERR_INVALID_ARG, "coeffs/out_counts/out_squarefree/out_tuples/out_mult must all be host or all device pointers");
+    CountTail T;
+    if ((rc = count_impl(S, q, g, coeffs, n, out_counts, out_squarefree, nullptr, nullptr, true, T))) return rc;
+    // the histogram reads the device copies (for host callers: while the last D2H copies of the counts are still running)
+    const hec_count_stats keep = S.stats;
+    const int hrc = hec_histogram_mixed(T.d_counts, T.d_sf, n, g, out_tuples, out_mult, cap, out_m);
+    S.stats = keep;
+    rc = finish_count(S, T);
+    return rc ? rc : hrc;
 }
 
 int hec_set_fast_tables(int on) {
@@ -840,6 +960,11 @@ void hec_shutdown(void) {
     if (g_state.d_shift) { cudaFree(g_state.d_shift); g_state.d_shift = nullptr; g_state.shift_bytes = 0; }
     hec_histogram_release_pool();
     hec_clear_field_cache();
+    for (auto &e : g_state.ev) if (e) { cudaEventDestroy(e); e = nullptr; }
+    for (auto &e : g_state.ev_chunk) if (e) { cudaEventDestroy(e); e = nullptr; }
+    if (g_state.copy_in) { cudaStreamDestroy(g_state.copy_in); g_state.copy_in = nullptr; }
+    if (g_state.copy_out) { cudaStreamDestroy(g_state.copy_out); g_state.copy_out = nullptr; }
+    g_state.device_ready = false;                 // the next call binds to the device current then
 }
 
 }  // extern "C"

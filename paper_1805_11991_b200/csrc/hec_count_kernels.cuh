@@ -72,6 +72,9 @@ struct LibState {
     std::map<std::tuple<uint32_t, uint32_t, int, int>, std::unique_ptr<DevicePlan>> plans;
     hec_count_stats stats{};
     cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};
+    // host-buffer pipeline of hec_count (hec_count.cu: count_impl): copy streams and per-chunk events
+    cudaStream_t copy_in = nullptr, copy_out = nullptr;
+    cudaEvent_t ev_chunk[16] = {};
     // staging buffers for host-pointer calls
     void *d_stage = nullptr;
     size_t stage_bytes = 0;
@@ -81,6 +84,7 @@ struct LibState {
     bool shift_enabled = true;
     bool fast_enabled = true;  // fast tables of the PAIR16 fields (radix_fast_x); part of the plan key
     int sm_count = 0, smem_optin = 0;
+    int device = -1;           // the CUDA device the state lives on: the one current at the first call
     bool device_ready = false;
 };
 
@@ -262,7 +266,7 @@ __global__ void __launch_bounds__(kThreads, 1) hec_count_kernel(const __grid_con
         const uint32_t nz = __ballot_sync(0xffffffffu, cj != 0);          // bit j: c_j != 0
         const bool mine = lane + 1 >= P.k_lo && lane + 1 <= P.k_hi;
         if (bad_range || (nz >> (D - 1)) == 0) {
-            if (lane == 0) atomicMin(&P.err[bad_range ? 0 : 1], curve);
+            if (lane == 0) atomicMin(&P.err[bad_range ? 0 : 1], curve + P.row0);
             if (mine) { P.out[curve * G + lane] = 0; if (P.out_r0) P.out_r0[curve * G + lane] = 0; }
             continue;
         }
@@ -415,7 +419,7 @@ __global__ void __launch_bounds__(kThreads, 1) hec_count_radix_kernel(const __gr
         const uint32_t nz = __ballot_sync(0xffffffffu, cj != 0);
         const bool mine = lane + 1 >= P.k_lo && lane + 1 <= P.k_hi;
         if (bad_range || (nz >> (D - 1)) == 0) {
-            if (lane == 0) atomicMin(&P.err[bad_range ? 0 : 1], curve);
+            if (lane == 0) atomicMin(&P.err[bad_range ? 0 : 1], curve + P.row0);
             if (mine && !SPLIT) { P.out[curve * G + lane] = 0; if (P.out_r0) P.out_r0[curve * G + lane] = 0; }
             continue;
         }

@@ -61,6 +61,7 @@ struct HecCountParams {
     uint32_t scratch_off;          // radix kernel: byte offset (after the blob) of the per-warp scratch words
     uint32_t *out_r0;              // [n][g] or NULL: r0_k = #{x in F_{q^k}: f(x) = 0}, the input of lambda
     uint32_t splits;               // radix kernel: warps per curve (>= 1); > 1: out is pre-zeroed and accumulated with atomics
+    unsigned long long row0;       // index of this launch's first row in the caller's batch (error reporting)
     HecFieldDev f[HEC_MAX_GENUS];
 };
 

@@ -267,8 +267,9 @@ struct DeviceBuf {
 
 void hec_histogram_release_pool() { g_pool.clear(); }
 
+// mixed: device inputs with outputs on either side (hec_count_histogram with host buffers: the counts are still on the device)
 static int histogram_impl(const uint32_t *counts, const uint8_t *mask, const uint64_t *weights, size_t n, uint32_t g,
-                          uint32_t *out_tuples, uint64_t *out_mult, size_t cap, size_t *out_m) {
+                          uint32_t *out_tuples, uint64_t *out_mult, size_t cap, size_t *out_m, bool mixed = false) {
     if (g < 1 || g > HEC_MAX_GENUS) HEC_FAIL(HEC_ERR_INVALID_ARG, "g must be in [1, HEC_MAX_GENUS]");
     if (!out_m) HEC_FAIL(HEC_ERR_INVALID_ARG, "out_m must not be NULL");
     *out_m = 0;
@@ -280,7 +281,8 @@ static int histogram_impl(const uint32_t *counts, const uint8_t *mask, const uin
     if (rc) return rc;
     cudaStream_t st = hec_current_stream();
     const bool dev = hec_is_device_pointer(counts);
-    if ((mask && hec_is_device_pointer(mask) != dev) || (weights && hec_is_device_pointer(weights) != dev) || (cap > 0 && (hec_is_device_pointer(out_tuples) != dev || hec_is_device_pointer(out_mult) != dev)))
+    const bool dev_out = (mixed && cap > 0) ? hec_is_device_pointer(out_tuples) : dev;
+    if ((mask && hec_is_device_pointer(mask) != dev) || (weights && hec_is_device_pointer(weights) != dev) || (cap > 0 && (hec_is_device_pointer(out_tuples) != dev_out || hec_is_device_pointer(out_mult) != dev_out)))
         HEC_FAIL(HEC_ERR_INVALID_ARG, "counts/mask/out_tuples/out_mult must all be host or all device pointers");
 
     DeviceBuf in_counts, in_mask, in_w;
@@ -388,7 +390,7 @@ static int histogram_impl(const uint32_t *counts, const uint8_t *mask, const uin
     DeviceBuf o_t, o_m;
     uint32_t *d_t = out_tuples;
     unsigned long long *d_mu = reinterpret_cast<unsigned long long *>(out_mult);
-    if (!dev) {
+    if (!dev_out) {
         if ((rc = o_t.alloc(m * g * 4)) || (rc = o_m.alloc(m * 8))) return rc;
         d_t = static_cast<uint32_t *>(o_t.p);
         d_mu = static_cast<unsigned long long *>(o_m.p);
@@ -396,7 +398,7 @@ static int histogram_impl(const uint32_t *counts, const uint8_t *mask, const uin
     hist_unpack_kernel<<<(unsigned)((m + 255) / 256), 256, 0, st>>>(ka, va, m, S, d_t, d_mu);
     hec_launch_counter::value++;
     HEC_CUDA_OK(cudaGetLastError());
-    if (!dev) {
+    if (!dev_out) {
         HEC_CUDA_OK(cudaMemcpyAsync(out_tuples, d_t, m * g * 4, cudaMemcpyDeviceToHost, st));
         HEC_CUDA_OK(cudaMemcpyAsync(out_mult, d_mu, m * 8, cudaMemcpyDeviceToHost, st));
     }
@@ -407,6 +409,12 @@ static int histogram_impl(const uint32_t *counts, const uint8_t *mask, const uin
 extern "C" int hec_histogram(const uint32_t *counts, const uint8_t *mask, size_t n, uint32_t g, uint32_t *out_tuples,
                              uint64_t *out_mult, size_t cap, size_t *out_m) {
     return histogram_impl(counts, mask, nullptr, n, g, out_tuples, out_mult, cap, out_m);
+}
+
+// hec_count.cu (hec_count_histogram): device counts / mask, outputs on the caller's side
+int hec_histogram_mixed(const uint32_t *counts, const uint8_t *mask, size_t n, uint32_t g, uint32_t *out_tuples, uint64_t *out_mult,
+                        size_t cap, size_t *out_m) {
+    return histogram_impl(counts, mask, nullptr, n, g, out_tuples, out_mult, cap, out_m, true);
 }
 
 // hec_enum.cu: weighted histogram of the rows with a nonzero mask (Algorithm 1 line 20 for one chunk).

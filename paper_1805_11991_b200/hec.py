@@ -34,7 +34,7 @@ SYMBOLS = [
     "hec_field_degree", "hec_field_q", "hec_field_Q", "hec_field_embed_unit", "hec_field_modulus",
     "hec_field_antilog", "hec_field_log", "hec_field_zech", "hec_field_embed", "hec_count", "hec_histogram",
     "hec_histogram_merge", "hec_reduced_total", "hec_reduced_rows", "hec_curve_map",
-    "hec_count_ex", "hec_lambda_partitions", "hec_curve_map_lambda", "hec_set_map_chunk_rows", "hec_curve_map_range", "hec_curve_map_all", "hec_set_shift", "hec_shift_rows", "hec_set_fast_tables",
+    "hec_count_ex", "hec_lambda_partitions", "hec_curve_map_lambda", "hec_set_map_chunk_rows", "hec_curve_map_range", "hec_curve_map_all", "hec_set_shift", "hec_shift_rows", "hec_set_fast_tables", "hec_count_histogram",
     "hec_set_stream", "hec_set_regime", "hec_set_eval", "hec_last_count_stats", "hec_launch_count", "hec_gather_bench",
     "hec_shutdown",
 ]
@@ -51,7 +51,7 @@ class CountStats(ctypes.Structure):
                 ("launches", ctypes.c_uint32), ("regime", ctypes.c_uint32), ("smem_bytes", ctypes.c_uint32),
                 ("grid", ctypes.c_uint32), ("block", ctypes.c_uint32), ("chains_per_lane", ctypes.c_uint32),
                 ("table_mode", ctypes.c_uint32), ("radix_fields", ctypes.c_uint32), ("splits", ctypes.c_uint32),
-                ("fast_fields", ctypes.c_uint32)]
+                ("fast_fields", ctypes.c_uint32), ("chunks", ctypes.c_uint32)]
 
 
 def lib():
@@ -78,6 +78,7 @@ def lib():
             f.restype, f.argtypes = None, [vp, vp]
         L.hec_count.argtypes = [u32, u32, vp, sz, vp, vp]
         L.hec_histogram.argtypes = [vp, vp, sz, u32, vp, vp, sz, ctypes.POINTER(sz)]
+        L.hec_count_histogram.argtypes = [u32, u32, vp, sz, vp, vp, vp, vp, sz, ctypes.POINTER(sz)]
         L.hec_histogram_merge.argtypes = [vp, vp, sz, u32, vp, vp, sz, ctypes.POINTER(sz)]
         L.hec_reduced_total.argtypes = [u32, u32, u32, ctypes.POINTER(ctypes.c_uint64)]
         L.hec_reduced_rows.argtypes = [u32, u32, u32, ctypes.c_uint64, sz, vp, vp]
@@ -259,6 +260,54 @@ def histogram(counts, mask=None, _weights=None):
         _check(rc)
     _cap_hint[key] = m.value
     return tup[: m.value], mult[: m.value]
+
+
+def count_histogram(q: int, g: int, coeffs, out_counts=None, out_squarefree=None, want_squarefree: bool = True,
+                    out_tuples=None, out_mult=None):
+    """hec_count_histogram: one pass of the whole hot path in one library call.  Returns (counts, squarefree, tuples,
+    multiplicities), all of the same kind as coeffs (numpy: host; torch CUDA tensor: device).  out_tuples [cap][g] /
+    out_mult [cap]: caller-owned result buffers (e.g. pinned host memory), used when their capacity suffices."""
+    n = int(coeffs.shape[0])
+    if tuple(coeffs.shape[1:]) != (2 * g + 3,):
+        raise ValueError("coeffs must be [n][2g+3]")
+    dev = _is_torch(coeffs)
+    if dev:
+        import torch
+        if coeffs.dtype not in (torch.uint16, torch.int16) or not coeffs.is_contiguous():
+            raise ValueError("device coeffs must be a contiguous uint16/int16 tensor")
+        if out_counts is None:
+            out_counts = torch.empty((n, g), dtype=torch.int32, device=coeffs.device)
+        if out_squarefree is None and want_squarefree:
+            out_squarefree = torch.empty((n,), dtype=torch.uint8, device=coeffs.device)
+    else:
+        coeffs = np.ascontiguousarray(coeffs, dtype=np.uint16)
+        if out_counts is None:
+            out_counts = np.empty((n, g), dtype=np.uint32)
+        if out_squarefree is None and want_squarefree:
+            out_squarefree = np.empty((n,), dtype=np.uint8)
+
+    def buffers(cap):
+        if dev:
+            return (torch.empty((cap, g), dtype=torch.int32, device=coeffs.device),
+                    torch.empty((cap,), dtype=torch.int64, device=coeffs.device))
+        return np.empty((cap, g), dtype=np.uint32), np.empty((cap,), dtype=np.uint64)
+
+    key = (n, g, "count_histogram", q)
+    hint = _cap_hint.get(key)
+    cap = min(n, hint + hint // 4 + 1024) if hint is not None else min(n, 1 << 20)
+    if out_tuples is not None and out_mult is not None:
+        tup, mult, cap = out_tuples, out_mult, min(int(out_tuples.shape[0]), int(out_mult.shape[0]))
+    else:
+        tup, mult = buffers(cap)
+    m = ctypes.c_size_t(0)
+    rc = lib().hec_count_histogram(q, g, _ptr(coeffs), n, _ptr(out_counts), _ptr(out_squarefree), _ptr(tup), _ptr(mult),
+                                   cap, ctypes.byref(m))
+    if rc == HEC_ERR_CAPACITY:          # counts and flags are complete: only the histogram is repeated, at the right size
+        tup, mult = buffers(m.value)
+        rc = lib().hec_histogram(_ptr(out_counts), _ptr(out_squarefree), n, g, _ptr(tup), _ptr(mult), m.value, ctypes.byref(m))
+    _check(rc)
+    _cap_hint[key] = m.value
+    return out_counts, out_squarefree, tup[: m.value], mult[: m.value]
 
 
 def histogram_merge(tuples, mult):

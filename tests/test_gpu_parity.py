@@ -470,3 +470,78 @@ def test_shift_prepass_off_agrees(torch_cuda, cid):
         hec.set_shift(True)
     on = _gpu_count(torch_cuda, cfg.q, cfg.g, rows)
     assert (on[0] == off[0]).all() and (on[1] == off[1]).all()
+
+
+# ------------------------------------------------------------------------------------------ host-buffer pipeline, fused call
+
+def test_host_pointer_pipeline_large_batch(torch_cuda):
+    """Host buffers from 2^20 rows on go through the library's chunked copy/compute pipeline (hec.h: hec_count): the
+    outputs must equal those of the device-pointer call on the same rows, row for row, for 2^22 rows of config 4 and all of
+    config 2 -- with pinned and with pageable host memory -- and an invalid row must be reported at its index in the batch."""
+    if torch_cuda.eval_scheme != "auto":
+        pytest.skip("one scheme is enough: the pipeline is host-side")
+    torch = torch_cuda
+    for cid, n in [(4, 1 << 22), (2, 1 << 20)]:
+        cfg = W.CONFIGS[cid]
+        rows = W.generate(cfg, 0, n)
+        d_cnt, d_sf = hec.count(cfg.q, cfg.g, _dev(torch, rows))
+        assert hec.last_count_stats()["chunks"] == 1
+        ref_cnt, ref_sf = d_cnt.cpu().numpy().view(np.uint32), d_sf.cpu().numpy()
+        h_cnt, h_sf = hec.count(cfg.q, cfg.g, rows)                          # pageable
+        assert hec.last_count_stats()["chunks"] == 4
+        assert (h_cnt == ref_cnt).all() and (h_sf == ref_sf).all()
+        p_rows = torch.from_numpy(rows.view(np.int16)).pin_memory()
+        p_cnt = torch.empty((n, cfg.g), dtype=torch.int32).pin_memory()
+        p_sf = torch.empty((n,), dtype=torch.uint8).pin_memory()
+        hec.count(cfg.q, cfg.g, p_rows.numpy().view(np.uint16), p_cnt.numpy().view(np.uint32), p_sf.numpy())
+        assert (p_cnt.numpy().view(np.uint32) == ref_cnt).all() and (p_sf.numpy() == ref_sf).all()
+    bad = rows.copy()
+    bad[3 * (n // 4) + 17, 2] = cfg.q                                        # in the last chunk
+    with pytest.raises(hec.HecError) as e:
+        hec.count(cfg.q, cfg.g, bad)
+    assert e.value.code == hec.HEC_ERR_COEFF_RANGE and e.value.index == 3 * (n // 4) + 17
+    cnt, _ = hec.count(cfg.q, cfg.g, rows[:100])                             # still works
+    assert (cnt == ref_cnt[:100]).all()
+
+
+@pytest.mark.parametrize("cid,n", [(1, None), (2, 70000), (2, 1 << 20), (5, 3000)])
+def test_count_histogram_fused_call(torch_cuda, cid, n):
+    """hec_count_histogram = hec_count + hec_histogram of the squarefree rows, host and device pointers, incl. the
+    capacity retry of the binding and the pipelined host path (2^20 rows)."""
+    torch = torch_cuda
+    cfg = W.CONFIGS[cid]
+    rows = W.generate(cfg, 0, n)
+    cnt, sf = _gpu_count(torch, cfg.q, cfg.g, rows)
+    otup, omult = O.histogram(cnt, sf)
+    hec._cap_hint.clear()
+    for kind in ("host", "device", "host"):                                  # the second host call uses the capacity hint
+        if kind == "host":
+            c, s, t, m = hec.count_histogram(cfg.q, cfg.g, rows)
+        else:
+            c, s, t, m = (x.cpu().numpy() for x in hec.count_histogram(cfg.q, cfg.g, _dev(torch, rows)))
+        assert (c.view(np.uint32) == cnt).all() and (s == sf).all()
+        assert t.shape == otup.shape and (t.view(np.uint32) == otup).all() and (m.view(np.uint64) == omult).all()
+    # every row (no flag wanted)
+    c, s, t, m = hec.count_histogram(cfg.q, cfg.g, rows, want_squarefree=False)
+    atup, amult = O.histogram(cnt, None)
+    assert s is None and (t == atup).all() and (m == amult).all()
+
+
+@pytest.mark.parametrize("cid,n", [(2, 12000), (4, 12000), (5, 12000), (3, 10000)])
+def test_fast_tables_off_agrees(torch_cuda, cid, n):
+    """hec_set_fast_tables: the transposed chain-start table and the tabulated set-up change no count."""
+    cfg = W.CONFIGS[cid]
+    rows = np.concatenate([W.generate(cfg, 12345, n), W.edge_rows(cfg.q, cfg.g)])
+    on = _gpu_count(torch_cuda, cfg.q, cfg.g, rows)
+    st = hec.last_count_stats()
+    if torch_cuda.eval_scheme == "auto":
+        assert st["fast_fields"] != 0
+    else:
+        assert st["fast_fields"] == 0
+    try:
+        hec.set_fast_tables(False)
+        off = _gpu_count(torch_cuda, cfg.q, cfg.g, rows)
+        assert hec.last_count_stats()["fast_fields"] == 0
+    finally:
+        hec.set_fast_tables(True)
+    assert (on[0] == off[0]).all() and (on[1] == off[1]).all()
