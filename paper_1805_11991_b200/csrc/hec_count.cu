@@ -153,11 +153,12 @@ __global__ void __launch_bounds__(256) hec_shift_kernel(const HecShiftParams P) 
         if (c[j]) { nz |= 1u << j; d = (int)j; }
     }
     auto all_present = [&](uint32_t mask) {
+        if (P.dense) return d >= 0 && (mask & ((2u << d) - 1u)) == (2u << d) - 1u;
         uint32_t m = mask;
         for (uint32_t s = P.R; s < P.ncoef; s += P.R) m |= mask >> s;
         return (m & ((1u << P.R) - 1u)) == (1u << P.R) - 1u;
     };
-    bool done = !ok || d < (int)P.ncoef - 2 || d + 1 < (int)P.R || all_present(nz);
+    bool done = !ok || d < (int)P.ncoef - 2 || (!P.dense && d + 1 < (int)P.R) || all_present(nz);
     if (!done) {
         for (int j = 0; j <= d; j++) a[j] = c[j] ? __ldg(P.emb + c[j]) : ZERO;
         for (int s = 0; s < kShiftTries && s < (int)P.M && !done; s++) {
@@ -291,6 +292,17 @@ void fill_fast_tables(const hec_field &F, uint32_t M, uint32_t R, uint32_t D, ui
     }
 }
 
+// Packed parity table of a field (hec_radix.cuh: network_mono): entry n = parity(Z[n]) | parity(Z[n + M/2]) << 1, four per byte.
+uint32_t parity_table_bytes(uint32_t M) { return align16((M + 3u) / 4u); }
+void fill_parity_table(const hec_field &F, uint32_t M, uint8_t *out) {
+    const uint32_t h = M >> 1;
+    std::fill(out, out + parity_table_bytes(M), (uint8_t)0);
+    for (uint32_t n = 0; n < M; n++) {
+        const uint32_t bits = (zech0(F, M, n) & 1u) | ((zech0(F, M, n + h >= M ? n + h - M : n + h) & 1u) << 1);
+        out[n >> 2] |= (uint8_t)(bits << ((n & 3u) * 2u));
+    }
+}
+
 // Smallest field for which the half-table step is valid: the lane term must stay below h (kernel comment).
 constexpr uint32_t kHalfMinM = 1u << 13;
 constexpr uint32_t kHalf24MaxM = 1u << 22;      // |Z - h| < 127 * 65536
@@ -399,8 +411,16 @@ int build_plan(LibState &S, uint32_t q, uint32_t g, int regime, int eval, Device
     // fast tables (radix_fast_x) for the PAIR16 fields, the largest field first, as long as one launch still holds everything
     std::vector<uint32_t> radix_of(g, 0), fastb(g, 0);
     for (uint32_t k = 1; k <= g; k++) radix_of[k - 1] = radix ? pick_radix(geom[k - 1].M, eval, mode[k - 1], g) : 0u;
+    // monomial classes on the top field (radix_mono8_x): at most 8 coefficients, 8 | M, 32-bit half table, room for the parity table
+    uint32_t ptb = 0;
+    if (radix && S.fast_enabled && (eval == HEC_EVAL_AUTO || eval == HEC_EVAL_RADIX8) && mode[g - 1] == HEC_TAB_RHALF32 && D + 1 <= 8 &&
+        geom[g - 1].M % 8u == 0 && geom[g - 1].M >= 4096u) {
+        uint64_t total = parity_table_bytes(geom[g - 1].M);
+        for (uint32_t k = 1; k <= g; k++) total += bytes[k - 1];
+        if (total <= budget) { ptb = parity_table_bytes(geom[g - 1].M); radix_of[g - 1] = 8u; }
+    }
     if (radix && S.fast_enabled) {
-        uint64_t total = 0;
+        uint64_t total = ptb;
         for (uint32_t k = 1; k <= g; k++) total += bytes[k - 1];
         for (uint32_t k = g; k >= 1; k--) {
             if (mode[k - 1] != HEC_TAB_PAIR16) continue;
@@ -415,9 +435,10 @@ int build_plan(LibState &S, uint32_t q, uint32_t g, int regime, int eval, Device
     {
         Group cur{1, 0, 0};
         for (uint32_t k = 1; k <= g; k++) {
-            if (cur.k_hi >= cur.k_lo && cur.smem + bytes[k - 1] + fastb[k - 1] > budget) { groups.push_back(cur); cur = Group{k, 0, 0}; }
+            const uint32_t extra = fastb[k - 1] + (k == g ? ptb : 0u);
+            if (cur.k_hi >= cur.k_lo && cur.smem + bytes[k - 1] + extra > budget) { groups.push_back(cur); cur = Group{k, 0, 0}; }
             cur.k_hi = k;
-            cur.smem += bytes[k - 1] + fastb[k - 1];
+            cur.smem += bytes[k - 1] + extra;
             if (mode[k - 1] != base_mode) { groups.push_back(cur); cur = Group{k + 1, 0, 0}; }   // only the top of a launch may differ
         }
         if (cur.k_hi >= cur.k_lo) groups.push_back(cur);
@@ -438,7 +459,7 @@ int build_plan(LibState &S, uint32_t q, uint32_t g, int regime, int eval, Device
             fd.lane_cap = std::min<uint32_t>(32u * U, t.M);
             fd.smem_off = so; fd.smem_off2 = 0; fd.gtab = nullptr;
             fd.radix = radix_of[k - 1];
-            fd.fast_off = 0; fd.fast_row = 0;
+            fd.fast_off = 0; fd.fast_row = 0; fd.pt_off = 0;
             uint8_t *dst = host.data() + blob_off[gi] + so;
             switch (mode[k - 1]) {
                 case HEC_TAB_EXT16:
@@ -463,6 +484,10 @@ int build_plan(LibState &S, uint32_t q, uint32_t g, int regime, int eval, Device
                     break;
                 case HEC_TAB_RHALF32:
                     fill_rhalf32(*fields[k - 1], t.M, reinterpret_cast<uint32_t *>(dst));
+                    if (k == g && ptb) {
+                        fd.pt_off = so + bytes[k - 1];
+                        fill_parity_table(*fields[k - 1], t.M, dst + bytes[k - 1]);
+                    }
                     break;
                 case HEC_TAB_RHALF17: {
                     const uint32_t lo_bytes = align16(((t.M >> 1) + 1u) * 2u);
@@ -473,7 +498,7 @@ int build_plan(LibState &S, uint32_t q, uint32_t g, int regime, int eval, Device
                 default:
                     break;
             }
-            so += bytes[k - 1] + fastb[k - 1];
+            so += bytes[k - 1] + fastb[k - 1] + (k == g ? ptb : 0u);
         }
     }
     for (uint32_t k = 1; k <= g; k++) {
@@ -552,6 +577,8 @@ int build_plan(LibState &S, uint32_t q, uint32_t g, int regime, int eval, Device
     plan->sq_antilog = reinterpret_cast<const uint32_t *>(base + sqa_off);
     // the shift pre-pass pays where the dominant (largest) field has R >= 4 and the rows have at least R coefficients
     plan->shift_R = (radix && plan->f[g - 1].radix >= 4u && 2 * g + 2 >= plan->f[g - 1].radix) ? plan->f[g - 1].radix : 0u;
+    plan->shift_dense = ptb != 0;                    // monomial classes: every coefficient up to the degree nonzero
+    if (plan->shift_dense) plan->shift_R = 8u;
     plan->d_part_codes = reinterpret_cast<const unsigned long long *>(base + part_off);
     plan->n_parts = (uint32_t)parts.size();
 
@@ -576,6 +603,7 @@ int run_shift(LibState &S, const DevicePlan &plan, const uint16_t *d_rows, size_
     HecShiftParams H;
     H.coeffs = d_rows; H.out = d_out; H.n = n; H.q = plan.q; H.M = plan.q - 1; H.ncoef = ncoef;
     H.R = plan.shift_R ? plan.shift_R : 2u;
+    H.dense = plan.shift_dense ? 1u : 0u;
     H.zech = plan.sq_zech; H.emb = plan.sq_emb; H.antilog = plan.sq_antilog;
     hec_shift_kernel<<<(unsigned)((n + 255) / 256), 256, 0, S.stream>>>(H);
     hec_launch_counter::value++;

@@ -55,6 +55,7 @@ struct DevicePlan {
     // squarefree
     const uint32_t *sq_zech = nullptr, *sq_emb = nullptr, *sq_antilog = nullptr;
     uint32_t shift_R = 0;             // hec_shift_kernel's target radix (0: no pre-pass for this plan)
+    bool shift_dense = false;         // the pre-pass asks for every coefficient up to the degree to be nonzero
     const unsigned long long *d_part_codes = nullptr;   // lambda: packed partitions of 2g+2 in index order
     uint32_t n_parts = 0;
     unsigned long long *d_err = nullptr;
@@ -436,7 +437,17 @@ __global__ void __launch_bounds__(kThreads, 1) hec_count_radix_kernel(const __gr
                 radix_dispatch<D, hec_radix::ArPacked, ORBIT, !SPLIT && !ORBIT>(F, pol, smem_base, lane, nz, lcj, scratch, part, splits, n_sq, n_zero);
             } else if constexpr (TOP == HEC_TAB_RHALF32) {
                 const hec_radix::HalfS32 pol{smem_base + F.smem_off, smem_base + F.smem_off + 4u * (M >> 1)};
-                radix_dispatch<D, hec_radix::ArScalar, ORBIT, false>(F, pol, smem_base, lane, nz, lcj, scratch, part, splits, n_sq, n_zero);
+                bool mono = false;
+                if constexpr (!SPLIT && !ORBIT && D + 1 <= 8) {           // monomial classes on a field with a parity table
+                    const uint32_t dense = (nz >> D) ? (1u << (D + 1)) - 1u : (1u << D) - 1u;
+                    if (F.pt_off && nz == dense) {
+                        const uint2 res = (nz >> D) ? hec_radix::radix_mono8_x<D, D + 1>(pol, smem_base + F.pt_off, M, lane, nz, lcj, scratch)
+                                                    : hec_radix::radix_mono8_x<D, D>(pol, smem_base + F.pt_off, M, lane, nz, lcj, scratch);
+                        n_sq = res.x; n_zero = res.y;
+                        mono = true;
+                    }
+                }
+                if (!mono) radix_dispatch<D, hec_radix::ArScalar, ORBIT, false>(F, pol, smem_base, lane, nz, lcj, scratch, part, splits, n_sq, n_zero);
             } else if constexpr (TOP == HEC_TAB_RHALF17) {
                 const hec_radix::HalfS17 pol{smem_base + F.smem_off, smem_base + F.smem_off + 2u * (M >> 1), smem_base + F.smem_off2};
                 radix_dispatch<D, hec_radix::ArScalar, ORBIT, false>(F, pol, smem_base, lane, nz, lcj, scratch, part, splits, n_sq, n_zero);
@@ -509,7 +520,7 @@ int launch_count(LibState &S, const DevicePlan &plan, HecCountParams P) {
         if (plan.radix)
             for (uint32_t k = L.k_lo; k <= L.k_hi; k++) {
                 S.stats.radix_fields |= plan.f[k - 1].radix << (4u * (k - 1));
-                if (plan.f[k - 1].fast_off && P.splits == 1u && !plan.f[k - 1].orb[0]) S.stats.fast_fields |= 1u << (k - 1);
+                if ((plan.f[k - 1].fast_off || plan.f[k - 1].pt_off) && P.splits == 1u && !plan.f[k - 1].orb[0]) S.stats.fast_fields |= 1u << (k - 1);
             }
     }
     return HEC_OK;

@@ -42,6 +42,8 @@ struct HecFieldDev {
     uint32_t radix;      // radix evaluation: R in {2, 4, 8}, the largest with R | M; 0 for the Horner tables
     uint32_t fast_off;   // PAIR16: byte offset inside the blob of the field's fast tables (hec_radix.cuh: radix_fast_x), 0: none
     uint32_t fast_row;   // bytes per row of the transposed Zech table inside them
+    uint32_t pt_off;     // RHALF32 top field with monomial classes (hec_radix.cuh: radix_mono8_x): byte offset of the packed
+                         // parity table (2 bits per n: parity of Z[n], of Z[n + M/2]; four entries per byte), 0: none
     const uint32_t *orb[3]; // HEC_EVAL_ORBIT: Frobenius-orbit representatives of the cosets of mu_R, R = 2, 4, 8 (hec_radix.cuh)
     uint32_t n_orb[3];
     const uint32_t *gtab;   // GLOBAL32: extended table in global memory; GPAIR64: the pair table
@@ -73,6 +75,7 @@ struct HecShiftParams {
     uint32_t q, M;                 // M = q - 1
     uint32_t ncoef;                // 2g+3
     uint32_t R;                    // target radix (4 or 8)
+    uint32_t dense;                // 1: a row qualifies only if EVERY coefficient up to its degree is nonzero (monomial classes)
     const uint32_t *zech;          // F_q: M entries, paper's convention (sentinel M)
     const uint32_t *emb;           // q entries: log in F_q or HEC_LOG_ZERO
     const uint32_t *antilog;       // M entries: alpha^i in the integer encoding

@@ -679,6 +679,113 @@ __device__ __noinline__ uint2 radix_fast_x(const PairS16 pol, const uint32_t ft,
 }
 
 // ---------------------------------------------------------------------------------------------------------
+// Monomial classes (genus <= 2 on a field with 8 | M, i.e. every F_{q^2}: D + 1 <= 8 terms, at most one per residue
+// class mod 8): G_r = c_r x^r needs no chain at all, so the 8 points of a coset cost the butterflies only -- NP - 4 + 8
+// pair lookups for NP = deg f + 1 nonzero coefficients against 3 chain + 4 pair lookups per FOUR points at R = 4.  The
+// network is specialised at compile time on the present classes 0 .. NP-1 (the shift pre-pass makes every coefficient
+// up to the degree nonzero).  For the half-table layout, where a pair costs two loads and a fold, the LAST stage -- which
+// only classifies -- reads a 2-bit entry (parity of Z[n], parity of Z[n + M/2]) from a packed parity table instead
+// (tp: its shared byte address, four entries per byte); zero sums are seen from n itself (n = 0 or M/2).
+// One coset per lane and pass (scalar arithmetic: these fields have more than 2^16 elements).
+// ---------------------------------------------------------------------------------------------------------
+template <int R, int NP, typename Pol>
+__device__ __forceinline__ void network_mono(const ArScalar &ar, const Pol &pol, const uint32_t tp, const uint32_t unit,
+                                             uint32_t (&v)[R], uint32_t &ps, uint32_t &mn) {
+    int pend[R];
+    bool pres[R];
+#pragma unroll
+    for (int i = 0; i < R; i++) { pend[i] = 0; pres[i] = i < NP; }
+#pragma unroll
+    for (int H = R / 2; H >= 1; H >>= 1) {
+#pragma unroll
+        for (int blk = 0; blk < R; blk += 2 * H) {
+#pragma unroll
+            for (int j = 0; j < H; j++) {
+                const int i1 = blk + j, i2 = i1 + H;
+                const int oe = (pend[i2] - pend[i1]) & (R - 1);
+                pend[i2] = (pend[i1] + j * (R / (2 * H))) & (R - 1);
+                const bool pa = pres[i1], pb = pres[i2];              // compile-time after unrolling
+                if (pa && pb) {
+                    uint32_t n = ar.subm(v[i2], v[i1]);
+                    if (oe) n = ar.wrap(n + (uint32_t)oe * unit);
+                    const uint32_t a = v[i1];
+                    if (H > 1) {
+                        uint32_t za, zs;
+                        ar.lookup_pair(pol, n, za, zs, mn);
+                        v[i1] = ar.wrap(a + za);
+                        v[i2] = ar.wrap(a + zs);
+                    } else {
+                        mn = min(mn, min(n, n - ar.h));               // 0 iff one of the two sums vanishes
+                        const uint32_t p = lds_u8(tp + (n >> 2)) >> ((n & 3u) << 1);
+                        ps += ((a ^ p) & 1u) + ((a ^ (p >> 1)) & 1u);
+                    }
+                } else if (pa) {                                      // b = 0: both outputs are a
+                    if (H > 1) v[i2] = v[i1];
+                    else ps += 2u * (v[i1] & 1u);
+                } else if (pb) {                                      // a = 0: w b and -w b
+                    uint32_t t = v[i2];
+                    if (oe) t = ar.wrap(t + (uint32_t)oe * unit);
+                    const uint32_t u = ar.wrap(t + unit * (R / 2));
+                    if (H > 1) { v[i1] = t; v[i2] = u; }
+                    else ps += (t & 1u) + (u & 1u);
+                }
+                if (pa || pb) { pres[i1] = true; pres[i2] = true; }
+            }
+        }
+    }
+}
+
+template <int D, int NP, typename Pol>
+__device__ __noinline__ uint2 radix_mono8_x(const Pol pol, const uint32_t tp, const uint32_t M, const uint32_t lane,
+                                            const uint32_t nz, const uint32_t lcj, volatile uint32_t *scratch) {
+    constexpr int R = 8;
+    static_assert(NP <= R && NP >= R / 2, "monomial classes: one term per class, classes 0 .. NP-1");
+    const ArScalar ar(M);
+    const uint32_t S = M >> 3, unit = S;
+
+    __syncwarp();
+    if (lane <= (uint32_t)D) scratch[lane] = lcj;
+    __syncwarp();
+    uint32_t kc[NP];                                   // log G_r = log c_r + r n for this lane's coset n = base + lane
+#pragma unroll
+    for (int r = 0; r < NP; r++) kc[r] = ar.wrap(__shfl_sync(0xffffffffu, lcj, r) + (uint32_t)r * lane);     // r lane < 8 * 32 <= M
+
+    uint32_t acc = 0, pushed = 0, qn = 0, nz_exact = 0, odd_exact = 0;
+    for (uint32_t base = 0; base < S; base += 32u) {
+        uint32_t v[R];
+        uint32_t mn = ar.mn_init(), ps = 0;
+#pragma unroll
+        for (int r = 0; r < R; r++) v[r] = r < NP ? kc[r] : 0u;
+#pragma unroll
+        for (int r = 1; r < NP; r++) kc[r] = ar.wrap(kc[r] + 32u * (uint32_t)r);
+        network_mono<R, NP>(ar, pol, tp, unit, v, ps, mn);
+        const bool z = mn == 0u;
+        if (__any_sync(0xffffffffu, z) || base + 32u > S) {              // rare: a zero somewhere, or the ragged last pass
+            const bool valid = base + lane < S, flag = valid && z;
+            const uint32_t bal = __ballot_sync(0xffffffffu, flag);
+            if (bal) {
+                if (flag) { scratch[16 + qn + __popc(bal & ((1u << lane) - 1u))] = base + lane; pushed++; }
+                qn += __popc(bal);
+                __syncwarp();
+                if (qn >= 32u) {
+                    exact_queue<D, R>(pol, M, nz, scratch, qn, lane, nz_exact, odd_exact);
+                    qn = 0;
+                    __syncwarp();
+                }
+            }
+            ps = (valid && !flag) ? ps : 0u;
+        }
+        acc += ps;
+    }
+    exact_queue<D, R>(pol, M, nz, scratch, qn, lane, nz_exact, odd_exact);
+    __syncwarp();
+    const uint32_t n_valid = lane < S ? (S - lane + 31u) / 32u : 0u;
+    const uint32_t n_nz = (n_valid - pushed) * R + nz_exact;            // every value of an unflagged coset is nonzero
+    const uint32_t n_zero = n_valid * R - n_nz;
+    return make_uint2(n_nz - (acc + odd_exact), n_zero);
+}
+
+// ---------------------------------------------------------------------------------------------------------
 // The same, over ONE representative per Frobenius orbit of cosets (HEC_EVAL_ORBIT; not in the
 // paper).  f has coefficients in F_q, so f(x^q) = f(x)^q: x and x^q give values that vanish together and are squares
 // together.  On logs x -> x^q is n -> q n mod M; it permutes the cosets of mu_R (q is odd, R a power of two), acting on
