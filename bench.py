@@ -86,8 +86,10 @@ def executed_loads(cfg: W.Workload, rows: np.ndarray, stats: dict) -> dict:
         Rf = (stats["radix_fields"] >> (4 * (k - 1))) & 15
         mode = top_mode if k == cfg.g else (4 if Rf else 1)
         single, pair = LOADS[mode]
-        if Rf == 0:
-            random += int((nzm.sum(axis=1) - 1).sum()) * M * single
+        if Rf == 0:                                          # Horner: the first link of every chain starts from W = log 1 = 0 on
+            nnz = nzm.sum(axis=1)                            # all lanes, so its index is uniform + gap * lane: conflict-free
+            conflict_free += int((nnz >= 2).sum()) * M * single
+            random += int(np.maximum(nnz - 2, 0).sum()) * M * single
             continue
         if M <= DIRECT_MAX_M and mode == 4 and stats.get("eval") != "orbit":
             random += int(nzm.sum()) * M
@@ -95,6 +97,14 @@ def executed_loads(cfg: W.Workload, rows: np.ndarray, stats: dict) -> dict:
         fast = bool((stats.get("fast_fields", 0) >> (k - 1)) & 1)
         todo = np.ones(n, dtype=bool)
         R = Rf
+        if fast and mode == 5 and k == cfg.g and Rf == 8 and ncoef <= 8:
+            # monomial classes (radix_mono8_x): rows with every coefficient up to the degree nonzero run NP - 4 + 4 pair
+            # lookups (two loads each) and four parity lookups (one load) per coset of 8 points
+            deg = ncoef - 1 - (~nzm[:, ::-1]).cumprod(axis=1).sum(axis=1)
+            dense = nzm.sum(axis=1) == deg + 1
+            NP = deg[dense] + 1
+            random += int((2 * NP + 4).sum()) * (M // 8)
+            todo &= ~dense
         while R >= 2:
             present = np.zeros((n, R), dtype=bool)
             for r in range(R):
