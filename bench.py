@@ -97,13 +97,14 @@ def executed_loads(cfg: W.Workload, rows: np.ndarray, stats: dict) -> dict:
         fast = bool((stats.get("fast_fields", 0) >> (k - 1)) & 1)
         todo = np.ones(n, dtype=bool)
         R = Rf
-        if fast and mode == 5 and k == cfg.g and Rf == 8 and ncoef <= 8:
-            # monomial classes (radix_mono8_x): rows with every coefficient up to the degree nonzero run NP - 4 + 4 pair
-            # lookups (two loads each) and four parity lookups (one load) per coset of 8 points
+        if fast and Rf == 8 and ncoef <= 8 and ((mode == 5 and k == cfg.g) or mode == 4):
+            # monomial classes (radix_mono8_x / radix_mono8_packed_x): rows with every coefficient up to the degree nonzero
+            # run NP - 4 + 8 butterflies per coset of 8 points and no chain lookup.  Pair table: one load each; 32-bit half
+            # table: two loads each except the last four, which read the parity table (one load)
             deg = ncoef - 1 - (~nzm[:, ::-1]).cumprod(axis=1).sum(axis=1)
             dense = nzm.sum(axis=1) == deg + 1
             NP = deg[dense] + 1
-            random += int((2 * NP + 4).sum()) * (M // 8)
+            random += int(((2 * NP + 4) if mode == 5 else (NP + 4)).sum()) * (M // 8)
             todo &= ~dense
         while R >= 2:
             present = np.zeros((n, R), dtype=bool)

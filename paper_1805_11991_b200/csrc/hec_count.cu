@@ -577,7 +577,8 @@ int build_plan(LibState &S, uint32_t q, uint32_t g, int regime, int eval, Device
     plan->sq_antilog = reinterpret_cast<const uint32_t *>(base + sqa_off);
     // the shift pre-pass pays where the dominant (largest) field has R >= 4 and the rows have at least R coefficients
     plan->shift_R = (radix && plan->f[g - 1].radix >= 4u && 2 * g + 2 >= plan->f[g - 1].radix) ? plan->f[g - 1].radix : 0u;
-    plan->shift_dense = ptb != 0;                    // monomial classes: every coefficient up to the degree nonzero
+    // monomial classes (radix_mono8_x / radix_mono8_packed_x): every coefficient up to the degree nonzero
+    plan->shift_dense = ptb != 0 || (radix && D + 1 <= 8 && plan->f[g - 1].radix == 8u && plan->f[g - 1].fast_off != 0);
     if (plan->shift_dense) plan->shift_R = 8u;
     plan->d_part_codes = reinterpret_cast<const unsigned long long *>(base + part_off);
     plan->n_parts = (uint32_t)parts.size();

@@ -367,6 +367,15 @@ __device__ __forceinline__ void radix_dispatch(const HecFieldDev &F, const Pol p
     if constexpr (FAST) {
         if (F.fast_off) {
             const uint32_t ft = smem_base + F.fast_off;
+            if constexpr (D + 1 <= 8) {                   // monomial classes (genus <= 2): R = 8 without chains
+                const uint32_t dense = (nz >> D) ? (1u << (D + 1)) - 1u : (1u << D) - 1u;
+                if (R == 8 && nz == dense) {
+                    const uint2 res = (nz >> D) ? radix_mono8_packed_x<D, D + 1>(pol, ft, M, lane, nz, lcj, scratch)
+                                                : radix_mono8_packed_x<D, D>(pol, ft, M, lane, nz, lcj, scratch);
+                    n_sq = res.x; n_zero = res.y;
+                    return;
+                }
+            }
             if (R == 8) { if (all_classes_present<D, 8>(nz)) { const uint2 res = radix_fast_x<D, 8>(pol, ft, F.fast_row, M, lane, nz, lcj, scratch); n_sq = res.x; n_zero = res.y; return; } }
             else if (R == 4) { if (all_classes_present<D, 4>(nz)) { const uint2 res = radix_fast_x<D, 4>(pol, ft, F.fast_row, M, lane, nz, lcj, scratch); n_sq = res.x; n_zero = res.y; return; } }
             else if (all_classes_present<D, 2>(nz)) { const uint2 res = radix_fast_x<D, 2>(pol, ft, F.fast_row, M, lane, nz, lcj, scratch); n_sq = res.x; n_zero = res.y; return; }

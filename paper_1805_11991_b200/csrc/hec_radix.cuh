@@ -688,8 +688,8 @@ __device__ __noinline__ uint2 radix_fast_x(const PairS16 pol, const uint32_t ft,
 // (tp: its shared byte address, four entries per byte); zero sums are seen from n itself (n = 0 or M/2).
 // One coset per lane and pass (scalar arithmetic: these fields have more than 2^16 elements).
 // ---------------------------------------------------------------------------------------------------------
-template <int R, int NP, typename Pol>
-__device__ __forceinline__ void network_mono(const ArScalar &ar, const Pol &pol, const uint32_t tp, const uint32_t unit,
+template <int R, int NP, bool PT, typename Ar, typename Pol>
+__device__ __forceinline__ void network_mono(const Ar &ar, const Pol &pol, const uint32_t tp, const uint32_t unit,
                                              uint32_t (&v)[R], uint32_t &ps, uint32_t &mn) {
     int pend[R];
     bool pres[R];
@@ -707,27 +707,33 @@ __device__ __forceinline__ void network_mono(const ArScalar &ar, const Pol &pol,
                 const bool pa = pres[i1], pb = pres[i2];              // compile-time after unrolling
                 if (pa && pb) {
                     uint32_t n = ar.subm(v[i2], v[i1]);
-                    if (oe) n = ar.wrap(n + (uint32_t)oe * unit);
+                    if (oe) n = ar.wrap(n + ar.rep((uint32_t)oe * unit));
                     const uint32_t a = v[i1];
-                    if (H > 1) {
+                    if (H > 1 || !PT) {
                         uint32_t za, zs;
                         ar.lookup_pair(pol, n, za, zs, mn);
-                        v[i1] = ar.wrap(a + za);
-                        v[i2] = ar.wrap(a + zs);
+                        if (H > 1) {
+                            v[i1] = ar.wrap(a + za);
+                            v[i2] = ar.wrap(a + zs);
+                        } else {
+                            ps += ar.parity2(a, za, zs);
+                        }
                     } else {
-                        mn = min(mn, min(n, n - ar.h));               // 0 iff one of the two sums vanishes
-                        const uint32_t p = lds_u8(tp + (n >> 2)) >> ((n & 3u) << 1);
-                        ps += ((a ^ p) & 1u) + ((a ^ (p >> 1)) & 1u);
+                        if constexpr (PT) {                           // scalar arithmetic only
+                            mn = min(mn, min(n, n - ar.h));           // 0 iff one of the two sums vanishes
+                            const uint32_t p = lds_u8(tp + (n >> 2)) >> ((n & 3u) << 1);
+                            ps += ((a ^ p) & 1u) + ((a ^ (p >> 1)) & 1u);
+                        }
                     }
                 } else if (pa) {                                      // b = 0: both outputs are a
                     if (H > 1) v[i2] = v[i1];
-                    else ps += 2u * (v[i1] & 1u);
+                    else ps += 2u * ar.parity1(v[i1]);
                 } else if (pb) {                                      // a = 0: w b and -w b
                     uint32_t t = v[i2];
-                    if (oe) t = ar.wrap(t + (uint32_t)oe * unit);
-                    const uint32_t u = ar.wrap(t + unit * (R / 2));
+                    if (oe) t = ar.wrap(t + ar.rep((uint32_t)oe * unit));
+                    const uint32_t u = ar.wrap(t + ar.rep(unit * (R / 2)));
                     if (H > 1) { v[i1] = t; v[i2] = u; }
-                    else ps += (t & 1u) + (u & 1u);
+                    else ps += ar.parity1(t) + ar.parity1(u);
                 }
                 if (pa || pb) { pres[i1] = true; pres[i2] = true; }
             }
@@ -758,7 +764,7 @@ __device__ __noinline__ uint2 radix_mono8_x(const Pol pol, const uint32_t tp, co
         for (int r = 0; r < R; r++) v[r] = r < NP ? kc[r] : 0u;
 #pragma unroll
         for (int r = 1; r < NP; r++) kc[r] = ar.wrap(kc[r] + 32u * (uint32_t)r);
-        network_mono<R, NP>(ar, pol, tp, unit, v, ps, mn);
+        network_mono<R, NP, true>(ar, pol, tp, unit, v, ps, mn);
         const bool z = mn == 0u;
         if (__any_sync(0xffffffffu, z) || base + 32u > S) {              // rare: a zero somewhere, or the ragged last pass
             const bool valid = base + lane < S, flag = valid && z;
@@ -783,6 +789,68 @@ __device__ __noinline__ uint2 radix_mono8_x(const Pol pol, const uint32_t tp, co
     const uint32_t n_nz = (n_valid - pushed) * R + nz_exact;            // every value of an unflagged coset is nonzero
     const uint32_t n_zero = n_valid * R - n_nz;
     return make_uint2(n_nz - (acc + odd_exact), n_zero);
+}
+
+// The same for PAIR16 fields (genus <= 2, q^2 <= 32768: most of the paper's genus-2 range): packed arithmetic, two cosets per
+// lane and pass; the lanes' first offsets and the per-pass steps come from the field's fast tables (radix_fast_x).
+template <int D, int NP>
+__device__ __noinline__ uint2 radix_mono8_packed_x(const PairS16 pol, const uint32_t ft, const uint32_t M, const uint32_t lane,
+                                                   const uint32_t nz, const uint32_t lcj, volatile uint32_t *scratch) {
+    constexpr int R = 8;
+    static_assert(NP <= R && NP >= R / 2, "monomial classes: one term per class, classes 0 .. NP-1");
+    const ArPacked ar(M);
+    const uint32_t S = M >> 3, unit = S;
+    const uint32_t tLP = ft + 4u * lane, tSE = ft + (uint32_t)(D + 1) * 128u;
+
+    __syncwarp();
+    if (lane <= (uint32_t)D) scratch[lane] = lcj;
+    __syncwarp();
+    uint32_t kc[NP], kinc[NP];
+#pragma unroll
+    for (int r = 0; r < NP; r++) {
+        kc[r] = ar.wrap(ar.rep(__shfl_sync(0xffffffffu, lcj, r)) + lds_u32(tLP + (uint32_t)r * 128u));
+        kinc[r] = lds_u32(tSE + 4u * (uint32_t)r);
+    }
+    uint32_t acc = 0, pushed = 0, qn = 0, nz_exact = 0, odd_exact = 0;
+    for (uint32_t base = 0; base < S; base += 64u) {
+        uint32_t v[R];
+        uint32_t mn = ar.mn_init(), ps = 0;
+#pragma unroll
+        for (int r = 0; r < R; r++) v[r] = r < NP ? kc[r] : 0u;
+#pragma unroll
+        for (int r = 1; r < NP; r++) kc[r] = ar.wrap(kc[r] + kinc[r]);
+        network_mono<R, NP, false>(ar, pol, 0u, unit, v, ps, mn);
+        const bool zany = ((mn - 0x10001u) & ~mn & 0x80008000u) != 0u;
+        if (__any_sync(0xffffffffu, zany) || base + 64u > S) {
+            const bool z0 = (mn & 0xFFFFu) == 0u, z1 = (mn >> 16) == 0u;
+            const bool valid0 = base + lane < S, valid1 = base + lane + 32u < S;
+            const bool flag0 = valid0 && z0, flag1 = valid1 && z1;
+            if (__any_sync(0xffffffffu, flag0 || flag1)) {
+                uint32_t bal = __ballot_sync(0xffffffffu, flag0);
+                if (flag0) { scratch[16 + qn + __popc(bal & ((1u << lane) - 1u))] = base + lane; pushed++; }
+                qn += __popc(bal);
+                bal = __ballot_sync(0xffffffffu, flag1);
+                if (flag1) { scratch[16 + qn + __popc(bal & ((1u << lane) - 1u))] = base + lane + 32u; pushed++; }
+                qn += __popc(bal);
+                __syncwarp();
+                if (qn >= 32u) {
+                    exact_queue<D, R>(pol, M, nz, scratch, qn, lane, nz_exact, odd_exact);
+                    qn = 0;
+                    __syncwarp();
+                }
+            }
+            ps = ar.keep(ps, valid0 && !flag0, valid1 && !flag1);
+        }
+        acc += ps;                                     // <= 8 per half and pass, at most 65 passes: no carry
+    }
+    exact_queue<D, R>(pol, M, nz, scratch, qn, lane, nz_exact, odd_exact);
+    __syncwarp();
+    uint32_t n_valid = 0;
+    if (lane < S) n_valid += (S - lane + 63u) / 64u;
+    if (lane + 32u < S) n_valid += (S - lane - 32u + 63u) / 64u;
+    const uint32_t n_nz = (n_valid - pushed) * R + nz_exact;
+    const uint32_t n_zero = n_valid * R - n_nz;
+    return make_uint2(n_nz - (ar.total(acc) + odd_exact), n_zero);
 }
 
 // ---------------------------------------------------------------------------------------------------------
