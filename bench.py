@@ -127,16 +127,21 @@ def executed_loads(cfg: W.Workload, rows: np.ndarray, stats: dict) -> dict:
                     tl = np.zeros(len(cls), dtype=bool)
                     tl[ok] = cls[idx[ok], nxt[ok]]
                     tlinks += int(tl.sum())
-            pairs = 0
+            pairs = last = 0
             H = R // 2
             while H >= 1:
                 for blk in range(0, R, 2 * H):
                     for j in range(H):
                         a, b = pr[:, blk + j].copy(), pr[:, blk + j + H].copy()
-                        pairs += int((a & b).sum())
+                        if H == 1:
+                            last += int((a & b).sum())
+                        else:
+                            pairs += int((a & b).sum())
                         pr[:, blk + j] = pr[:, blk + j + H] = a | b
                 H //= 2
-            random += ((chain - tlinks) * single + pairs * pair) * (M // R)
+            # half-table layouts with a parity table (fast bit of the top field): the last stage reads one 2-bit entry
+            last_cost = 1 if (fast and mode in (5, 6) and k == cfg.g) else pair
+            random += ((chain - tlinks) * single + pairs * pair + last * last_cost) * (M // R)
             conflict_free += tlinks * (M // R)
             R //= 2
     return {"random": random, "conflict_free": conflict_free}

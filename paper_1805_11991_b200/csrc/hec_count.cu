@@ -412,12 +412,19 @@ int build_plan(LibState &S, uint32_t q, uint32_t g, int regime, int eval, Device
     std::vector<uint32_t> radix_of(g, 0), fastb(g, 0);
     for (uint32_t k = 1; k <= g; k++) radix_of[k - 1] = radix ? pick_radix(geom[k - 1].M, eval, mode[k - 1], g) : 0u;
     // monomial classes on the top field (radix_mono8_x): at most 8 coefficients, 8 | M, 32-bit half table, room for the parity table
+    // Packed parity table of the top field (half-table layouts: the classifying last stage reads it instead of the pair), if it fits.
+    // With it, a 32-bit half table with at most 8 coefficients and 8 | M runs the monomial-class loop (radix_mono8_x) at R = 8.
     uint32_t ptb = 0;
-    if (radix && S.fast_enabled && (eval == HEC_EVAL_AUTO || eval == HEC_EVAL_RADIX8) && mode[g - 1] == HEC_TAB_RHALF32 && D + 1 <= 8 &&
-        geom[g - 1].M % 8u == 0 && geom[g - 1].M >= 4096u) {
+    bool mono = false;
+    if (radix && S.fast_enabled && (mode[g - 1] == HEC_TAB_RHALF32 || mode[g - 1] == HEC_TAB_RHALF17)) {
         uint64_t total = parity_table_bytes(geom[g - 1].M);
         for (uint32_t k = 1; k <= g; k++) total += bytes[k - 1];
-        if (total <= budget) { ptb = parity_table_bytes(geom[g - 1].M); radix_of[g - 1] = 8u; }
+        if (total <= budget) {
+            ptb = parity_table_bytes(geom[g - 1].M);
+            mono = (eval == HEC_EVAL_AUTO || eval == HEC_EVAL_RADIX8) && mode[g - 1] == HEC_TAB_RHALF32 && D + 1 <= 8 &&
+                   geom[g - 1].M % 8u == 0 && geom[g - 1].M >= 4096u;
+            if (mono) radix_of[g - 1] = 8u;
+        }
     }
     if (radix && S.fast_enabled) {
         uint64_t total = ptb;
@@ -493,6 +500,10 @@ int build_plan(LibState &S, uint32_t q, uint32_t g, int regime, int eval, Device
                     const uint32_t lo_bytes = align16(((t.M >> 1) + 1u) * 2u);
                     fd.smem_off2 = so + lo_bytes;
                     fill_rhalf17(*fields[k - 1], t.M, reinterpret_cast<uint16_t *>(dst), dst + lo_bytes);
+                    if (k == g && ptb) {
+                        fd.pt_off = so + bytes[k - 1];
+                        fill_parity_table(*fields[k - 1], t.M, dst + bytes[k - 1]);
+                    }
                     break;
                 }
                 default:
@@ -578,7 +589,7 @@ int build_plan(LibState &S, uint32_t q, uint32_t g, int regime, int eval, Device
     // the shift pre-pass pays where the dominant (largest) field has R >= 4 and the rows have at least R coefficients
     plan->shift_R = (radix && plan->f[g - 1].radix >= 4u && 2 * g + 2 >= plan->f[g - 1].radix) ? plan->f[g - 1].radix : 0u;
     // monomial classes (radix_mono8_x / radix_mono8_packed_x): every coefficient up to the degree nonzero
-    plan->shift_dense = ptb != 0 || (radix && D + 1 <= 8 && plan->f[g - 1].radix == 8u && plan->f[g - 1].fast_off != 0);
+    plan->shift_dense = mono || (radix && D + 1 <= 8 && plan->f[g - 1].radix == 8u && plan->f[g - 1].fast_off != 0);
     if (plan->shift_dense) plan->shift_R = 8u;
     plan->d_part_codes = reinterpret_cast<const unsigned long long *>(base + part_off);
     plan->n_parts = (uint32_t)parts.size();

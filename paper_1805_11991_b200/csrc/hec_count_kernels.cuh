@@ -449,17 +449,29 @@ __global__ void __launch_bounds__(kThreads, 1) hec_count_radix_kernel(const __gr
                 bool mono = false;
                 if constexpr (!SPLIT && !ORBIT && D + 1 <= 8) {           // monomial classes on a field with a parity table
                     const uint32_t dense = (nz >> D) ? (1u << (D + 1)) - 1u : (1u << D) - 1u;
-                    if (F.pt_off && nz == dense) {
+                    if (F.pt_off && F.radix == 8u && nz == dense) {
                         const uint2 res = (nz >> D) ? hec_radix::radix_mono8_x<D, D + 1>(pol, smem_base + F.pt_off, M, lane, nz, lcj, scratch)
                                                     : hec_radix::radix_mono8_x<D, D>(pol, smem_base + F.pt_off, M, lane, nz, lcj, scratch);
                         n_sq = res.x; n_zero = res.y;
                         mono = true;
                     }
                 }
-                if (!mono) radix_dispatch<D, hec_radix::ArScalar, ORBIT, false>(F, pol, smem_base, lane, nz, lcj, scratch, part, splits, n_sq, n_zero);
+                if (!mono) {
+                    if (F.pt_off) {                                       // parity table for the classifying last stage
+                        const hec_radix::HalfS32T<true> polp{pol.tb, pol.tbh, smem_base + F.pt_off};
+                        radix_dispatch<D, hec_radix::ArScalar, ORBIT, false>(F, polp, smem_base, lane, nz, lcj, scratch, part, splits, n_sq, n_zero);
+                    } else {
+                        radix_dispatch<D, hec_radix::ArScalar, ORBIT, false>(F, pol, smem_base, lane, nz, lcj, scratch, part, splits, n_sq, n_zero);
+                    }
+                }
             } else if constexpr (TOP == HEC_TAB_RHALF17) {
                 const hec_radix::HalfS17 pol{smem_base + F.smem_off, smem_base + F.smem_off + 2u * (M >> 1), smem_base + F.smem_off2};
-                radix_dispatch<D, hec_radix::ArScalar, ORBIT, false>(F, pol, smem_base, lane, nz, lcj, scratch, part, splits, n_sq, n_zero);
+                if (F.pt_off) {
+                    const hec_radix::HalfS17T<true> polp{pol.tb, pol.tbh, pol.bb, smem_base + F.pt_off};
+                    radix_dispatch<D, hec_radix::ArScalar, ORBIT, false>(F, polp, smem_base, lane, nz, lcj, scratch, part, splits, n_sq, n_zero);
+                } else {
+                    radix_dispatch<D, hec_radix::ArScalar, ORBIT, false>(F, pol, smem_base, lane, nz, lcj, scratch, part, splits, n_sq, n_zero);
+                }
             } else if constexpr (TOP == HEC_TAB_GPAIR64) {
                 const hec_radix::PairG64 pol{reinterpret_cast<const uint2 *>(F.gtab)};
                 radix_dispatch<D, hec_radix::ArScalar, ORBIT, false>(F, pol, smem_base, lane, nz, lcj, scratch, part, splits, n_sq, n_zero);

@@ -66,6 +66,7 @@ __device__ __forceinline__ void packed_addr(uint32_t tb, uint32_t n2, uint32_t &
 
 // PAIR16: shared memory, M 32-bit entries, lo16 = Z[n], hi16 = Z[n + h]  (M <= 32768).
 struct PairS16 {
+    static constexpr bool kParity = false;
     uint32_t tb;                                             // shared byte address of entry 0
     __device__ __forceinline__ uint32_t pair_word(uint32_t n) const { return lds_u32(tb + 4u * n); }
     __device__ __forceinline__ void pair(uint32_t n, uint32_t, uint32_t, uint32_t &za, uint32_t &zs) const {
@@ -79,8 +80,13 @@ struct PairS16 {
 // RHALF32: shared memory, HT[i] = Z[i] for 0 <= i <= h (HT[h] = 0), 32-bit entries.  Z(-m) = Z(m) - m (reading
 // G16) gives Z[i + h] = HT[h - i] + i + h (mod M) for 0 <= i < h, so with i = n mod h the pair is
 // (HT[i], HT[h - i] + i + h), swapped when n >= h.
-struct HalfS32 {
+// PT: the field also carries a packed parity table (tp: its shared byte address; 2 bits per n: parity of Z[n], of Z[n + h]; four
+// entries per byte), which the classifying last stage of the network reads instead of the pair (one load instead of two / three).
+template <bool PT>
+struct HalfS32T {
+    static constexpr bool kParity = PT;
     uint32_t tb, tbh;                                        // shared byte addresses of HT[0] and HT[h]
+    uint32_t tp;
     __device__ __forceinline__ void pair(uint32_t n, uint32_t M, uint32_t h, uint32_t &za, uint32_t &zs) const {
         const uint32_t i = min(n, n - h);
         const uint32_t t1 = lds_u32(tb + 4u * i);
@@ -100,8 +106,13 @@ struct HalfS32 {
 
 // RHALF17: as RHALF32 for M < 2^17: a 16-bit plane with the low halves of HT[0..h] and a byte plane whose
 // entry i holds bit 16 of HT[i] (bit 0) and of HT[h - i] (bit 1): three loads per pair.
-struct HalfS17 {
+using HalfS32 = HalfS32T<false>;
+
+template <bool PT>
+struct HalfS17T {
+    static constexpr bool kParity = PT;
     uint32_t tb, tbh, bb;                                    // 16-bit plane: HT[0], HT[h]; byte plane
+    uint32_t tp;
     __device__ __forceinline__ void pair(uint32_t n, uint32_t M, uint32_t h, uint32_t &za, uint32_t &zs) const {
         const uint32_t i = min(n, n - h);
         const uint32_t l1 = lds_u16(tb + 2u * i), l2 = lds_u16(tbh - 2u * i), b = lds_u8(bb + i);
@@ -120,8 +131,11 @@ struct HalfS17 {
     }
 };
 
+using HalfS17 = HalfS17T<false>;
+
 // GPAIR64: global memory (L1/L2-resident regime), M entries (Z[n], Z[n + h]) as uint2.
 struct PairG64 {
+    static constexpr bool kParity = false;
     const uint2 *t;
     __device__ __forceinline__ void pair(uint32_t n, uint32_t, uint32_t, uint32_t &za, uint32_t &zs) const {
         const uint2 w = __ldg(t + n);
@@ -154,6 +168,12 @@ struct ArScalar {
     }
     __device__ __forceinline__ uint32_t parity2(uint32_t a, uint32_t za, uint32_t zs) const { return ((a ^ za) & 1u) + ((a ^ zs) & 1u); }
     __device__ __forceinline__ uint32_t parity1(uint32_t a) const { return a & 1u; }
+    // number of odd logs among a + Z[n], a + Z[n + h] from the packed parity table at tp; a zero sum is n = 0 or n = h
+    __device__ __forceinline__ uint32_t parity_lookup(uint32_t tp, uint32_t a, uint32_t n, uint32_t &mn) const {
+        mn = min(mn, min(n, n - h));
+        const uint32_t p = lds_u8(tp + (n >> 2)) >> ((n & 3u) << 1);
+        return ((a ^ p) & 1u) + ((a ^ (p >> 1)) & 1u);
+    }
     __device__ __forceinline__ bool flagged(uint32_t mn, int) const { return mn == 0u; }
     __device__ __forceinline__ uint32_t keep(uint32_t v, bool k0, bool) const { return k0 ? v : 0u; }
     __device__ __forceinline__ uint32_t total(uint32_t v) const { return v; }
@@ -347,14 +367,25 @@ __device__ __forceinline__ void network(const Ar &ar, const Pol &pol, const uint
                 if (pa && pb) {
                     uint32_t n = ar.subm(v[i2], v[i1]);
                     if (oe) n = ar.wrap(n + ar.rep((uint32_t)oe * unit));
-                    uint32_t za, zs;
-                    ar.lookup_pair(pol, n, za, zs, mn);
                     const uint32_t a = v[i1];
-                    if (H > 1) {
-                        v[i1] = ar.wrap(a + za);
-                        v[i2] = ar.wrap(a + zs);
+                    if constexpr (Pol::kParity) {
+                        if (H == 1) {
+                            ps += ar.parity_lookup(pol.tp, a, n, mn);
+                        } else {
+                            uint32_t za, zs;
+                            ar.lookup_pair(pol, n, za, zs, mn);
+                            v[i1] = ar.wrap(a + za);
+                            v[i2] = ar.wrap(a + zs);
+                        }
                     } else {
-                        ps += ar.parity2(a, za, zs);
+                        uint32_t za, zs;
+                        ar.lookup_pair(pol, n, za, zs, mn);
+                        if (H > 1) {
+                            v[i1] = ar.wrap(a + za);
+                            v[i2] = ar.wrap(a + zs);
+                        } else {
+                            ps += ar.parity2(a, za, zs);
+                        }
                     }
                 } else if (pa) {                                           // b = 0: both outputs are a
                     if (H > 1) v[i2] = v[i1];
@@ -719,11 +750,7 @@ __device__ __forceinline__ void network_mono(const Ar &ar, const Pol &pol, const
                             ps += ar.parity2(a, za, zs);
                         }
                     } else {
-                        if constexpr (PT) {                           // scalar arithmetic only
-                            mn = min(mn, min(n, n - ar.h));           // 0 iff one of the two sums vanishes
-                            const uint32_t p = lds_u8(tp + (n >> 2)) >> ((n & 3u) << 1);
-                            ps += ((a ^ p) & 1u) + ((a ^ (p >> 1)) & 1u);
-                        }
+                        if constexpr (PT) ps += ar.parity_lookup(tp, a, n, mn);     // scalar arithmetic only
                     }
                 } else if (pa) {                                      // b = 0: both outputs are a
                     if (H > 1) v[i2] = v[i1];
