@@ -380,7 +380,11 @@ def roofline_record(torch, hec, cfg, rows, m, local_rank, counters):
                       "wavefronts_per_request": wf / (ld / 32),
                       "model_over_counter": (rec.get("executed_loads_per_launch") or 0) / ld if ld else None,
                       "smem_pipe_frac": wf / (k_ms * 1e-3) / (sms * mhz * 1e6),
-                      "dram_bytes_per_launch": (float(c["dram__bytes_read.sum"]) + float(c["dram__bytes_write.sum"])) * scale}
+                      "dram_bytes_per_launch": (float(c["dram__bytes_read.sum"]) + float(c["dram__bytes_write.sum"])) * scale,
+                      "step_dram_bytes": float(c["step_dram_bytes"]) * scale,      # pre-pass + count + squarefree kernels
+                      "smem_pipe_pct": float(c["l1tex__data_pipe_lsu_wavefronts_mem_shared.sum.pct_of_peak_sustained_elapsed"]),
+                      "alu_pipe_pct": float(c["sm__inst_executed_pipe_alu.avg.pct_of_peak_sustained_active"]),
+                      "issue_active_pct": float(c["smsp__issue_active.avg.pct_of_peak_sustained_active"])}
         rec["traffic"] = rec["ncu"]["dram_bytes_per_launch"]
         rec["traffic_unit"] = "bytes per launch: ncu dram read + write of the count kernel (profiles/r02_counters.csv), scaled"
     else:
