@@ -306,6 +306,15 @@ int hec_shift_rows(uint32_t q, uint32_t g, const uint16_t *coeffs, size_t n, uin
  * for a (q, g) (the setting is part of the plan key). */
 int hec_set_fast_tables(int on);
 
+/* Representation independence ("rerun with another primitive polynomial -- every N_k identical").
+ * v = 0 (default): the library's own fields F_{q^k} are built on the lexicographically smallest primitive polynomial
+ * (reading G7); v > 0: on the (v+1)-th smallest, i.e. another generator alpha, other log / Zech / embedding tables.
+ * Every output of hec_count / hec_count_ex / hec_curve_map must be unchanged.  F_q itself (k = 1) keeps its smallest
+ * polynomial: for q = p^r, r > 1 it fixes the encoding of the inputs, and the reduced polynomials of Algorithm 1 are
+ * defined through its generator.  hec_build_field / hec_build_field_device always return the smallest.
+ * Drops the cached plans; v <= 16. */
+int hec_set_field_variant(uint32_t v);
+
 /* Total number of kernels launched by this library since load (bench.py's gpu_launches). */
 uint64_t hec_launch_count(void);
 

@@ -938,6 +938,14 @@ int hec_count_histogram(uint32_t q, uint32_t g, const uint16_t *coeffs, size_t n
     return rc ? rc : hrc;
 }
 
+int hec_set_field_variant(uint32_t v) {
+    if (v > 16u) HEC_FAIL(HEC_ERR_INVALID_ARG, "variant must be at most 16");
+    std::lock_guard<std::recursive_mutex> lock(g_state.mu);
+    hec_set_field_variant_impl(v);
+    g_state.plans.clear();                        // plans hold tables of the previous representation
+    return HEC_OK;
+}
+
 int hec_set_fast_tables(int on) {
     std::lock_guard<std::recursive_mutex> lock(g_state.mu);
     g_state.fast_enabled = on != 0;

@@ -80,9 +80,11 @@ bool walk_powers(const Ring &R, uint32_t Q, std::vector<uint32_t> &antilog) {
 
 std::mutex g_cache_mutex;
 std::atomic<bool> g_device_build{false};
-std::map<std::tuple<uint32_t, uint32_t, uint32_t>, std::unique_ptr<hec_field>> g_cache;
+std::atomic<uint32_t> g_variant{0};          // hec_set_field_variant: which primitive polynomial the library's own fields use
+std::map<std::tuple<uint32_t, uint32_t, uint32_t, uint32_t>, std::unique_ptr<hec_field>> g_cache;
 
-hec_field *build_field_impl(uint32_t p, uint32_t r, uint32_t k) {
+// skip: take the (skip+1)-th lexicographically smallest primitive polynomial (0: the smallest, reading G7)
+hec_field *build_field_impl(uint32_t p, uint32_t r, uint32_t k, uint32_t skip = 0) {
     if (!is_odd_prime(p)) { hec_set_error(HEC_ERR_INVALID_FIELD, "p must be an odd prime"); return nullptr; }
     if (r < 1 || k < 1) { hec_set_error(HEC_ERR_INVALID_FIELD, "r and k must be >= 1"); return nullptr; }
     uint64_t q64 = 1, Q64 = 1;
@@ -104,6 +106,7 @@ hec_field *build_field_impl(uint32_t p, uint32_t r, uint32_t k) {
 
     // lexicographic order of (a_{n-1}, .., a_0): a_0 runs fastest, i.e. count e = sum a_i p^i upwards
     bool found = false;
+    uint32_t seen = 0;
     for (uint32_t e = 1; e < Q && !found; e++) {
         unpack(R, e, R.mod.data());
         R.mod[n] = 1;
@@ -122,6 +125,7 @@ hec_field *build_field_impl(uint32_t p, uint32_t r, uint32_t k) {
         } else {
             found = walk_powers(R, Q, F->antilog);
         }
+        if (found && seen < skip) { seen++; found = false; }
     }
     if (!found) { hec_set_error(HEC_ERR_INVALID_FIELD, "no primitive polynomial found"); return nullptr; }
     F->modulus = R.mod;
@@ -193,24 +197,28 @@ bool hec_factor_q(uint32_t q, uint32_t *p_out, uint32_t *r_out) {
 }
 
 const hec_field *hec_cached_field(uint32_t p, uint32_t r, uint32_t k) {
+    // F_q itself keeps the smallest polynomial: for q = p^r, r > 1 it fixes the encoding of the inputs (hec.h), and the
+    // reduced polynomials of Algorithm 1 are defined through its generator (hec_enum.cu)
+    const uint32_t skip = k == 1 ? 0u : g_variant.load();
     {
         std::lock_guard<std::mutex> lock(g_cache_mutex);
-        auto it = g_cache.find(std::make_tuple(p, r, k));
+        auto it = g_cache.find(std::make_tuple(p, r, k, skip));
         if (it != g_cache.end()) return it->second.get();
     }
     uint64_t Q = 1;
     for (uint32_t i = 0; i < r * k && Q <= HEC_MAX_FIELD_SIZE; i++) Q *= p;
     const bool on_device = g_device_build.load() && Q > kDeviceBuildMinQ && Q <= HEC_MAX_FIELD_SIZE && p < 65536;
-    hec_field *F = on_device ? hec_build_field_device_impl(p, r, k) : build_field_impl(p, r, k);   // may recurse into the cache for (p, r, 1)
+    hec_field *F = on_device ? hec_build_field_device_impl(p, r, k, skip) : build_field_impl(p, r, k, skip);   // may recurse into the cache for (p, r, 1)
     if (!F) return nullptr;
     std::lock_guard<std::mutex> lock(g_cache_mutex);
-    auto &slot = g_cache[std::make_tuple(p, r, k)];
+    auto &slot = g_cache[std::make_tuple(p, r, k, skip)];
     if (slot) { delete F; return slot.get(); }
     slot.reset(F);
     return F;
 }
 
 void hec_allow_device_field_build(bool on) { g_device_build.store(on); }
+void hec_set_field_variant_impl(uint32_t v) { g_variant.store(v); }
 
 void hec_clear_field_cache() {
     std::lock_guard<std::mutex> lock(g_cache_mutex);

@@ -190,7 +190,7 @@ std::vector<uint32_t> prime_factors(uint32_t m) {
 }  // namespace
 
 // Device build of the field; same result as the host build (hec_field.cpp), bit for bit.
-hec_field *hec_build_field_device_impl(uint32_t p, uint32_t r, uint32_t k) {
+hec_field *hec_build_field_device_impl(uint32_t p, uint32_t r, uint32_t k, uint32_t skip) {
     if (p < 3 || p % 2 == 0) { hec_set_error(HEC_ERR_INVALID_FIELD, "p must be an odd prime"); return nullptr; }
     for (uint32_t d = 3; (uint64_t)d * d <= p; d += 2)
         if (p % d == 0) { hec_set_error(HEC_ERR_INVALID_FIELD, "p must be an odd prime"); return nullptr; }
@@ -215,6 +215,7 @@ hec_field *hec_build_field_device_impl(uint32_t p, uint32_t r, uint32_t k) {
     const std::vector<uint32_t> ell = prime_factors(M);
     HostRing R{p, n, std::vector<uint32_t>(n, 0)};
     bool found = false;
+    uint32_t seen = 0;
     std::vector<uint32_t> modulus(n + 1, 0);
     for (uint32_t e = 1; e < Q && !found; e++) {
         uint32_t v = e;
@@ -228,6 +229,7 @@ hec_field *hec_build_field_device_impl(uint32_t p, uint32_t r, uint32_t k) {
         for (uint32_t l : ell)
             if (R.is_one(R.pow(t, M / l))) { prim = false; break; }
         found = prim;
+        if (found && seen < skip) { seen++; found = false; }
     }
     if (!found) { hec_set_error(HEC_ERR_INVALID_FIELD, "no primitive polynomial found"); return nullptr; }
     F->modulus = modulus;
@@ -317,4 +319,4 @@ hec_field *hec_build_field_device_impl(uint32_t p, uint32_t r, uint32_t k) {
     return F.release();
 }
 
-extern "C" hec_field *hec_build_field_device(uint32_t p, uint32_t r, uint32_t k) { return hec_build_field_device_impl(p, r, k); }
+extern "C" hec_field *hec_build_field_device(uint32_t p, uint32_t r, uint32_t k) { return hec_build_field_device_impl(p, r, k, 0); }

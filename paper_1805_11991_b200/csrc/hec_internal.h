@@ -31,7 +31,9 @@ bool hec_factor_q(uint32_t q, uint32_t *p, uint32_t *r);
 const hec_field *hec_cached_field(uint32_t p, uint32_t r, uint32_t k);
 void hec_clear_field_cache();
 // Tables built on the device (hec_field_device.cu); same result as the host build.
-hec_field *hec_build_field_device_impl(uint32_t p, uint32_t r, uint32_t k);
+hec_field *hec_build_field_device_impl(uint32_t p, uint32_t r, uint32_t k, uint32_t skip = 0);
+// hec_set_field_variant: the library's own fields take the (v+1)-th smallest primitive polynomial (hec.h)
+void hec_set_field_variant_impl(uint32_t v);
 // hec_cached_field builds fields above this size on the device once hec_count has initialised one.
 constexpr uint32_t kDeviceBuildMinQ = 1u << 16;
 void hec_allow_device_field_build(bool on);

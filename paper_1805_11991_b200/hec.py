@@ -34,7 +34,7 @@ SYMBOLS = [
     "hec_field_degree", "hec_field_q", "hec_field_Q", "hec_field_embed_unit", "hec_field_modulus",
     "hec_field_antilog", "hec_field_log", "hec_field_zech", "hec_field_embed", "hec_count", "hec_histogram",
     "hec_histogram_merge", "hec_reduced_total", "hec_reduced_rows", "hec_curve_map",
-    "hec_count_ex", "hec_lambda_partitions", "hec_curve_map_lambda", "hec_set_map_chunk_rows", "hec_curve_map_range", "hec_curve_map_all", "hec_set_shift", "hec_shift_rows", "hec_set_fast_tables", "hec_count_histogram",
+    "hec_count_ex", "hec_lambda_partitions", "hec_curve_map_lambda", "hec_set_map_chunk_rows", "hec_curve_map_range", "hec_curve_map_all", "hec_set_shift", "hec_shift_rows", "hec_set_fast_tables", "hec_count_histogram", "hec_set_field_variant",
     "hec_set_stream", "hec_set_regime", "hec_set_eval", "hec_last_count_stats", "hec_launch_count", "hec_gather_bench",
     "hec_shutdown",
 ]
@@ -89,6 +89,7 @@ def lib():
         L.hec_set_map_chunk_rows.argtypes = [sz]
         L.hec_set_shift.argtypes = [ctypes.c_int]
         L.hec_set_fast_tables.argtypes = [ctypes.c_int]
+        L.hec_set_field_variant.argtypes = [ctypes.c_uint32]
         L.hec_shift_rows.argtypes = [u32, u32, vp, sz, vp]
         L.hec_curve_map_all.argtypes = [u32, u32, ctypes.c_int, vp, vp, sz, ctypes.POINTER(sz)]
         L.hec_curve_map_range.argtypes = [u32, u32, u32, ctypes.c_uint64, ctypes.c_uint64, ctypes.c_int, vp, vp, sz, ctypes.POINTER(sz)]
@@ -401,6 +402,11 @@ def set_shift(on: bool):
 
 def set_fast_tables(on: bool):
     _check(lib().hec_set_fast_tables(int(on)))
+
+
+def set_field_variant(v: int):
+    """hec_set_field_variant: the library's own fields use the (v+1)-th smallest primitive polynomial (0: the smallest)."""
+    _check(lib().hec_set_field_variant(int(v)))
 
 
 def shift_rows(q: int, g: int, coeffs):

@@ -569,3 +569,41 @@ def test_monomial_class_loops_against_oracle(torch_cuda, q, g, n):
     assert (cnt.reshape(-1, m, g) == ocnt).all() and (sf.reshape(-1, m) == osf).all()          # every copy of the rows
     cnt2, sf2 = _gpu_count(torch_cuda, q, g, rows)                          # the same rows in split mode
     assert (cnt2 == ocnt).all() and (sf2 == osf).all()
+
+
+@pytest.mark.parametrize("cid,n", [(2, None), (3, None), (4, None), (5, None), (1, None)])
+def test_other_primitive_polynomial_full_size(torch_cuda, cid, n):
+    """SURVEY.md 8(c) "whole GPU path at full size": rerun on ANOTHER primitive polynomial (hec_set_field_variant: another
+    generator of every F_{q^k}, k >= 2, hence other log / Zech / embedding tables and other table indices throughout) --
+    every N_k and every flag of every row must be identical.  Together with test_eval_schemes_agree_full_config (another
+    kernel and table layout) this is the representation independence of the counts at full size."""
+    if torch_cuda.eval_scheme != "auto":
+        pytest.skip("one scheme is enough: the field build is shared")
+    cfg = W.CONFIGS[cid]
+    d_rows = _dev(torch_cuda, W.generate(cfg))
+    a, sa = hec.count(cfg.q, cfg.g, d_rows)
+    try:
+        for v in ((1,) if cid == 1 else (1, 2)):                         # F_9 has only two primitive quadratics
+            hec.set_field_variant(v)
+            b, sb = hec.count(cfg.q, cfg.g, d_rows)
+            assert bool((a == b).all()) and bool((sa == sb).all()), (cid, v)
+    finally:
+        hec.set_field_variant(0)
+
+
+def test_other_primitive_polynomial_changes_the_tables_not_the_map(torch_cuda):
+    """Algorithm 1's map (lambda included) and hec_count_ex's root counts and lambda do not notice the other representation."""
+    if torch_cuda.eval_scheme != "auto":
+        pytest.skip("one scheme is enough")
+    ref = hec.curve_map(7, 2, 6, True)
+    rows = W.generate(W.CONFIGS[3], 0, 6000)
+    r0 = hec.count_ex(49, 3, _dev(torch_cuda, rows))
+    try:
+        hec.set_field_variant(1)
+        got = hec.curve_map(7, 2, 6, True)
+        r1 = hec.count_ex(49, 3, _dev(torch_cuda, rows))
+    finally:
+        hec.set_field_variant(0)
+    assert (ref[0] == got[0]).all() and (ref[1] == got[1]).all()
+    for x, y in zip(r0, r1):
+        assert bool((x == y).all())
