@@ -91,7 +91,7 @@ def executed_loads(cfg: W.Workload, rows: np.ndarray, stats: dict) -> dict:
             conflict_free += int((nnz >= 2).sum()) * M * single
             random += int(np.maximum(nnz - 2, 0).sum()) * M * single
             continue
-        if M <= DIRECT_MAX_M and mode == 4 and stats.get("eval") != "orbit":
+        if M <= DIRECT_MAX_M and mode == 4:
             random += int(nzm.sum()) * M
             continue
         fast = bool((stats.get("fast_fields", 0) >> (k - 1)) & 1)

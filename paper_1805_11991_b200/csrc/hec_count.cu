@@ -579,6 +579,7 @@ int build_plan(LibState &S, uint32_t q, uint32_t g, int regime, int eval, Device
         plan->f[k - 1].gtab = glob ? reinterpret_cast<const uint32_t *>(base + gtab_off[k - 1]) : nullptr;
         plan->f[k - 1].emb = reinterpret_cast<const uint32_t *>(base + emb_off[k - 1]);
         for (int t = 0; t < 3; t++) {
+            plan->f[k - 1].orb_fast = (eval == HEC_EVAL_ORBIT && mode[k - 1] == HEC_TAB_PAIR16 && S.fast_enabled) ? 1u : 0u;
             plan->f[k - 1].n_orb[t] = orb_cnt[k - 1][t];
             plan->f[k - 1].orb[t] = orb_cnt[k - 1][t] ? reinterpret_cast<const uint32_t *>(base + orb_off[k - 1][t]) : nullptr;
         }

@@ -356,7 +356,7 @@ __device__ __forceinline__ void radix_dispatch(const HecFieldDev &F, const Pol p
                                                const uint32_t splits, uint32_t &n_sq, uint32_t &n_zero) {
     using namespace hec_radix;
     const uint32_t R = F.radix, M = F.M, rcpM = F.rcpM;
-    if constexpr (!ORBIT && std::is_same<Pol, PairS16>::value) {
+    if constexpr (std::is_same<Pol, PairS16>::value) {
         if (M <= kDirectMaxM) {                       // tiny field: every point directly (splits: part 0 takes them all)
             uint2 res = make_uint2(0u, 0u);
             if (part == 0u) res = direct_all_x<D>(pol, M, lane, nz, lcj, scratch);
@@ -382,6 +382,12 @@ __device__ __forceinline__ void radix_dispatch(const HecFieldDev &F, const Pol p
         }
     }
     uint2 res;
+    if constexpr (ORBIT && std::is_same<Pol, PairS16>::value) {
+        if (F.orb_fast) {                                 // every class present at R = 4 or 8: offsets by repeated addition
+            if (R >= 8 && all_classes_present<D, 8>(nz)) { res = radix_orbit_fast_x<D, 8>(pol, M, rcpM, lane, nz, lcj, scratch, F.orb[2], F.n_orb[2]); n_sq = res.x; n_zero = res.y; return; }
+            if (R >= 4 && all_classes_present<D, 4>(nz)) { res = radix_orbit_fast_x<D, 4>(pol, M, rcpM, lane, nz, lcj, scratch, F.orb[1], F.n_orb[1]); n_sq = res.x; n_zero = res.y; return; }
+        }
+    }
     if constexpr (ORBIT) {
         if (R >= 8 && all_classes_present<D, 8>(nz)) res = radix_orbit_x<D, 8, true, Ar>(pol, M, rcpM, lane, nz, lcj, scratch, F.orb[2], F.n_orb[2]);
         else if (R >= 4 && all_classes_present<D, 4>(nz)) res = radix_orbit_x<D, 4, true, Ar>(pol, M, rcpM, lane, nz, lcj, scratch, F.orb[1], F.n_orb[1]);

@@ -307,7 +307,8 @@ __device__ __forceinline__ uint32_t horner_point(const Pol &pol, const uint32_t 
     return zero ? kZero : acc;
 }
 
-template <int D, int R, typename Pol>
+// WEIGHTED (orbit scheme): a queue entry is n | (orbit length << 28) and every count is multiplied by the orbit length.
+template <int D, int R, typename Pol, bool WEIGHTED = false>
 __device__ __noinline__ void exact_queue(const Pol pol, const uint32_t M, const uint32_t nz, const volatile uint32_t *sc,
                                          const uint32_t qn, const uint32_t lane, uint32_t &nz_exact, uint32_t &odd_exact) {
     constexpr uint32_t LG = R == 8 ? 3u : R == 4 ? 2u : 1u;
@@ -315,8 +316,10 @@ __device__ __noinline__ void exact_queue(const Pol pol, const uint32_t M, const 
     const uint32_t j = lane & (uint32_t)(R - 1), slot = lane >> LG;
     for (uint32_t q0 = 0; q0 < qn; q0 += 32u / R) {
         const uint32_t qi = min(q0 + slot, qn - 1u);                       // idle slots repeat the last coset (not counted)
-        const uint32_t acc = horner_point<D>(pol, M, nz, sc, sc[16 + qi] + j * S);     // log x < M
-        if (q0 + slot < qn && acc < M) { nz_exact++; odd_exact += acc & 1u; }
+        const uint32_t e = sc[16 + qi];
+        const uint32_t n = WEIGHTED ? (e & 0x0FFFFFFFu) : e, w = WEIGHTED ? (e >> 28) : 1u;
+        const uint32_t acc = horner_point<D>(pol, M, nz, sc, n + j * S);   // log x < M
+        if (q0 + slot < qn && acc < M) { nz_exact += w; odd_exact += w * (acc & 1u); }
     }
 }
 
@@ -1013,6 +1016,118 @@ __device__ __noinline__ uint2 radix_orbit_x(const Pol pol, const uint32_t M, con
     n_zero = w_flagged * R - nz_exact;
     n_sq = n_nz - (odd_fast + odd_exact);
     return make_uint2(n_sq, n_zero);
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// radix_orbit_x for PAIR16 fields, R in {4, 8}, every class non-empty (HEC_EVAL_ORBIT, round 2).  The offsets e n mod M
+// of a representative n are built by repeated addition, n, 2n, .., Dn (one packed add + wrap each), instead of one
+// multiply-high reduction per term and coset, and flagged cosets are re-evaluated one point per lane (exact_queue).
+// Links whose exponent gap exceeds 2R (possible from D >= 3R on) are left to radix_orbit_x.
+// ---------------------------------------------------------------------------------------------------------
+template <int D, int R>
+__device__ __noinline__ uint2 radix_orbit_fast_x(const PairS16 pol, const uint32_t M, const uint32_t rcpM, const uint32_t lane,
+                                                 const uint32_t nz, const uint32_t lcj, volatile uint32_t *scratch,
+                                                 const uint32_t *__restrict__ reps, const uint32_t n_reps) {
+    constexpr int NT = D + 1 > R ? D + 1 - R : 0;
+    constexpr int NTA = NT > 0 ? NT : 1;
+    const ArPacked ar(M);
+    const uint32_t unit = M / R;
+    if (n_reps == 0u) return make_uint2(0u, 0u);
+
+    uint32_t dl[NTA];                                  // chain links: rep(delta)
+    uint32_t cm = 0, far = 0, present = 0, topmask = 0;   // far: links whose gap is 2R; topmask: bit e set iff e is the top exponent of its class
+    bool ok = true;
+    uint32_t last_lc[R], last_e[R];
+#pragma unroll
+    for (int r = 0; r < R; r++) { last_lc[r] = 0; last_e[r] = 0; }
+#pragma unroll
+    for (int i = D; i >= 0; i--) {
+        const int r = i % R;
+        const uint32_t lci = __shfl_sync(0xffffffffu, lcj, i);
+        if (i < NT) dl[i] = 0;
+        if (nz & (1u << i)) {
+            if (i < NT && (present & (1u << r))) {
+                const uint32_t m = last_e[r] - (uint32_t)i;
+                dl[i] = ar.rep(last_lc[r] >= lci ? last_lc[r] - lci : last_lc[r] + M - lci);
+                cm |= 1u << i;
+                if (m == 2u * R) far |= 1u << i;
+                else if (m != (uint32_t)R) ok = false;
+            }
+            present |= 1u << r;
+            last_lc[r] = lci;
+            last_e[r] = (uint32_t)i;
+        }
+    }
+    if (!ok) return radix_orbit_x<D, R, true, ArPacked>(pol, M, rcpM, lane, nz, lcj, scratch, reps, n_reps);
+#pragma unroll
+    for (int r = 0; r < R; r++) { topmask |= 1u << last_e[r]; last_lc[r] = ar.rep(last_lc[r]); }
+
+    __syncwarp();
+    if (lane <= (uint32_t)D) scratch[lane] = lcj;
+    __syncwarp();
+
+    uint32_t acc = 0, qn = 0, nz_exact = 0, odd_exact = 0, w_ok = 0, w_flagged = 0;
+    for (uint32_t base = 0; base < n_reps; base += 64u) {
+        const uint32_t i0 = base + lane, i1 = i0 + 32u;
+        const uint32_t e0 = i0 < n_reps ? __ldg(reps + i0) : 0u, e1 = i1 < n_reps ? __ldg(reps + i1) : 0u;   // weight 0: an invalid slot
+        uint32_t w0 = e0 >> 28, w1 = e1 >> 28;
+        const uint32_t nn = (e0 & 0xFFFFu) | (e1 << 16);                 // coset indices are below M / R <= 2^13
+        // kn[r] = last_e[r] n mod M; pR = R n, p2R = 2R n
+        uint32_t kn[R], pR = 0, p2R = 0, cur = 0;
+#pragma unroll
+        for (int r = 0; r < R; r++) kn[r] = 0;
+#pragma unroll
+        for (int e = 1; e <= D; e++) {
+            cur = e == 1 ? nn : ar.wrap(cur + nn);
+            if (e == R) pR = cur;
+            if (e == 2 * R) p2R = cur;
+            if (topmask & (1u << e)) kn[e % R] = cur;                    // warp-uniform
+        }
+        uint32_t v[R];
+        uint32_t mn = ar.mn_init();
+#pragma unroll
+        for (int r = 0; r < R; r++) {
+            uint32_t w = 0;
+            bool chained = false;
+#pragma unroll
+            for (int i = NT - 1; i >= 0; i--) {
+                if (i % R != r) continue;
+                if (cm & (1u << i)) {
+                    const uint32_t ul = ar.wrap(dl[i] + ((2 * R <= D && (far & (1u << i))) ? p2R : pR));
+                    const uint32_t n = chained ? ar.wrap(w + ul) : ul;
+                    w = ar.lookup_single(pol, n, mn);
+                    chained = true;
+                }
+            }
+            const uint32_t kc = ar.wrap(last_lc[r] + kn[r]);
+            v[r] = chained ? ar.wrap(w + kc) : kc;
+        }
+        uint32_t ps = 0;
+        network<R, true>(ar, pol, unit, present, v, ps, mn);
+        const bool f0 = w0 != 0u && ar.flagged(mn, 0), f1 = w1 != 0u && ar.flagged(mn, 1);
+        if (__any_sync(0xffffffffu, f0 || f1)) {
+            uint32_t bal = __ballot_sync(0xffffffffu, f0);
+            if (f0) { scratch[16 + qn + __popc(bal & ((1u << lane) - 1u))] = e0; w_flagged += w0; w0 = 0u; }
+            qn += __popc(bal);
+            bal = __ballot_sync(0xffffffffu, f1);
+            if (f1) { scratch[16 + qn + __popc(bal & ((1u << lane) - 1u))] = e1; w_flagged += w1; w1 = 0u; }
+            qn += __popc(bal);
+            __syncwarp();
+            if (qn >= 32u) {
+                exact_queue<D, R, PairS16, true>(pol, M, nz, scratch, qn, lane, nz_exact, odd_exact);
+                qn = 0;
+                __syncwarp();
+            }
+        }
+        acc += (ps & 0xFFFFu) * w0 + (ps >> 16) * w1;  // <= 8 * 4 per pass: a plain 32-bit sum
+        w_ok += w0 + w1;
+    }
+    exact_queue<D, R, PairS16, true>(pol, M, nz, scratch, qn, lane, nz_exact, odd_exact);
+    __syncwarp();
+    const uint32_t n_nz = w_ok * R + nz_exact;          // every value of an unflagged coset is nonzero
+    // nz_exact / odd_exact are spread over the lanes by point, w_flagged by coset: only the warp sums are meaningful, and
+    // n_zero = sum(w_flagged) R - sum(nz_exact) may be "negative" in one lane (mod 2^32 the warp sum is right)
+    return make_uint2(n_nz - (acc + odd_exact), w_flagged * R - nz_exact);
 }
 
 }  // namespace hec_radix
