@@ -97,6 +97,27 @@ def executed_loads(cfg: W.Workload, rows: np.ndarray, stats: dict) -> dict:
         fast = bool((stats.get("fast_fields", 0) >> (k - 1)) & 1)
         todo = np.ones(n, dtype=bool)
         R = Rf
+        if fast and ncoef > 8 and ncoef <= 16 and mode in (5, 6) and k == cfg.g and M % 16 == 0 and stats.get("eval") in ("auto", "radix8"):
+            # monomial classes at R = 16 (radix_mono_x): butterflies with both inputs present, the last stage from the parity table
+            deg = ncoef - 1 - (~nzm[:, ::-1]).cumprod(axis=1).sum(axis=1)
+            dense = nzm.sum(axis=1) == deg + 1
+            for NP in (ncoef - 1, ncoef):
+                cnt_np = int((dense & (deg + 1 == NP)).sum())
+                pres, full, last = [i < NP for i in range(16)], 0, 0
+                H = 8
+                while H >= 1:
+                    for blk in range(0, 16, 2 * H):
+                        for j in range(H):
+                            a, b = pres[blk + j], pres[blk + j + H]
+                            if a and b:
+                                if H == 1:
+                                    last += 1
+                                else:
+                                    full += 1
+                            pres[blk + j] = pres[blk + j + H] = a or b
+                    H //= 2
+                random += cnt_np * (full * pair + last) * (M // 16)
+            todo &= ~dense
         if fast and Rf == 8 and ncoef <= 8 and ((mode == 5 and k == cfg.g) or mode == 4):
             # monomial classes (radix_mono8_x / radix_mono8_packed_x): rows with every coefficient up to the degree nonzero
             # run NP - 4 + 8 butterflies per coset of 8 points and no chain lookup.  Pair table: one load each; 32-bit half

@@ -411,19 +411,20 @@ int build_plan(LibState &S, uint32_t q, uint32_t g, int regime, int eval, Device
     // fast tables (radix_fast_x) for the PAIR16 fields, the largest field first, as long as one launch still holds everything
     std::vector<uint32_t> radix_of(g, 0), fastb(g, 0);
     for (uint32_t k = 1; k <= g; k++) radix_of[k - 1] = radix ? pick_radix(geom[k - 1].M, eval, mode[k - 1], g) : 0u;
-    // monomial classes on the top field (radix_mono8_x): at most 8 coefficients, 8 | M, 32-bit half table, room for the parity table
     // Packed parity table of the top field (half-table layouts: the classifying last stage reads it instead of the pair), if it fits.
-    // With it, a 32-bit half table with at most 8 coefficients and 8 | M runs the monomial-class loop (radix_mono8_x) at R = 8.
-    uint32_t ptb = 0;
-    bool mono = false;
+    // With it, dense rows run the monomial-class loop (radix_mono_x).
+    uint32_t ptb = 0, mono_r = 0;
     if (radix && S.fast_enabled && (mode[g - 1] == HEC_TAB_RHALF32 || mode[g - 1] == HEC_TAB_RHALF17)) {
         uint64_t total = parity_table_bytes(geom[g - 1].M);
         for (uint32_t k = 1; k <= g; k++) total += bytes[k - 1];
         if (total <= budget) {
             ptb = parity_table_bytes(geom[g - 1].M);
-            mono = (eval == HEC_EVAL_AUTO || eval == HEC_EVAL_RADIX8) && mode[g - 1] == HEC_TAB_RHALF32 && D + 1 <= 8 &&
-                   geom[g - 1].M % 8u == 0 && geom[g - 1].M >= 4096u;
-            if (mono) radix_of[g - 1] = 8u;
+            // monomial classes (radix_mono_x): R = 8 for at most 8 coefficients, R = 16 for 9 .. 16, where R | M
+            const uint32_t Rm = D + 1 <= 8 ? 8u : 16u;
+            if ((eval == HEC_EVAL_AUTO || eval == HEC_EVAL_RADIX8) && D + 1 <= 16 && geom[g - 1].M % Rm == 0 && geom[g - 1].M >= 4096u) {
+                mono_r = Rm;
+                if (Rm == 8u) radix_of[g - 1] = 8u;      // rows that do not qualify run the general loops at R <= 8 either way
+            }
         }
     }
     if (radix && S.fast_enabled) {
@@ -466,7 +467,7 @@ int build_plan(LibState &S, uint32_t q, uint32_t g, int regime, int eval, Device
             fd.lane_cap = std::min<uint32_t>(32u * U, t.M);
             fd.smem_off = so; fd.smem_off2 = 0; fd.gtab = nullptr;
             fd.radix = radix_of[k - 1];
-            fd.fast_off = 0; fd.fast_row = 0; fd.pt_off = 0;
+            fd.fast_off = 0; fd.fast_row = 0; fd.pt_off = 0; fd.mono_r = (k == g) ? mono_r : 0u;
             uint8_t *dst = host.data() + blob_off[gi] + so;
             switch (mode[k - 1]) {
                 case HEC_TAB_EXT16:
@@ -589,8 +590,8 @@ int build_plan(LibState &S, uint32_t q, uint32_t g, int regime, int eval, Device
     plan->sq_antilog = reinterpret_cast<const uint32_t *>(base + sqa_off);
     // the shift pre-pass pays where the dominant (largest) field has R >= 4 and the rows have at least R coefficients
     plan->shift_R = (radix && plan->f[g - 1].radix >= 4u && 2 * g + 2 >= plan->f[g - 1].radix) ? plan->f[g - 1].radix : 0u;
-    // monomial classes (radix_mono8_x / radix_mono8_packed_x): every coefficient up to the degree nonzero
-    plan->shift_dense = mono || (radix && D + 1 <= 8 && plan->f[g - 1].radix == 8u && plan->f[g - 1].fast_off != 0);
+    // monomial classes (radix_mono_x / radix_mono8_packed_x): every coefficient up to the degree nonzero
+    plan->shift_dense = mono_r != 0 || (radix && D + 1 <= 8 && plan->f[g - 1].radix == 8u && plan->f[g - 1].fast_off != 0);
     if (plan->shift_dense) plan->shift_R = 8u;
     plan->d_part_codes = reinterpret_cast<const unsigned long long *>(base + part_off);
     plan->n_parts = (uint32_t)parts.size();

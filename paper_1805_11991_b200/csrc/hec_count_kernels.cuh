@@ -403,6 +403,26 @@ __device__ __forceinline__ void radix_dispatch(const HecFieldDev &F, const Pol p
     n_zero = res.y;
 }
 
+// Monomial classes on a half-table top field with a parity table (hec_radix.cuh: radix_mono_x): rows with every coefficient up to
+// the degree nonzero, at R = 8 (at most 8 coefficients) or R = 16 (9 .. 16).  Returns false if the row or the field does not qualify.
+template <int D, bool SPLIT, bool ORBIT, typename Pol>
+__device__ __forceinline__ bool mono_dispatch(const HecFieldDev &F, const Pol pol, const uint32_t smem_base, const uint32_t lane,
+                                              const uint32_t nz, const uint32_t lcj, volatile uint32_t *scratch, uint32_t &n_sq, uint32_t &n_zero) {
+    if constexpr (!SPLIT && !ORBIT && D + 1 <= 16) {
+        const uint32_t dense = (nz >> D) ? (1u << (D + 1)) - 1u : (1u << D) - 1u;
+        if (!F.mono_r || nz != dense) return false;
+        constexpr int R = D + 1 <= 8 ? 8 : 16;
+        if (F.mono_r != (uint32_t)R) return false;
+        const uint32_t tp = smem_base + F.pt_off;
+        const uint2 res = (nz >> D) ? hec_radix::radix_mono_x<D, R, D + 1>(pol, tp, F.M, lane, nz, lcj, scratch)
+                                    : hec_radix::radix_mono_x<D, R, D>(pol, tp, F.M, lane, nz, lcj, scratch);
+        n_sq = res.x; n_zero = res.y;
+        return true;
+    } else {
+        return false;
+    }
+}
+
 // SPLIT = false: one warp per curve (batches; P.splits == 1).  SPLIT = true: a separate instantiation for small batches,
 // so that the batch kernel carries none of the split bookkeeping (measured: 610 -> 685 ms on config 4 when it did).
 // ORBIT (HEC_EVAL_ORBIT, never with SPLIT): one representative per Frobenius orbit of cosets, hec_radix::radix_orbit_x.
@@ -452,17 +472,7 @@ __global__ void __launch_bounds__(kThreads, 1) hec_count_radix_kernel(const __gr
                 radix_dispatch<D, hec_radix::ArPacked, ORBIT, !SPLIT && !ORBIT>(F, pol, smem_base, lane, nz, lcj, scratch, part, splits, n_sq, n_zero);
             } else if constexpr (TOP == HEC_TAB_RHALF32) {
                 const hec_radix::HalfS32 pol{smem_base + F.smem_off, smem_base + F.smem_off + 4u * (M >> 1)};
-                bool mono = false;
-                if constexpr (!SPLIT && !ORBIT && D + 1 <= 8) {           // monomial classes on a field with a parity table
-                    const uint32_t dense = (nz >> D) ? (1u << (D + 1)) - 1u : (1u << D) - 1u;
-                    if (F.pt_off && F.radix == 8u && nz == dense) {
-                        const uint2 res = (nz >> D) ? hec_radix::radix_mono8_x<D, D + 1>(pol, smem_base + F.pt_off, M, lane, nz, lcj, scratch)
-                                                    : hec_radix::radix_mono8_x<D, D>(pol, smem_base + F.pt_off, M, lane, nz, lcj, scratch);
-                        n_sq = res.x; n_zero = res.y;
-                        mono = true;
-                    }
-                }
-                if (!mono) {
+                if (!mono_dispatch<D, SPLIT, ORBIT>(F, pol, smem_base, lane, nz, lcj, scratch, n_sq, n_zero)) {
                     if (F.pt_off) {                                       // parity table for the classifying last stage
                         const hec_radix::HalfS32T<true> polp{pol.tb, pol.tbh, smem_base + F.pt_off};
                         radix_dispatch<D, hec_radix::ArScalar, ORBIT, false>(F, polp, smem_base, lane, nz, lcj, scratch, part, splits, n_sq, n_zero);
@@ -472,11 +482,13 @@ __global__ void __launch_bounds__(kThreads, 1) hec_count_radix_kernel(const __gr
                 }
             } else if constexpr (TOP == HEC_TAB_RHALF17) {
                 const hec_radix::HalfS17 pol{smem_base + F.smem_off, smem_base + F.smem_off + 2u * (M >> 1), smem_base + F.smem_off2};
-                if (F.pt_off) {
-                    const hec_radix::HalfS17T<true> polp{pol.tb, pol.tbh, pol.bb, smem_base + F.pt_off};
-                    radix_dispatch<D, hec_radix::ArScalar, ORBIT, false>(F, polp, smem_base, lane, nz, lcj, scratch, part, splits, n_sq, n_zero);
-                } else {
-                    radix_dispatch<D, hec_radix::ArScalar, ORBIT, false>(F, pol, smem_base, lane, nz, lcj, scratch, part, splits, n_sq, n_zero);
+                if (!mono_dispatch<D, SPLIT, ORBIT>(F, pol, smem_base, lane, nz, lcj, scratch, n_sq, n_zero)) {
+                    if (F.pt_off) {
+                        const hec_radix::HalfS17T<true> polp{pol.tb, pol.tbh, pol.bb, smem_base + F.pt_off};
+                        radix_dispatch<D, hec_radix::ArScalar, ORBIT, false>(F, polp, smem_base, lane, nz, lcj, scratch, part, splits, n_sq, n_zero);
+                    } else {
+                        radix_dispatch<D, hec_radix::ArScalar, ORBIT, false>(F, pol, smem_base, lane, nz, lcj, scratch, part, splits, n_sq, n_zero);
+                    }
                 }
             } else if constexpr (TOP == HEC_TAB_GPAIR64) {
                 const hec_radix::PairG64 pol{reinterpret_cast<const uint2 *>(F.gtab)};

@@ -46,6 +46,7 @@ struct HecFieldDev {
                          // parity table (2 bits per n: parity of Z[n], of Z[n + M/2]; four entries per byte), 0: none
     const uint32_t *orb[3]; // HEC_EVAL_ORBIT: Frobenius-orbit representatives of the cosets of mu_R, R = 2, 4, 8 (hec_radix.cuh)
     uint32_t n_orb[3];
+    uint32_t mono_r;        // half-table top field with a parity table: 8 or 16 if dense rows run radix_mono_x at that radix, else 0
     uint32_t orb_fast;      // HEC_EVAL_ORBIT: the field may run radix_orbit_fast_x (PAIR16 and hec_set_fast_tables on)
     const uint32_t *gtab;   // GLOBAL32: extended table in global memory; GPAIR64: the pair table
     const uint32_t *emb;    // q entries: log in F_{q^k} of the embedded coefficient, HEC_LOG_ZERO for 0

@@ -311,7 +311,7 @@ __device__ __forceinline__ uint32_t horner_point(const Pol &pol, const uint32_t 
 template <int D, int R, typename Pol, bool WEIGHTED = false>
 __device__ __noinline__ void exact_queue(const Pol pol, const uint32_t M, const uint32_t nz, const volatile uint32_t *sc,
                                          const uint32_t qn, const uint32_t lane, uint32_t &nz_exact, uint32_t &odd_exact) {
-    constexpr uint32_t LG = R == 8 ? 3u : R == 4 ? 2u : 1u;
+    constexpr uint32_t LG = R == 16 ? 4u : R == 8 ? 3u : R == 4 ? 2u : 1u;
     const uint32_t S = M >> LG;
     const uint32_t j = lane & (uint32_t)(R - 1), slot = lane >> LG;
     for (uint32_t q0 = 0; q0 < qn; q0 += 32u / R) {
@@ -771,20 +771,22 @@ __device__ __forceinline__ void network_mono(const Ar &ar, const Pol &pol, const
     }
 }
 
-template <int D, int NP, typename Pol>
-__device__ __noinline__ uint2 radix_mono8_x(const Pol pol, const uint32_t tp, const uint32_t M, const uint32_t lane,
-                                            const uint32_t nz, const uint32_t lcj, volatile uint32_t *scratch) {
-    constexpr int R = 8;
-    static_assert(NP <= R && NP >= R / 2, "monomial classes: one term per class, classes 0 .. NP-1");
+// R = 8 for at most 8 coefficients (genus <= 2), R = 16 for at most 16 (genus 3 .. 6 on fields with 16 | M, e.g. 49^3 - 1:
+// 9 coefficients, one butterfly with both inputs in the first stage, 24 in the other three, the last 8 from the parity table).
+template <int D, int R, int NP, typename Pol>
+__device__ __noinline__ uint2 radix_mono_x(const Pol pol, const uint32_t tp, const uint32_t M, const uint32_t lane,
+                                           const uint32_t nz, const uint32_t lcj, volatile uint32_t *scratch) {
+    static_assert((R == 8 || R == 16) && NP <= R && NP >= R / 2, "monomial classes: one term per class, classes 0 .. NP-1");
+    constexpr uint32_t LG = R == 16 ? 4u : 3u;
     const ArScalar ar(M);
-    const uint32_t S = M >> 3, unit = S;
+    const uint32_t S = M >> LG, unit = S;
 
     __syncwarp();
     if (lane <= (uint32_t)D) scratch[lane] = lcj;
     __syncwarp();
     uint32_t kc[NP];                                   // log G_r = log c_r + r n for this lane's coset n = base + lane
 #pragma unroll
-    for (int r = 0; r < NP; r++) kc[r] = ar.wrap(__shfl_sync(0xffffffffu, lcj, r) + (uint32_t)r * lane);     // r lane < 8 * 32 <= M
+    for (int r = 0; r < NP; r++) kc[r] = ar.wrap(__shfl_sync(0xffffffffu, lcj, r) + (uint32_t)r * lane);     // r lane < 16 * 32 <= M
 
     uint32_t acc = 0, pushed = 0, qn = 0, nz_exact = 0, odd_exact = 0;
     for (uint32_t base = 0; base < S; base += 32u) {

@@ -547,18 +547,20 @@ def test_fast_tables_off_agrees(torch_cuda, cid, n):
     assert (on[0] == off[0]).all() and (on[1] == off[1]).all()
 
 
-@pytest.mark.parametrize("q,g,n", [(73, 1, 200), (97, 1, 200), (31, 2, 300), (49, 2, 200), (181, 2, 60), (191, 2, 60), (293, 1, 300), (17, 2, 300)])
+@pytest.mark.parametrize("q,g,n", [(73, 1, 200), (97, 1, 200), (31, 2, 300), (49, 2, 200), (181, 2, 60), (191, 2, 60), (293, 1, 300), (17, 2, 300),
+                                   (49, 3, 24), (17, 4, 16), (19, 4, 10)])
 def test_monomial_class_loops_against_oracle(torch_cuda, q, g, n):
-    """Genus <= 2 on fields with 8 | M (hec_radix.cuh: radix_mono8_x for the 32-bit half table + parity table of q = 191,
-    radix_mono8_packed_x for pair tables): dense rows take the monomial-class loop at R = 8, rows with zero coefficients are
-    shifted or fall back to the general loops; both degrees; batches large enough for one warp per curve.  All against the oracle."""
+    """Genus <= 2 on fields with 8 | M (hec_radix.cuh: radix_mono_x at R = 8 for the 32-bit half table + parity table of q = 191,
+    radix_mono8_packed_x for pair tables) and genus 3, 4 on half-table fields with 16 | M (radix_mono_x at R = 16: 49^3, 17^4 with
+    32-bit entries, 19^4 with 16+1-bit planes): dense rows take the monomial-class loop, rows with zero coefficients are shifted
+    or fall back to the general loops; both degrees; batches large enough for one warp per curve.  All against the oracle."""
     rng = np.random.default_rng(1000 * q + g)
     nc = 2 * g + 3
     rows = rng.integers(0, q, size=(n, nc)).astype(np.uint16)
     rows[: n // 4][rng.random((n // 4, nc)) < 0.3] = 0                      # some sparse rows
     rows[:, -1] = np.where(rng.random(n) < 0.5, rng.integers(1, q, n), 0)
     rows[:, -2] = np.where(rows[:, -1] == 0, rng.integers(1, q, n), rows[:, -2])
-    rows = np.concatenate([rows, W.edge_rows(q, g)[:30]])
+    rows = np.concatenate([rows, W.edge_rows(q, g)[:30 if g <= 2 else 6]])
     ocnt, osf, _ = O.count(q, g, rows)
     big = np.tile(rows, (12000 // len(rows) + 1, 1))                        # above 2 * 148 * 32 rows: no split mode
     cnt, sf = _gpu_count(torch_cuda, q, g, big)
