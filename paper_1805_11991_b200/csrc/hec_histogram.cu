@@ -127,17 +127,21 @@ __global__ void __launch_bounds__(kSortThreads) radix_hist_kernel(const unsigned
     hist[(size_t)threadIdx.x * nblocks + blockIdx.x] = h[threadIdx.x];
 }
 
-// exclusive scan of `len` counters in place, one block
+// exclusive scan of `len` counters in place, one block; every thread takes kScanItems consecutive counters per round
+constexpr int kScanItems = 16;
 __global__ void __launch_bounds__(1024) radix_scan_kernel(uint32_t *hist, unsigned long long len) {
     __shared__ uint32_t wsum[32];
     __shared__ uint32_t carry_s;
     if (threadIdx.x == 0) carry_s = 0;
     __syncthreads();
     const uint32_t lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    for (unsigned long long base = 0; base < len; base += 1024) {
-        const unsigned long long i = base + threadIdx.x;
-        const uint32_t v = i < len ? hist[i] : 0;
-        uint32_t s = v;
+    for (unsigned long long base = 0; base < len; base += 1024ull * kScanItems) {
+        const unsigned long long i0 = base + (unsigned long long)threadIdx.x * kScanItems;
+        uint32_t v[kScanItems];
+        uint32_t tsum = 0;
+#pragma unroll
+        for (int j = 0; j < kScanItems; j++) { v[j] = i0 + j < len ? hist[i0 + j] : 0u; tsum += v[j]; }
+        uint32_t s = tsum;
         for (int o = 1; o < 32; o <<= 1) { const uint32_t t = __shfl_up_sync(0xffffffffu, s, o); if (lane >= (uint32_t)o) s += t; }
         if (lane == 31) wsum[warp] = s;
         __syncthreads();
@@ -148,8 +152,9 @@ __global__ void __launch_bounds__(1024) radix_scan_kernel(uint32_t *hist, unsign
         }
         __syncthreads();
         const uint32_t carry = carry_s;
-        const uint32_t excl = carry + (warp ? wsum[warp - 1] : 0) + s - v;
-        if (i < len) hist[i] = excl;
+        uint32_t excl = carry + (warp ? wsum[warp - 1] : 0) + s - tsum;
+#pragma unroll
+        for (int j = 0; j < kScanItems; j++) { if (i0 + j < len) hist[i0 + j] = excl; excl += v[j]; }
         __syncthreads();
         if (threadIdx.x == 0) carry_s = carry + wsum[31];
         __syncthreads();
