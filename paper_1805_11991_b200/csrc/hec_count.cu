@@ -591,7 +591,10 @@ int build_plan(LibState &S, uint32_t q, uint32_t g, int regime, int eval, Device
     // the shift pre-pass pays where the dominant (largest) field has R >= 4 and the rows have at least R coefficients
     plan->shift_R = (radix && plan->f[g - 1].radix >= 4u && 2 * g + 2 >= plan->f[g - 1].radix) ? plan->f[g - 1].radix : 0u;
     // monomial classes (radix_mono_x / radix_mono8_packed_x): every coefficient up to the degree nonzero
-    plan->shift_dense = mono_r != 0 || (radix && D + 1 <= 8 && plan->f[g - 1].radix == 8u && plan->f[g - 1].fast_off != 0);
+    // (not below 2048 elements: there the pre-pass costs more than the rows it moves onto the monomial loop save -- q = 25, g = 2:
+    // 0.23 ms of pre-pass against a 1.4 ms count kernel; rows with a zero coefficient then take radix_fast_x at R = 4)
+    plan->shift_dense = mono_r != 0 || (radix && D + 1 <= 8 && plan->f[g - 1].radix == 8u && plan->f[g - 1].fast_off != 0 &&
+                                        geom[g - 1].M >= 2048u);
     if (plan->shift_dense) plan->shift_R = 8u;
     plan->d_part_codes = reinterpret_cast<const unsigned long long *>(base + part_off);
     plan->n_parts = (uint32_t)parts.size();
