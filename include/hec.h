@@ -279,7 +279,7 @@ typedef struct hec_count_stats {
     uint32_t radix_fields;     /* nibble k-1: radix R used for N_k (0: one Horner chain per x) */
     uint32_t splits;           /* warps per curve: 1 for batches; > 1 when a small batch (down to a single curve) is spread
                                   over the whole GPU, each warp taking a slice of the x range of every field */
-    uint32_t fast_fields;      /* bit k-1: field k carried fast tables (hec_set_fast_tables) */
+    uint32_t fast_fields;      /* bit k-1: field k carried fast tables or a parity table (hec_set_fast_tables) */
     uint32_t chunks;           /* host-pointer calls: number of row chunks pipelined through the copy streams (1: none) */
 } hec_count_stats;
 int hec_last_count_stats(hec_count_stats *out);
@@ -301,8 +301,12 @@ int hec_shift_rows(uint32_t q, uint32_t g, const uint16_t *coeffs, size_t n, uin
  * room, (i) a copy of Z transposed by residue mod R, T[c][j] = Z[c + R j], which serves the first lookup of every
  * residue-class chain of Algorithm 1 line 8 -- there lane l reads Z[delta + R (n0 + l)], R words apart in the
  * plain table (an R-way bank conflict) and consecutive entries of one row of T -- and (ii) e n mod M for the lanes' first
- * cosets and the step 64 e mod M, e = 0 .. 2g+2, so that the per-curve set-up needs no modular reduction.
- * hec_count_stats.fast_fields: bit k-1 set iff field k carried them in the last call.  Takes effect on the next plan build
+ * cosets and the step 64 e mod M, e = 0 .. 2g+2, so that the per-curve set-up needs no modular reduction.  A top field stored as a
+ * half table (Z[0 .. M/2]) gets (iii) a packed parity table, 2 bits per n (parity of Z[n], of Z[n + M/2]), which the last stage of
+ * the evaluation -- it only classifies, PAPER.md:145-147 -- reads instead of the two or three loads of a pair.  With these tables, rows
+ * whose coefficients up to the degree are all nonzero run loops specialised on "one term per residue class" (at most 8 coefficients
+ * and 8 | M, or at most 16 and 16 | M; the shift pre-pass then asks for every coefficient to be nonzero).
+ * hec_count_stats.fast_fields: bit k-1 set iff field k carried such tables in the last call.  Takes effect on the next plan build
  * for a (q, g) (the setting is part of the plan key). */
 int hec_set_fast_tables(int on);
 
