@@ -64,7 +64,7 @@ def algorithmic_lookups(cfg: W.Workload, rows: np.ndarray) -> int:
 
 
 # loads per Zech value (single) and per butterfly pair (Z[n], Z[n + M/2]) in each table layout (hec_radix.cuh)
-LOADS = {0: (1, None), 1: (1, None), 2: (1, None), 3: (2, None), 4: (1, 1), 5: (1, 2), 6: (2, 3), 7: (1, 1)}
+LOADS = {0: (1, None), 1: (1, None), 2: (1, None), 3: (2, None), 4: (1, 1), 5: (1, 2), 6: (2, 3), 7: (1, 1), 8: (1, 1)}
 
 
 def executed_loads(cfg: W.Workload, rows: np.ndarray, stats: dict) -> dict:
@@ -97,7 +97,7 @@ def executed_loads(cfg: W.Workload, rows: np.ndarray, stats: dict) -> dict:
         fast = bool((stats.get("fast_fields", 0) >> (k - 1)) & 1)
         todo = np.ones(n, dtype=bool)
         R = Rf
-        if fast and ncoef > 8 and ncoef <= 16 and mode in (5, 6) and k == cfg.g and M % 16 == 0 and stats.get("eval") in ("auto", "radix8"):
+        if fast and ncoef > 8 and ncoef <= 16 and mode in (5, 6, 8) and k == cfg.g and M % 16 == 0 and stats.get("eval") in ("auto", "radix8"):
             # monomial classes at R = 16 (radix_mono_x): butterflies with both inputs present, the last stage from the parity table
             deg = ncoef - 1 - (~nzm[:, ::-1]).cumprod(axis=1).sum(axis=1)
             dense = nzm.sum(axis=1) == deg + 1
@@ -116,9 +116,9 @@ def executed_loads(cfg: W.Workload, rows: np.ndarray, stats: dict) -> dict:
                                     full += 1
                             pres[blk + j] = pres[blk + j + H] = a or b
                     H //= 2
-                random += cnt_np * (full * pair + last) * (M // 16)
+                random += cnt_np * (full * pair + last * (1 if mode in (5, 6) else pair)) * (M // 16)
             todo &= ~dense
-        if fast and Rf == 8 and ncoef <= 8 and ((mode == 5 and k == cfg.g) or mode == 4):
+        if fast and Rf == 8 and ncoef <= 8 and ((mode in (5, 8) and k == cfg.g) or mode == 4):
             # monomial classes (radix_mono8_x / radix_mono8_packed_x): rows with every coefficient up to the degree nonzero
             # run NP - 4 + 8 butterflies per coset of 8 points and no chain lookup.  Pair table: one load each; 32-bit half
             # table: two loads each except the last four, which read the parity table (one load)
@@ -297,7 +297,7 @@ def gather_ceiling(hec, q, g, mode):
     Mtop = q ** g - 1
     ext_entries = 3 * Mtop + 2 * min(32 * 4, Mtop) * (2 * g + 2)
     where, entries, width = {0: (1, ext_entries, 4), 1: (0, ext_entries, 2), 2: (0, Mtop // 2 + 2, 4), 3: (0, Mtop // 2 + 2, 2),
-                             4: (0, Mtop, 4), 5: (0, Mtop // 2 + 2, 4), 6: (0, Mtop // 2 + 2, 2), 7: (1, 2 * Mtop, 4)}[mode]
+                             4: (0, Mtop, 4), 5: (0, Mtop // 2 + 2, 4), 6: (0, Mtop // 2 + 2, 2), 7: (1, 2 * Mtop, 4), 8: (0, Mtop, 4)}[mode]
     rate, _ = hec.gather_bench(where, max(entries, 1024), width, 1024, 1, 4, 8192 if where == 0 else 1024)
     return rate
 

@@ -366,6 +366,10 @@ int build_plan(LibState &S, uint32_t q, uint32_t g, int regime, int eval, Device
                 if (M > 32768u) return 0;                                 // both halves of a packed value stay below 2 M <= 65536
                 b = (uint64_t)M * 4u;
                 break;
+            case HEC_TAB_SPAIR16:
+                if (M <= 32768u || M >= 65536u) return 0;                 // below: PAIR16 with packed arithmetic; above: 17-bit values
+                b = (uint64_t)M * 4u;
+                break;
             case HEC_TAB_RHALF32:
                 b = ((uint64_t)(M >> 1) + 1u) * 4u;
                 break;
@@ -394,12 +398,14 @@ int build_plan(LibState &S, uint32_t q, uint32_t g, int regime, int eval, Device
             try_mode(global_mode);
         } else if (top && regime == HEC_REGIME_SMEM) {
             try_mode(base_mode);
+            if (radix) try_mode(HEC_TAB_SPAIR16);
             if (m < 0) HEC_FAIL(HEC_ERR_INVALID_ARG, "HEC_REGIME_SMEM: the full Zech table of the largest field does not fit shared memory");
         } else if (top && regime == HEC_REGIME_SMEM_HALF) {
             if (geom[k - 1].M >= kHalfMinM) { try_mode(half_a); try_mode(half_b); }
             if (m < 0) HEC_FAIL(HEC_ERR_INVALID_ARG, "HEC_REGIME_SMEM_HALF: the half table of the largest field does not fit shared memory (or the field is below 2^13 elements)");
         } else {
             try_mode(base_mode);
+            if (radix && top) try_mode(HEC_TAB_SPAIR16);                  // one load per pair where a half table needs two and a fold
             try_mode(half_a);
             try_mode(half_b);
             try_mode(global_mode);
@@ -426,6 +432,10 @@ int build_plan(LibState &S, uint32_t q, uint32_t g, int regime, int eval, Device
                 if (Rm == 8u) radix_of[g - 1] = 8u;      // rows that do not qualify run the general loops at R <= 8 either way
             }
         }
+    }
+    if (radix && S.fast_enabled && mode[g - 1] == HEC_TAB_SPAIR16 && (eval == HEC_EVAL_AUTO || eval == HEC_EVAL_RADIX8) && D + 1 <= 16) {
+        const uint32_t Rm = D + 1 <= 8 ? 8u : 16u;
+        if (geom[g - 1].M % Rm == 0) mono_r = Rm;                        // the pair table serves the last stage too
     }
     if (radix && S.fast_enabled) {
         uint64_t total = ptb;
@@ -482,6 +492,9 @@ int build_plan(LibState &S, uint32_t q, uint32_t g, int regime, int eval, Device
                     fill_half24(*fields[k - 1], t.M, reinterpret_cast<uint16_t *>(dst), reinterpret_cast<int8_t *>(dst + lo_bytes));
                     break;
                 }
+                case HEC_TAB_SPAIR16:
+                    fill_pair16(*fields[k - 1], t.M, reinterpret_cast<uint32_t *>(dst));
+                    break;
                 case HEC_TAB_PAIR16:
                     fill_pair16(*fields[k - 1], t.M, reinterpret_cast<uint32_t *>(dst));
                     if (fastb[k - 1]) {
@@ -811,7 +824,7 @@ int count_impl(LibState &S, uint32_t q, uint32_t g, const uint16_t *coeffs, size
 
     S.stats = hec_count_stats{};
     S.stats.table_mode = (uint32_t)plan->top_mode;
-    S.stats.regime = (plan->top_mode == HEC_TAB_EXT16 || plan->top_mode == HEC_TAB_PAIR16) ? HEC_REGIME_SMEM
+    S.stats.regime = (plan->top_mode == HEC_TAB_EXT16 || plan->top_mode == HEC_TAB_PAIR16 || plan->top_mode == HEC_TAB_SPAIR16) ? HEC_REGIME_SMEM
                      : (plan->top_mode == HEC_TAB_GLOBAL32 || plan->top_mode == HEC_TAB_GPAIR64) ? HEC_REGIME_L2 : HEC_REGIME_SMEM_HALF;
     S.stats.splits = P.splits;
 

@@ -356,7 +356,7 @@ __device__ __forceinline__ void radix_dispatch(const HecFieldDev &F, const Pol p
                                                const uint32_t splits, uint32_t &n_sq, uint32_t &n_zero) {
     using namespace hec_radix;
     const uint32_t R = F.radix, M = F.M, rcpM = F.rcpM;
-    if constexpr (std::is_same<Pol, PairS16>::value) {
+    if constexpr (std::is_same<Pol, PairS16>::value && std::is_same<Ar, ArPacked>::value) {
         if (M <= kDirectMaxM) {                       // tiny field: every point directly (splits: part 0 takes them all)
             uint2 res = make_uint2(0u, 0u);
             if (part == 0u) res = direct_all_x<D>(pol, M, lane, nz, lcj, scratch);
@@ -382,7 +382,7 @@ __device__ __forceinline__ void radix_dispatch(const HecFieldDev &F, const Pol p
         }
     }
     uint2 res;
-    if constexpr (ORBIT && std::is_same<Pol, PairS16>::value) {
+    if constexpr (ORBIT && std::is_same<Pol, PairS16>::value && std::is_same<Ar, ArPacked>::value) {
         if (F.orb_fast) {                                 // every class present at R = 4 or 8: offsets by repeated addition
             if (R >= 8 && all_classes_present<D, 8>(nz)) { res = radix_orbit_fast_x<D, 8>(pol, M, rcpM, lane, nz, lcj, scratch, F.orb[2], F.n_orb[2]); n_sq = res.x; n_zero = res.y; return; }
             if (R >= 4 && all_classes_present<D, 4>(nz)) { res = radix_orbit_fast_x<D, 4>(pol, M, rcpM, lane, nz, lcj, scratch, F.orb[1], F.n_orb[1]); n_sq = res.x; n_zero = res.y; return; }
@@ -405,7 +405,7 @@ __device__ __forceinline__ void radix_dispatch(const HecFieldDev &F, const Pol p
 
 // Monomial classes on a half-table top field with a parity table (hec_radix.cuh: radix_mono_x): rows with every coefficient up to
 // the degree nonzero, at R = 8 (at most 8 coefficients) or R = 16 (9 .. 16).  Returns false if the row or the field does not qualify.
-template <int D, bool SPLIT, bool ORBIT, typename Pol>
+template <int D, bool SPLIT, bool ORBIT, bool PT, typename Pol>
 __device__ __forceinline__ bool mono_dispatch(const HecFieldDev &F, const Pol pol, const uint32_t smem_base, const uint32_t lane,
                                               const uint32_t nz, const uint32_t lcj, volatile uint32_t *scratch, uint32_t &n_sq, uint32_t &n_zero) {
     if constexpr (!SPLIT && !ORBIT && D + 1 <= 16) {
@@ -414,8 +414,8 @@ __device__ __forceinline__ bool mono_dispatch(const HecFieldDev &F, const Pol po
         constexpr int R = D + 1 <= 8 ? 8 : 16;
         if (F.mono_r != (uint32_t)R) return false;
         const uint32_t tp = smem_base + F.pt_off;
-        const uint2 res = (nz >> D) ? hec_radix::radix_mono_x<D, R, D + 1>(pol, tp, F.M, lane, nz, lcj, scratch)
-                                    : hec_radix::radix_mono_x<D, R, D>(pol, tp, F.M, lane, nz, lcj, scratch);
+        const uint2 res = (nz >> D) ? hec_radix::radix_mono_x<D, R, D + 1, PT>(pol, tp, F.M, lane, nz, lcj, scratch)
+                                    : hec_radix::radix_mono_x<D, R, D, PT>(pol, tp, F.M, lane, nz, lcj, scratch);
         n_sq = res.x; n_zero = res.y;
         return true;
     } else {
@@ -472,7 +472,7 @@ __global__ void __launch_bounds__(kThreads, 1) hec_count_radix_kernel(const __gr
                 radix_dispatch<D, hec_radix::ArPacked, ORBIT, !SPLIT && !ORBIT>(F, pol, smem_base, lane, nz, lcj, scratch, part, splits, n_sq, n_zero);
             } else if constexpr (TOP == HEC_TAB_RHALF32) {
                 const hec_radix::HalfS32 pol{smem_base + F.smem_off, smem_base + F.smem_off + 4u * (M >> 1)};
-                if (!mono_dispatch<D, SPLIT, ORBIT>(F, pol, smem_base, lane, nz, lcj, scratch, n_sq, n_zero)) {
+                if (!mono_dispatch<D, SPLIT, ORBIT, true>(F, pol, smem_base, lane, nz, lcj, scratch, n_sq, n_zero)) {
                     if (F.pt_off) {                                       // parity table for the classifying last stage
                         const hec_radix::HalfS32T<true> polp{pol.tb, pol.tbh, smem_base + F.pt_off};
                         radix_dispatch<D, hec_radix::ArScalar, ORBIT, false>(F, polp, smem_base, lane, nz, lcj, scratch, part, splits, n_sq, n_zero);
@@ -482,7 +482,7 @@ __global__ void __launch_bounds__(kThreads, 1) hec_count_radix_kernel(const __gr
                 }
             } else if constexpr (TOP == HEC_TAB_RHALF17) {
                 const hec_radix::HalfS17 pol{smem_base + F.smem_off, smem_base + F.smem_off + 2u * (M >> 1), smem_base + F.smem_off2};
-                if (!mono_dispatch<D, SPLIT, ORBIT>(F, pol, smem_base, lane, nz, lcj, scratch, n_sq, n_zero)) {
+                if (!mono_dispatch<D, SPLIT, ORBIT, true>(F, pol, smem_base, lane, nz, lcj, scratch, n_sq, n_zero)) {
                     if (F.pt_off) {
                         const hec_radix::HalfS17T<true> polp{pol.tb, pol.tbh, pol.bb, smem_base + F.pt_off};
                         radix_dispatch<D, hec_radix::ArScalar, ORBIT, false>(F, polp, smem_base, lane, nz, lcj, scratch, part, splits, n_sq, n_zero);
@@ -490,6 +490,10 @@ __global__ void __launch_bounds__(kThreads, 1) hec_count_radix_kernel(const __gr
                         radix_dispatch<D, hec_radix::ArScalar, ORBIT, false>(F, pol, smem_base, lane, nz, lcj, scratch, part, splits, n_sq, n_zero);
                     }
                 }
+            } else if constexpr (TOP == HEC_TAB_SPAIR16) {
+                const hec_radix::PairS16 pol{smem_base + F.smem_off};
+                if (!mono_dispatch<D, SPLIT, ORBIT, false>(F, pol, smem_base, lane, nz, lcj, scratch, n_sq, n_zero))
+                    radix_dispatch<D, hec_radix::ArScalar, ORBIT, false>(F, pol, smem_base, lane, nz, lcj, scratch, part, splits, n_sq, n_zero);
             } else if constexpr (TOP == HEC_TAB_GPAIR64) {
                 const hec_radix::PairG64 pol{reinterpret_cast<const uint2 *>(F.gtab)};
                 radix_dispatch<D, hec_radix::ArScalar, ORBIT, false>(F, pol, smem_base, lane, nz, lcj, scratch, part, splits, n_sq, n_zero);
@@ -551,6 +555,7 @@ int launch_count(LibState &S, const DevicePlan &plan, HecCountParams P) {
             case HEC_TAB_HALF24: rc = launch_kernel(S, hec_count_kernel<G, U, HEC_TAB_HALF24>, L, P, U); break;
             case HEC_TAB_EXT16: rc = launch_kernel(S, hec_count_kernel<G, U, HEC_TAB_EXT16>, L, P, U); break;
             case HEC_TAB_PAIR16: rc = launch_radix<G, HEC_TAB_PAIR16>(S, L, P, 2); break;
+            case HEC_TAB_SPAIR16: rc = launch_radix<G, HEC_TAB_SPAIR16>(S, L, P, 1); break;
             case HEC_TAB_RHALF32: rc = launch_radix<G, HEC_TAB_RHALF32>(S, L, P, 1); break;
             case HEC_TAB_RHALF17: rc = launch_radix<G, HEC_TAB_RHALF17>(S, L, P, 1); break;
             default: rc = launch_radix<G, HEC_TAB_GPAIR64>(S, L, P, 1); break;
@@ -559,7 +564,7 @@ int launch_count(LibState &S, const DevicePlan &plan, HecCountParams P) {
         if (plan.radix)
             for (uint32_t k = L.k_lo; k <= L.k_hi; k++) {
                 S.stats.radix_fields |= plan.f[k - 1].radix << (4u * (k - 1));
-                if ((plan.f[k - 1].fast_off || plan.f[k - 1].pt_off) && P.splits == 1u && !plan.f[k - 1].orb[0]) S.stats.fast_fields |= 1u << (k - 1);
+                if ((plan.f[k - 1].fast_off || plan.f[k - 1].pt_off || plan.f[k - 1].mono_r) && P.splits == 1u && !plan.f[k - 1].orb[0]) S.stats.fast_fields |= 1u << (k - 1);
             }
     }
     return HEC_OK;

@@ -27,7 +27,8 @@ enum HecTableMode : uint32_t {
     HEC_TAB_PAIR16 = 4,     // M 32-bit entries (Z[n] | Z[n + M/2] << 16), shared memory, M <= 32768
     HEC_TAB_RHALF32 = 5,    // Z[0 .. M/2], 32-bit entries, shared memory
     HEC_TAB_RHALF17 = 6,    // Z[0 .. M/2]: 16-bit plane + byte plane with bit 16 of entries i and M/2 - i, shared memory, M < 2^17
-    HEC_TAB_GPAIR64 = 7     // M entries (Z[n], Z[n + M/2]) as two 32-bit words, global memory (L1/L2-resident regime)
+    HEC_TAB_GPAIR64 = 7,    // M entries (Z[n], Z[n + M/2]) as two 32-bit words, global memory (L1/L2-resident regime)
+    HEC_TAB_SPAIR16 = 8     // PAIR16's entries for 32768 < M < 65536 (values still fit 16 bits): one coset per lane, 32-bit arithmetic
 };
 
 // One field F_{q^k} as the count kernel sees it.

@@ -773,7 +773,7 @@ __device__ __forceinline__ void network_mono(const Ar &ar, const Pol &pol, const
 
 // R = 8 for at most 8 coefficients (genus <= 2), R = 16 for at most 16 (genus 3 .. 6 on fields with 16 | M, e.g. 49^3 - 1:
 // 9 coefficients, one butterfly with both inputs in the first stage, 24 in the other three, the last 8 from the parity table).
-template <int D, int R, int NP, typename Pol>
+template <int D, int R, int NP, bool PT, typename Pol>
 __device__ __noinline__ uint2 radix_mono_x(const Pol pol, const uint32_t tp, const uint32_t M, const uint32_t lane,
                                            const uint32_t nz, const uint32_t lcj, volatile uint32_t *scratch) {
     static_assert((R == 8 || R == 16) && NP <= R && NP >= R / 2, "monomial classes: one term per class, classes 0 .. NP-1");
@@ -796,7 +796,7 @@ __device__ __noinline__ uint2 radix_mono_x(const Pol pol, const uint32_t tp, con
         for (int r = 0; r < R; r++) v[r] = r < NP ? kc[r] : 0u;
 #pragma unroll
         for (int r = 1; r < NP; r++) kc[r] = ar.wrap(kc[r] + 32u * (uint32_t)r);
-        network_mono<R, NP, true>(ar, pol, tp, unit, v, ps, mn);
+        network_mono<R, NP, PT>(ar, pol, tp, unit, v, ps, mn);
         const bool z = mn == 0u;
         if (__any_sync(0xffffffffu, z) || base + 32u > S) {              // rare: a zero somewhere, or the ragged last pass
             const bool valid = base + lane < S, flag = valid && z;

@@ -25,7 +25,7 @@ HEC_ERR_CAPACITY, HEC_ERR_UNSUPPORTED, HEC_ERR_CUDA, HEC_ERR_NOMEM = -5, -6, -7,
 REGIME_AUTO, REGIME_SMEM, REGIME_L2, REGIME_SMEM_HALF = 0, 1, 2, 3
 EVAL_AUTO, EVAL_HORNER, EVAL_RADIX2, EVAL_RADIX4, EVAL_RADIX8, EVAL_ORBIT = 0, 1, 2, 4, 8, 16
 TABLE_MODES = {0: "global32-extended", 1: "smem16-extended", 2: "smem32-half", 3: "smem16+8-half",
-               4: "smem2x16-pair", 5: "smem32-rhalf", 6: "smem16+1-rhalf", 7: "global2x32-pair"}
+               4: "smem2x16-pair", 5: "smem32-rhalf", 6: "smem16+1-rhalf", 7: "global2x32-pair", 8: "smem2x16-pair-scalar"}
 MAX_GENUS = 5
 
 # every symbol include/hec.h declares (tests check the library exports all of them)
