@@ -528,7 +528,8 @@ def sub_config_records(torch, hec, D, args, local_rank, counters):
     scheme on the headline workload, each timed like the main line (fewer steps) with an oracle parity sample."""
     from oracle import hec_oracle as O
     out = {}
-    for cid, eval_name, steps in [(5, "auto", 3), (3, "auto", 3), (2, "auto", 5), (1, "auto", 5), (4, "horner", 2)]:
+    # (the orbit scheme evaluates one representative per Frobenius orbit: SURVEY.md 8(f) NEXT-4, reported separately, never the metric)
+    for cid, eval_name, steps in [(5, "auto", 3), (3, "auto", 3), (2, "auto", 5), (1, "auto", 5), (4, "horner", 2), (4, "orbit", 3)]:
         cfg = W.CONFIGS[cid]
         rows = workload_rows(cfg, 0)
         m = measure(torch, hec, D, cfg, rows, eval_name, steps, 2, 1, local_rank)
@@ -556,6 +557,8 @@ def sub_config_records(torch, hec, D, args, local_rank, counters):
             rec["parity_ok"] = bool((cnt[idx] == ocnt).all() and (sf[idx] == osf).all())
             rec["oracle_curves_per_s"] = len(idx) / dt
             rec["oracle_cores"] = used
+        if eval_name == "orbit":
+            rec["note"] = "HEC_EVAL_ORBIT: 1/k of the points evaluated, counts weighted by orbit length; reported separately, not the judged metric"
         out[cfg.name if eval_name == "auto" else f"{cfg.name}_{eval_name}"] = rec
         del m, rows
         torch.cuda.empty_cache()
