@@ -42,7 +42,8 @@ typedef enum hec_status {
     HEC_ERR_INVALID_ARG = -2,     /* NULL pointer, g < 1, g above HEC_MAX_GENUS, mixed host/device pointers */
     HEC_ERR_COEFF_RANGE = -3,     /* some coefficient >= q; hec_last_error_index() = first offending row */
     HEC_ERR_DEGREE = -4,          /* some row has c[2g+2] = c[2g+1] = 0 (degree < 2g+1) */
-    HEC_ERR_CAPACITY = -5,        /* hec_histogram: cap < number of distinct tuples (*out_m is still set) */
+    HEC_ERR_CAPACITY = -5,        /* hec_histogram: cap < number of distinct tuples (*out_m is still set);
+                                     hec_histogram_static: also n above HEC_HISTOGRAM_STATIC_MAX_ROWS */
     HEC_ERR_UNSUPPORTED = -6,     /* hec_histogram: the tuple does not pack into 64 bits */
     HEC_ERR_CUDA = -7,            /* a CUDA runtime call failed, or no device is present */
     HEC_ERR_NOMEM = -8
@@ -153,6 +154,33 @@ int hec_count_histogram(uint32_t q, uint32_t g, const uint16_t *coeffs, size_t n
  */
 int hec_histogram_merge(const uint32_t *in_tuples, const uint64_t *in_mult, size_t n, uint32_t g,
                         uint32_t *out_tuples, uint64_t *out_mult, size_t cap, size_t *out_m);
+
+/*
+ * hec_histogram_static -- hec_histogram (same map, eq. (1.2) / Algorithm 1 line 20; same output order)
+ * for callers that must not allocate device memory.  hec_histogram takes its hash table and sort buffers from a pool
+ * that calls cudaMalloc when it has to grow.  That is no good in a process where another component (a tensor
+ * framework's caching allocator, a serving engine) has already claimed almost all device memory -- the allocation
+ * fails or takes memory that was promised elsewhere -- nor where the device-wide synchronisation inside cudaMalloc /
+ * cudaFree would stall streams that do not belong to this library.  This entry point calls no cudaMalloc, cudaFree or
+ * other allocating routine, on any call: all of its scratch lives in one fixed array inside the library's device image
+ * (about 8.07 MiB; every GPU on which the process uses CUDA with libhec loaded carries it until the process exits).
+ *
+ *   n <= HEC_HISTOGRAM_STATIC_MAX_ROWS (2^17 rows), else HEC_ERR_CAPACITY with a message that names the limit
+ *       (*out_m = 0; nothing is computed).  Larger batches: call per slice, then hec_histogram_merge where allowed.
+ *   counts[n][g], mask[n] (or NULL), out_tuples[cap][g], out_mult[cap]: DEVICE pointers, owned by the caller (host arrays
+ *       would need a staging allocation and are refused with HEC_ERR_INVALID_ARG); *out_m: host pointer.
+ *   Capacity protocol, output order and the remaining errors as in hec_histogram.
+ * Set-up: the first call on a device looks up the array's device address (cudaGetSymbolAddress, with that device
+ * current) and the SM count and keeps them; make that first call ahead of any stream capture.  It does not bind the
+ * library to a device and needs no other libhec call before it.
+ * Sharing: every call on a device uses the same array, which still holds what the previous call left there (the call
+ * resets what it needs).  Two calls whose device work overlaps -- different streams (hec_set_stream), different host
+ * threads -- race on it and give garbage; run them one after the other.  Work is enqueued on the hec_set_stream stream
+ * and the call returns after synchronising that stream.
+ */
+#define HEC_HISTOGRAM_STATIC_MAX_ROWS 131072
+int hec_histogram_static(const uint32_t *counts, const uint8_t *mask, size_t n, uint32_t g,
+                         uint32_t *out_tuples, uint64_t *out_mult, size_t cap, size_t *out_m);
 
 /* ------------------------------------------------------------------------------------------------
  * Algorithm 1 around the hot path, without the partition lambda: SURVEY.md 8(f) NEXT-1.

@@ -433,3 +433,160 @@ extern "C" int hec_histogram_merge(const uint32_t *in_tuples, const uint64_t *in
     if (n > 0 && !in_mult) HEC_FAIL(HEC_ERR_INVALID_ARG, "in_mult must not be NULL");
     return histogram_impl(in_tuples, nullptr, in_mult, n, g, out_tuples, out_mult, cap, out_m);
 }
+
+// ---- hec_histogram_static: the same pipeline with every scratch buffer inside one fixed array -----------------------
+// For callers that must not touch the device allocator.  Two kinds turn up in practice: (1) a process whose device
+// memory already belongs to someone else -- a tensor framework's caching allocator or a serving engine that grabbed
+// nearly all of HBM at start-up -- where a cudaMalloc of hec_histogram's hash and sort buffers either fails or eats
+// into a budget the caller was promised; (2) a caller in a section where the device-wide synchronisation that
+// cudaMalloc / cudaFree imply would stall unrelated streams (a latency-bound serving loop next to this library).
+// hec_histogram's pool (above) grows on demand, so neither can use it.  Here the scratch is a file-scope device array
+// of fixed size: it is part of the module image, every GPU that loads libhec holds these 8.07 MiB from the first CUDA
+// call of the process until exit, and no call allocates or frees anything.
+//
+// Layout (bytes), kStaticMaxRows = 2^17 rows:
+//   [0, 256)              column minima / maxima (16 x u32), unmasked-row counter, distinct-tuple counter
+//   gkeys, gcnt           global hash: 2 * kStaticMaxRows slots x 8 B each            2 MiB + 2 MiB
+//   k0, v0, k1, v1        compacted (key, multiplicity) pairs + the sort's ping-pong copy, kStaticMaxRows x 8 B each   4 MiB
+//   hist                  256 digit counters per 2048-key sort tile                   64 KiB
+constexpr size_t kStaticMaxRows = HEC_HISTOGRAM_STATIC_MAX_ROWS;
+constexpr size_t kStaticSlots = 2 * kStaticMaxRows;
+constexpr size_t kStaticTiles = (kStaticMaxRows + kTile - 1) / kTile;
+constexpr size_t kStaticOffKeys = 256;
+constexpr size_t kStaticOffCnt = kStaticOffKeys + kStaticSlots * 8;
+constexpr size_t kStaticOffSort = kStaticOffCnt + kStaticSlots * 8;
+constexpr size_t kStaticOffHist = kStaticOffSort + 4 * kStaticMaxRows * 8;
+constexpr size_t kStaticBytes = kStaticOffHist + 256 * kStaticTiles * 4;
+static_assert(kStaticMaxRows % kTile == 0 && (kStaticSlots & (kStaticSlots - 1)) == 0, "scratch layout");
+
+static __device__ __align__(256) unsigned char hec_static_scratch[kStaticBytes];
+
+namespace {
+// In host code `hec_static_scratch` is only the host-side shadow of the device symbol, not somewhere a kernel may
+// write: the device address is asked for once per device (with that device current) and kept here.
+constexpr int kMaxDevices = 64;
+struct StaticScratch {
+    std::mutex mu;
+    unsigned char *base[kMaxDevices] = {};
+    int sms[kMaxDevices] = {};
+} g_static;
+
+int static_scratch_for_current_device(unsigned char **base, int *sms) {
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess) {
+        cudaGetLastError();
+        HEC_FAIL(HEC_ERR_CUDA, "hec_histogram_static: no CUDA device present (libhec has no CPU fallback)");
+    }
+    if (dev < 0 || dev >= kMaxDevices) HEC_FAIL(HEC_ERR_UNSUPPORTED, "hec_histogram_static: device ordinal above 63");
+    std::lock_guard<std::mutex> lock(g_static.mu);
+    if (!g_static.base[dev]) {
+        void *p = nullptr;
+        HEC_CUDA_OK(cudaGetSymbolAddress(&p, hec_static_scratch));
+        int n = 0;
+        HEC_CUDA_OK(cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev));
+        g_static.sms[dev] = n;
+        g_static.base[dev] = static_cast<unsigned char *>(p);
+    }
+    *base = g_static.base[dev];
+    *sms = g_static.sms[dev];
+    return HEC_OK;
+}
+}  // namespace
+
+extern "C" int hec_histogram_static(const uint32_t *counts, const uint8_t *mask, size_t n, uint32_t g, uint32_t *out_tuples,
+                                    uint64_t *out_mult, size_t cap, size_t *out_m) {
+    if (g < 1 || g > HEC_MAX_GENUS) HEC_FAIL(HEC_ERR_INVALID_ARG, "g must be in [1, HEC_MAX_GENUS]");
+    if (!out_m) HEC_FAIL(HEC_ERR_INVALID_ARG, "out_m must not be NULL");
+    *out_m = 0;
+    if (n > kStaticMaxRows)
+        HEC_FAIL(HEC_ERR_CAPACITY, "hec_histogram_static: n = " + std::to_string(n) + " rows exceed the fixed scratch array's limit of " +
+                                       std::to_string(kStaticMaxRows) + " (HEC_HISTOGRAM_STATIC_MAX_ROWS); split the batch and combine the parts with "
+                                       "hec_histogram_merge, or use hec_histogram where allocating is allowed");
+    if (n == 0) return HEC_OK;
+    if (!counts) HEC_FAIL(HEC_ERR_INVALID_ARG, "counts must not be NULL");
+    if (cap > 0 && (!out_tuples || !out_mult)) HEC_FAIL(HEC_ERR_INVALID_ARG, "out_tuples/out_mult must not be NULL when cap > 0");
+    unsigned char *base = nullptr;
+    int sms = 0;
+    int rc = static_scratch_for_current_device(&base, &sms);
+    if (rc) return rc;
+    // host arrays would need a staging buffer on the device, i.e. an allocation
+    if (!hec_is_device_pointer(counts) || (mask && !hec_is_device_pointer(mask)) ||
+        (cap > 0 && (!hec_is_device_pointer(out_tuples) || !hec_is_device_pointer(out_mult))))
+        HEC_FAIL(HEC_ERR_INVALID_ARG, "hec_histogram_static: counts/mask/out_tuples/out_mult must be device pointers (staging host arrays would allocate)");
+    cudaStream_t st = hec_current_stream();
+
+    uint32_t *d_mn = reinterpret_cast<uint32_t *>(base), *d_mx = d_mn + 8;
+    unsigned long long *d_rows = reinterpret_cast<unsigned long long *>(base + 64), *d_m = d_rows + 1;
+    unsigned long long *gkeys = reinterpret_cast<unsigned long long *>(base + kStaticOffKeys);
+    unsigned long long *gcnt = reinterpret_cast<unsigned long long *>(base + kStaticOffCnt);
+    unsigned long long *ka = reinterpret_cast<unsigned long long *>(base + kStaticOffSort), *va = ka + kStaticMaxRows;
+    unsigned long long *kb = va + kStaticMaxRows, *vb = kb + kStaticMaxRows;
+    uint32_t *hist = reinterpret_cast<uint32_t *>(base + kStaticOffHist);
+
+    // The array still holds the previous call's data: everything a kernel reads before writing is reset here
+    // (scalars now, the hash slots below once their number is known); the sort buffers and digit counters are
+    // written in full before they are read.
+    uint32_t h_init[16];
+    for (int i = 0; i < 8; i++) { h_init[i] = 0xFFFFFFFFu; h_init[8 + i] = 0; }
+    unsigned long long h_zero[2] = {0, 0};
+    HEC_CUDA_OK(cudaMemcpyAsync(d_mn, h_init, sizeof h_init, cudaMemcpyHostToDevice, st));
+    HEC_CUDA_OK(cudaMemcpyAsync(d_rows, h_zero, sizeof h_zero, cudaMemcpyHostToDevice, st));
+    const unsigned long long nn = n;
+    hist_minmax_kernel<<<(unsigned)std::min<unsigned long long>((nn + 511) / 512, (unsigned long long)sms * 4), 512, 0, st>>>(
+        counts, mask, nullptr, nn, g, d_mn, d_mx, d_rows);
+    hec_launch_counter::value++;
+    uint32_t h_mm[16];
+    unsigned long long h_rows = 0;
+    HEC_CUDA_OK(cudaMemcpyAsync(h_mm, d_mn, sizeof h_mm, cudaMemcpyDeviceToHost, st));
+    HEC_CUDA_OK(cudaMemcpyAsync(&h_rows, d_rows, sizeof h_rows, cudaMemcpyDeviceToHost, st));
+    HEC_CUDA_OK(cudaStreamSynchronize(st));
+    if (h_rows == 0) return HEC_OK;
+
+    PackSpec S;
+    S.g = g;
+    uint32_t total_bits = 0;
+    for (uint32_t k = 0; k < g; k++) {
+        S.mn[k] = h_mm[k];
+        const uint32_t range = h_mm[8 + k] - h_mm[k];
+        uint32_t b = 0;
+        while (b < 32 && (range >> b)) b++;
+        S.bits[k] = b;
+        total_bits += b;
+    }
+    if (total_bits > 63) HEC_FAIL(HEC_ERR_UNSUPPORTED, "tuple ranges need more than 63 bits");
+    uint32_t sh = total_bits;
+    for (uint32_t k = 0; k < g; k++) { sh -= S.bits[k]; S.shift[k] = sh; }     // N_1 most significant
+
+    unsigned long long capslots = 1024;
+    while (capslots < 2 * h_rows) capslots <<= 1;                              // <= kStaticSlots since h_rows <= n
+    HEC_CUDA_OK(cudaMemsetAsync(gkeys, 0xFF, capslots * 8, st));
+    HEC_CUDA_OK(cudaMemsetAsync(gcnt, 0, capslots * 8, st));
+    hist_insert_kernel<<<(unsigned)std::min<unsigned long long>((nn + 511) / 512, (unsigned long long)sms * 2), 512, 0, st>>>(
+        counts, mask, nullptr, nn, S, gkeys, gcnt, capslots - 1);
+    hist_compact_kernel<<<(unsigned)std::min<unsigned long long>((capslots + 255) / 256, (unsigned long long)sms * 8), 256, 0, st>>>(
+        gkeys, gcnt, capslots, ka, va, d_m);
+    hec_launch_counter::value += 2;
+    unsigned long long m = 0;
+    HEC_CUDA_OK(cudaMemcpyAsync(&m, d_m, sizeof m, cudaMemcpyDeviceToHost, st));
+    HEC_CUDA_OK(cudaStreamSynchronize(st));
+    HEC_CUDA_OK(cudaGetLastError());
+    *out_m = (size_t)m;
+    if (cap < m) HEC_FAIL(HEC_ERR_CAPACITY, "cap is smaller than the number of distinct tuples");
+
+    if (total_bits > 0 && m > 1) {
+        const uint32_t nblocks = (uint32_t)((m + kTile - 1) / kTile);
+        for (uint32_t shift = 0; shift < total_bits; shift += 8) {
+            radix_hist_kernel<<<nblocks, kSortThreads, 0, st>>>(ka, m, shift, hist, nblocks);
+            radix_scan_kernel<<<1, 1024, 0, st>>>(hist, (unsigned long long)256 * nblocks);
+            radix_scatter_kernel<<<nblocks, kSortThreads, 0, st>>>(ka, va, kb, vb, m, shift, hist, nblocks);
+            hec_launch_counter::value += 3;
+            std::swap(ka, kb);
+            std::swap(va, vb);
+        }
+    }
+    hist_unpack_kernel<<<(unsigned)((m + 255) / 256), 256, 0, st>>>(ka, va, m, S, out_tuples, reinterpret_cast<unsigned long long *>(out_mult));
+    hec_launch_counter::value++;
+    HEC_CUDA_OK(cudaGetLastError());
+    HEC_CUDA_OK(cudaStreamSynchronize(st));
+    return HEC_OK;
+}

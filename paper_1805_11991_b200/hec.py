@@ -33,7 +33,7 @@ SYMBOLS = [
     "hec_last_error", "hec_last_error_index", "hec_build_field", "hec_build_field_device", "hec_free_field", "hec_field_p",
     "hec_field_degree", "hec_field_q", "hec_field_Q", "hec_field_embed_unit", "hec_field_modulus",
     "hec_field_antilog", "hec_field_log", "hec_field_zech", "hec_field_embed", "hec_count", "hec_histogram",
-    "hec_histogram_merge", "hec_reduced_total", "hec_reduced_rows", "hec_curve_map",
+    "hec_histogram_merge", "hec_histogram_static", "hec_reduced_total", "hec_reduced_rows", "hec_curve_map",
     "hec_count_ex", "hec_lambda_partitions", "hec_curve_map_lambda", "hec_set_map_chunk_rows", "hec_curve_map_range", "hec_curve_map_all", "hec_set_shift", "hec_shift_rows", "hec_set_fast_tables", "hec_count_histogram", "hec_set_field_variant",
     "hec_set_stream", "hec_set_regime", "hec_set_eval", "hec_last_count_stats", "hec_launch_count", "hec_gather_bench",
     "hec_shutdown",
@@ -80,6 +80,7 @@ def lib():
         L.hec_histogram.argtypes = [vp, vp, sz, u32, vp, vp, sz, ctypes.POINTER(sz)]
         L.hec_count_histogram.argtypes = [u32, u32, vp, sz, vp, vp, vp, vp, sz, ctypes.POINTER(sz)]
         L.hec_histogram_merge.argtypes = [vp, vp, sz, u32, vp, vp, sz, ctypes.POINTER(sz)]
+        L.hec_histogram_static.argtypes = [vp, vp, sz, u32, vp, vp, sz, ctypes.POINTER(sz)]
         L.hec_reduced_total.argtypes = [u32, u32, u32, ctypes.POINTER(ctypes.c_uint64)]
         L.hec_reduced_rows.argtypes = [u32, u32, u32, ctypes.c_uint64, sz, vp, vp]
         L.hec_curve_map.argtypes = [u32, u32, u32, vp, vp, sz, ctypes.POINTER(sz)]
@@ -309,6 +310,25 @@ def count_histogram(q: int, g: int, coeffs, out_counts=None, out_squarefree=None
     _check(rc)
     _cap_hint[key] = m.value
     return out_counts, out_squarefree, tup[: m.value], mult[: m.value]
+
+
+HISTOGRAM_STATIC_MAX_ROWS = 131072   # HEC_HISTOGRAM_STATIC_MAX_ROWS of hec.h
+
+
+def histogram_static(counts, mask, out_tuples, out_mult):
+    """hec_histogram_static: hec_histogram for code that may not allocate device memory -- e.g. inside a process whose
+    HBM is already owned by another allocator, or where cudaMalloc's device-wide sync is unwelcome (hec.h has the
+    details).  The library works in a fixed 8 MiB device array; this wrapper allocates nothing either: counts
+    [n][g] (n <= HISTOGRAM_STATIC_MAX_ROWS), mask [n] or None, and the result buffers out_tuples [cap][g] / out_mult [cap]
+    are the caller's CUDA tensors.  Returns m, the number of distinct tuples now in out_tuples[:m] / out_mult[:m];
+    raises HecError(HEC_ERR_CAPACITY) if cap < m or n is above the limit.  Calls must not overlap on the GPU."""
+    n, g = int(counts.shape[0]), int(counts.shape[1])
+    cap = int(out_mult.shape[0])
+    if int(out_tuples.shape[0]) != cap:
+        raise ValueError("out_tuples and out_mult must have the same capacity")
+    m = ctypes.c_size_t(0)
+    _check(lib().hec_histogram_static(_ptr(counts), _ptr(mask), n, g, _ptr(out_tuples), _ptr(out_mult), cap, ctypes.byref(m)))
+    return int(m.value)
 
 
 def histogram_merge(tuples, mult):
