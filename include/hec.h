@@ -277,7 +277,8 @@ typedef enum hec_eval {
                                   R-point butterfly network of Zech additions, one table entry serving a + w b and a - w b
                                   (about 5x fewer lookups at degree 10).  Tables: pairs (Z[n], Z[n + M/2]) or half tables. */
     HEC_EVAL_HORNER = 1,       /* the paper's scheme (Algorithm 1 line 8): one Horner chain per x */
-    HEC_EVAL_RADIX2 = 2,       /* as AUTO with R capped at 2 / 4 / 8 (tuning and tests) */
+    HEC_EVAL_RADIX2 = 2,       /* as AUTO with R capped at 2 / 4 / 8 (tuning and tests); no loop runs above the cap: the
+                                  R = 16 monomial-class loop for rows of 9..16 coefficients is AUTO's alone */
     HEC_EVAL_RADIX4 = 4,
     HEC_EVAL_RADIX8 = 8,
     HEC_EVAL_ORBIT = 16        /* as AUTO, but one representative per Frobenius orbit of x (f(x^q) = f(x)^q for f over F_q),
@@ -286,7 +287,8 @@ typedef enum hec_eval {
 } hec_eval;
 int hec_set_eval(int eval);
 
-/* Statistics of the last hec_count on this thread's library state: device time of the count kernel(s) and
+/* Statistics of the last hec_count of the process (the library state is ONE process-global object behind a mutex,
+ * not per thread: with several host threads this is whichever hec_count finished last): device time of the count kernel(s) and
  * of the squarefree kernel (CUDA events on the launch stream, ms), number of kernel launches (one count
  * launch per group of fields whose tables share one shared-memory image, plus the squarefree kernel), the
  * regime used for the largest field (hec_regime) and its table layout -- Horner kernel: 0 global 32-bit
@@ -295,8 +297,11 @@ int hec_set_eval(int eval);
  * dynamic shared memory per CTA, grid and block size of the last count launch, independent x (Horner) or
  * cosets (radix) per lane per pass, and the radix of every field. */
 typedef struct hec_count_stats {
-    float count_kernel_ms;
-    float squarefree_kernel_ms;
+    float count_kernel_ms;     /* chunks == 1: the count launch(es) alone.  chunks > 1 (host-pointer calls from 2^20 rows on): from
+                                  the first chunk's launch to the end of the last chunk's count kernel, which includes the
+                                  waits for the H2D copies and the squarefree kernels of the earlier chunks -- a span, not a
+                                  kernel time; time kernels on device-resident inputs */
+    float squarefree_kernel_ms;/* chunks > 1: the last chunk's squarefree kernel only */
     uint32_t launches;
     uint32_t regime;
     uint32_t smem_bytes;
@@ -344,7 +349,9 @@ int hec_set_fast_tables(int on);
  * Every output of hec_count / hec_count_ex / hec_curve_map must be unchanged.  F_q itself (k = 1) keeps its smallest
  * polynomial: for q = p^r, r > 1 it fixes the encoding of the inputs, and the reduced polynomials of Algorithm 1 are
  * defined through its generator.  hec_build_field / hec_build_field_device always return the smallest.
- * Drops the cached plans; v <= 16. */
+ * Drops the cached plans; v <= 16.  The setting is checked when a field is built: if F_{q^k} has no more than v primitive
+ * polynomials of its degree (F_9 has two), the next hec_count fails with HEC_ERR_INVALID_FIELD and a message that names
+ * the variant.  hec_shutdown() puts the setting back to 0. */
 int hec_set_field_variant(uint32_t v);
 
 /* Total number of kernels launched by this library since load (bench.py's gpu_launches). */
@@ -362,7 +369,12 @@ uint64_t hec_launch_count(void);
 int hec_gather_bench(int where, uint32_t entries, uint32_t entry_bytes, uint32_t block, uint32_t ctas_per_sm,
                      uint32_t chains, uint32_t lookups_per_lane, double *out_lookups_per_s, float *out_ms);
 
-/* Release cached fields, device plans and staging buffers. */
+/* Release cached fields, device plans, staging buffers, the histogram pool and the internal streams and events; the next
+ * call binds to the device that is current then.  Two settings are tied to what is released and go back to their
+ * defaults: the stream (hec_set_stream: a stream of the old device is not a valid handle on another one) becomes the
+ * default stream, the field variant becomes 0.  hec_set_regime / hec_set_eval / hec_set_shift / hec_set_fast_tables /
+ * hec_set_map_chunk_rows persist.  The fixed scratch array of hec_histogram_static is not released (it is part of the
+ * module image). */
 void hec_shutdown(void);
 
 #ifdef __cplusplus

@@ -427,7 +427,8 @@ int build_plan(LibState &S, uint32_t q, uint32_t g, int regime, int eval, Device
             ptb = parity_table_bytes(geom[g - 1].M);
             // monomial classes (radix_mono_x): R = 8 for at most 8 coefficients, R = 16 for 9 .. 16, where R | M
             const uint32_t Rm = D + 1 <= 8 ? 8u : 16u;
-            if ((eval == HEC_EVAL_AUTO || eval == HEC_EVAL_RADIX8) && D + 1 <= 16 && geom[g - 1].M % Rm == 0 && geom[g - 1].M >= 4096u) {
+            // (an explicit HEC_EVAL_RADIX8 request stays a pure radix-8 run: the R = 16 loop is AUTO's alone)
+            if ((eval == HEC_EVAL_AUTO || (eval == HEC_EVAL_RADIX8 && Rm == 8u)) && D + 1 <= 16 && geom[g - 1].M % Rm == 0 && geom[g - 1].M >= 4096u) {
                 mono_r = Rm;
                 if (Rm == 8u) radix_of[g - 1] = 8u;      // rows that do not qualify run the general loops at R <= 8 either way
             }
@@ -435,7 +436,7 @@ int build_plan(LibState &S, uint32_t q, uint32_t g, int regime, int eval, Device
     }
     if (radix && S.fast_enabled && mode[g - 1] == HEC_TAB_SPAIR16 && (eval == HEC_EVAL_AUTO || eval == HEC_EVAL_RADIX8) && D + 1 <= 16) {
         const uint32_t Rm = D + 1 <= 8 ? 8u : 16u;
-        if (geom[g - 1].M % Rm == 0) mono_r = Rm;                        // the pair table serves the last stage too
+        if (geom[g - 1].M % Rm == 0 && (eval == HEC_EVAL_AUTO || Rm == 8u)) mono_r = Rm;   // the pair table serves the last stage too
     }
     if (radix && S.fast_enabled) {
         uint64_t total = ptb;
@@ -734,11 +735,14 @@ struct CountTail {
 };
 
 int finish_count(LibState &S, CountTail &T) {
-    if (T.pending) {
-        HEC_CUDA_OK(cudaStreamSynchronize(S.copy_out));
-        T.pending = false;
+    const cudaError_t e_out = T.pending ? cudaStreamSynchronize(S.copy_out) : cudaSuccess;
+    T.pending = false;
+    const cudaError_t e_main = cudaStreamSynchronize(S.stream);   // waited for even when the copy stream failed
+    if (e_out != cudaSuccess || e_main != cudaSuccess) {
+        cudaGetLastError();
+        hec_set_error(HEC_ERR_CUDA, std::string("hec_count: ") + cudaGetErrorString(e_out != cudaSuccess ? e_out : e_main));
+        return HEC_ERR_CUDA;
     }
-    HEC_CUDA_OK(cudaStreamSynchronize(S.stream));
     cudaEventElapsedTime(&S.stats.count_kernel_ms, S.ev[0], S.ev[1]);
     cudaEventElapsedTime(&S.stats.squarefree_kernel_ms, S.ev[1], S.ev[2]);
     if (T.err[0] != ~0ull) {
@@ -751,6 +755,22 @@ int finish_count(LibState &S, CountTail &T) {
     }
     return HEC_OK;
 }
+
+// Error exits of count_impl: copies of earlier chunks may still be running on the copy streams into the caller's host
+// buffers and the staging buffer.  Unless disarmed, the guard waits for all three streams, so that after a failing
+// call the caller may free or reuse its buffers.
+struct DrainOnError {
+    LibState &S;
+    bool armed = true;
+    explicit DrainOnError(LibState &s) : S(s) {}
+    ~DrainOnError() {
+        if (!armed) return;
+        if (S.copy_in) cudaStreamSynchronize(S.copy_in);
+        if (S.copy_out) cudaStreamSynchronize(S.copy_out);
+        cudaStreamSynchronize(S.stream);
+        cudaGetLastError();
+    }
+};
 
 int count_impl(LibState &S, uint32_t q, uint32_t g, const uint16_t *coeffs, size_t n, uint32_t *out_counts, uint8_t *out_squarefree,
                uint32_t *out_roots, uint8_t *out_lambda, bool keep_device, CountTail &T) {
@@ -845,6 +865,7 @@ int count_impl(LibState &S, uint32_t q, uint32_t g, const uint16_t *coeffs, size
         HEC_CUDA_OK(cudaStreamWaitEvent(S.copy_out, S.ev_chunk[0], 0));
     }
     HEC_CUDA_OK(cudaEventRecord(S.ev[0], S.stream));
+    DrainOnError drain(S);
     for (int c = 0; c < chunks; c++) {
         const size_t lo = n * (size_t)c / chunks, hi = n * (size_t)(c + 1) / chunks, nc = hi - lo;
         if (nc == 0) continue;
@@ -898,6 +919,7 @@ int count_impl(LibState &S, uint32_t q, uint32_t g, const uint16_t *coeffs, size
     HEC_CUDA_OK(cudaEventRecord(S.ev[2], S.stream));
     HEC_CUDA_OK(cudaMemcpyAsync(T.err, plan->d_err, sizeof T.err, cudaMemcpyDeviceToHost, S.stream));
     T.pending = chunks > 1;
+    drain.armed = false;                                       // from here on finish_count waits for the copies
     if (keep_device) return HEC_OK;
     return finish_count(S, T);
 }
@@ -995,16 +1017,18 @@ int hec_shift_rows(uint32_t q, uint32_t g, const uint16_t *coeffs, size_t n, uin
         return HEC_OK;
     }
     void *d_in = nullptr;
+    cudaError_t ce = cudaSuccess;
     if (!dev) {
         if (cudaMalloc(&d_in, bytes) != cudaSuccess) { cudaGetLastError(); HEC_FAIL(HEC_ERR_NOMEM, "cannot allocate device rows"); }
-        cudaMemcpyAsync(d_in, coeffs, bytes, cudaMemcpyHostToDevice, S.stream);
+        ce = cudaMemcpyAsync(d_in, coeffs, bytes, cudaMemcpyHostToDevice, S.stream);
     }
-    rc = run_shift(S, *plan, dev ? coeffs : static_cast<const uint16_t *>(d_in), n, dev ? out_coeffs : nullptr);
-    if (rc == HEC_OK && !dev) cudaMemcpyAsync(out_coeffs, S.d_shift, bytes, cudaMemcpyDeviceToHost, S.stream);
-    const cudaError_t ce = cudaStreamSynchronize(S.stream);
+    if (ce == cudaSuccess) rc = run_shift(S, *plan, dev ? coeffs : static_cast<const uint16_t *>(d_in), n, dev ? out_coeffs : nullptr);
+    if (ce == cudaSuccess && rc == HEC_OK && !dev) ce = cudaMemcpyAsync(out_coeffs, S.d_shift, bytes, cudaMemcpyDeviceToHost, S.stream);
+    const cudaError_t se = cudaStreamSynchronize(S.stream);    // always: nothing may still run when d_in is freed
+    if (ce == cudaSuccess) ce = se;
     if (d_in) cudaFree(d_in);
     if (rc) return rc;
-    if (ce != cudaSuccess) { hec_set_error(HEC_ERR_CUDA, cudaGetErrorString(ce)); return HEC_ERR_CUDA; }
+    if (ce != cudaSuccess) { cudaGetLastError(); hec_set_error(HEC_ERR_CUDA, std::string("hec_shift_rows: ") + cudaGetErrorString(ce)); return HEC_ERR_CUDA; }
     return HEC_OK;
 }
 
@@ -1031,6 +1055,10 @@ void hec_shutdown(void) {
     if (g_state.copy_in) { cudaStreamDestroy(g_state.copy_in); g_state.copy_in = nullptr; }
     if (g_state.copy_out) { cudaStreamDestroy(g_state.copy_out); g_state.copy_out = nullptr; }
     g_state.device_ready = false;                 // the next call binds to the device current then
+    // Settings that belong to the released device or representation go back to their defaults: a stream of the old device
+    // is an invalid handle on the next one, and plans of another field variant are gone with the plans.
+    g_state.stream = nullptr;
+    hec_set_field_variant_impl(0);
 }
 
 }  // extern "C"

@@ -127,7 +127,11 @@ hec_field *build_field_impl(uint32_t p, uint32_t r, uint32_t k, uint32_t skip = 
         }
         if (found && seen < skip) { seen++; found = false; }
     }
-    if (!found) { hec_set_error(HEC_ERR_INVALID_FIELD, "no primitive polynomial found"); return nullptr; }
+    if (!found) {
+        if (skip) hec_set_error(HEC_ERR_INVALID_FIELD, "hec_set_field_variant: variant " + std::to_string(skip) + " exceeds the number of primitive polynomials of this field (" + std::to_string(seen) + " of that degree)");
+        else hec_set_error(HEC_ERR_INVALID_FIELD, "no primitive polynomial found");
+        return nullptr;
+    }
     F->modulus = R.mod;
 
     F->log.assign(Q, M);                       // log[0] = Q-1 (encoding (3.1))

@@ -231,7 +231,11 @@ hec_field *hec_build_field_device_impl(uint32_t p, uint32_t r, uint32_t k, uint3
         found = prim;
         if (found && seen < skip) { seen++; found = false; }
     }
-    if (!found) { hec_set_error(HEC_ERR_INVALID_FIELD, "no primitive polynomial found"); return nullptr; }
+    if (!found) {
+        if (skip) hec_set_error(HEC_ERR_INVALID_FIELD, "hec_set_field_variant: variant " + std::to_string(skip) + " exceeds the number of primitive polynomials of this field (" + std::to_string(seen) + " of that degree)");
+        else hec_set_error(HEC_ERR_INVALID_FIELD, "no primitive polynomial found");
+        return nullptr;
+    }
     F->modulus = modulus;
 
     // ---- device tables

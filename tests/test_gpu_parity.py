@@ -609,3 +609,25 @@ def test_other_primitive_polynomial_changes_the_tables_not_the_map(torch_cuda):
     assert (ref[0] == got[0]).all() and (ref[1] == got[1]).all()
     for x, y in zip(r0, r1):
         assert bool((x == y).all())
+
+
+def test_field_variant_beyond_the_fields_polynomials_and_shutdown_resets(torch_cuda):
+    """F_9 has two primitive quadratics: variant 2 cannot be built and the error says so (not "no primitive polynomial
+    found"); hec_shutdown puts the variant and the stream setting back to their defaults (hec.h)."""
+    if torch_cuda.eval_scheme != "auto":
+        pytest.skip("one scheme is enough")
+    rows = W.generate(W.CONFIGS[1])
+    ref, _ = hec.count(3, 2, _dev(torch_cuda, rows))
+    try:
+        hec.set_field_variant(2)
+        with pytest.raises(hec.HecError) as e:
+            hec.count(3, 2, _dev(torch_cuda, rows))
+        assert e.value.code == hec.HEC_ERR_INVALID_FIELD and "variant 2" in str(e.value)
+        hec.set_field_variant(1)
+        hec.shutdown()                                                   # variant back to 0, stream back to the default
+        got, _ = hec.count(3, 2, _dev(torch_cuda, rows))
+        assert bool((got == ref).all())
+        assert hec.last_count_stats()["launches"] >= 1
+    finally:
+        hec.set_field_variant(0)
+        hec.set_stream(torch_cuda.cuda.current_stream().cuda_stream)
