@@ -165,6 +165,29 @@ def test_curve_map_all_is_the_union_of_both_degrees(cuda, q, g):
     assert got == wantl
 
 
+@pytest.mark.parametrize("q,g,d,lam", [(13, 2, 5, False), (7, 3, 7, True)])
+def test_device_resident_curve_map_and_exchange_merge(cuda, q, g, d, lam):
+    """The device flow of distributed.global_curve_map on ONE GPU: hec_curve_map_range with device=True (outputs written
+    into CUDA tensors) equals the host-output call, and the gathered partial maps -- here simply concatenated, as the
+    all-gather would deliver them -- go through distributed._to_device / distributed._merge (hec_histogram_merge on the
+    device, ordered on torch's stream) to the full map."""
+    from paper_1805_11991_b200 import distributed as D, workloads as W
+    torch = cuda
+    total = hec.reduced_total(q, g, d)
+    parts_t, parts_w = [], []
+    for r in range(2):
+        lo, hi = W.shard_range(total, r, 2)
+        ht, hw = hec.curve_map(q, g, d, with_lambda=lam, index_range=(lo, hi - lo))
+        dt, dw = hec.curve_map(q, g, d, with_lambda=lam, index_range=(lo, hi - lo), device=True)
+        assert dt.is_cuda and dw.is_cuda
+        assert (dt.cpu().numpy().view(np.uint32) == ht).all() and (dw.cpu().numpy().view(np.uint64) == hw).all()
+        parts_t.append(D._to_device(dt, torch.int32))
+        parts_w.append(D._to_device(hw, torch.int64))                          # numpy input: the host-to-device branch
+    mt, mw = D._merge(torch.cat(parts_t), torch.cat(parts_w))
+    ft, fw = hec.curve_map(q, g, d, with_lambda=lam)
+    assert mt.is_cuda and (mt.cpu().numpy().view(np.uint32) == ft).all() and (mw.cpu().numpy().view(np.uint64) == fw).all()
+
+
 def test_global_curve_map_single_rank(cuda):
     """distributed.global_curve_map without a process group is hec_curve_map (the N > 1 exchange is all-gather +
     hec_histogram_merge, covered by test_curve_map_ranges_merge_to_the_map and the gloo tests)."""
