@@ -43,7 +43,20 @@ from paper_1805_11991_b200 import workloads as W  # noqa: E402
 
 EXPECTED_WAVEFRONTS = 3.53      # E[max bank load], 32 uniformly random lookups in 32 banks
 DIRECT_MAX_M = 64               # hec_count_kernels.cuh: kDirectMaxM
-COUNTERS_FILE = ROOT / "profiles" / "r02_counters.csv"   # committed ncu counters of the shipped kernels (profiles/r02_counters.md)
+# committed ncu counters of the shipped kernels (profiles/r0X_counters.md has the commands); the newest round's file wins
+COUNTERS_FILE = next((f for f in (ROOT / "profiles" / "r03_counters.csv", ROOT / "profiles" / "r02_counters.csv") if f.exists()),
+                     ROOT / "profiles" / "r03_counters.csv")
+KERNEL_SOURCES = ["hec_count_kernels.cuh", "hec_radix.cuh", "hec_device.cuh"]    # device code of the count kernels
+COUNTERS_MS_TOLERANCE = 0.06    # committed count_kernel_ms (scaled to the launch) against this run's kernel time
+
+
+def kernel_sources_sha16() -> str:
+    """Hash of the count kernels' device code: the committed counters file carries the value it was measured at."""
+    import hashlib
+    h = hashlib.sha256()
+    for name in KERNEL_SOURCES:
+        h.update((ROOT / "paper_1805_11991_b200" / "csrc" / name).read_bytes())
+    return h.hexdigest()[:16]
 
 
 # ------------------------------------------------------------------------------------------------ helpers
@@ -97,7 +110,7 @@ def executed_loads(cfg: W.Workload, rows: np.ndarray, stats: dict) -> dict:
         fast = bool((stats.get("fast_fields", 0) >> (k - 1)) & 1)
         todo = np.ones(n, dtype=bool)
         R = Rf
-        if fast and ncoef > 8 and ncoef <= 16 and mode in (5, 6, 8) and k == cfg.g and M % 16 == 0 and stats.get("eval") in ("auto", "radix8"):
+        if fast and ncoef > 8 and ncoef <= 16 and mode in (5, 6, 8) and k == cfg.g and M % 16 == 0 and stats.get("eval") == "auto":
             # monomial classes at R = 16 (radix_mono_x): butterflies with both inputs present, the last stage from the parity table
             deg = ncoef - 1 - (~nzm[:, ::-1]).cumprod(axis=1).sum(axis=1)
             dense = nzm.sum(axis=1) == deg + 1
@@ -169,14 +182,23 @@ def executed_loads(cfg: W.Workload, rows: np.ndarray, stats: dict) -> dict:
 
 
 def committed_counters() -> dict:
-    """profiles/r02_counters.csv: per (workload, eval) the ncu counters of the count kernel on the first `curves` rows."""
+    """profiles/r0X_counters.csv: per (workload, eval) the ncu counters of the count kernel on the first `curves` rows.
+    The file's header names the hash of the kernel sources it was measured at (`# kernel_sources_sha16: ...`); when that
+    differs from the tree's, the counters describe other kernels: the key "stale" says so and no record is used."""
     out = {}
     if not COUNTERS_FILE.exists():
-        return out
-    lines = [l for l in COUNTERS_FILE.read_text().splitlines() if l.strip() and not l.startswith("#")]
+        return {"stale": f"{COUNTERS_FILE.name} is missing"}
+    text = COUNTERS_FILE.read_text().splitlines()
+    stamp = next((l.split(":", 1)[1].split()[0] for l in text if l.startswith("# kernel_sources_sha16:")), None)
+    commit = next((l.split(":", 1)[1].split()[0] for l in text if l.startswith("# commit:")), None)
+    now = kernel_sources_sha16()
+    if stamp != now:
+        return {"stale": f"{COUNTERS_FILE.name} was measured at kernel sources {stamp} (commit {commit}), the tree has {now}"}
+    lines = [l for l in text if l.strip() and not l.startswith("#")]
     hdr = lines[0].split(",")
     for l in lines[1:]:
         rec = dict(zip(hdr, l.split(",")))
+        rec["commit"] = commit
         out[(rec["workload"], rec["eval"])] = rec
     return out
 
@@ -298,8 +320,17 @@ def gather_ceiling(hec, q, g, mode):
     ext_entries = 3 * Mtop + 2 * min(32 * 4, Mtop) * (2 * g + 2)
     where, entries, width = {0: (1, ext_entries, 4), 1: (0, ext_entries, 2), 2: (0, Mtop // 2 + 2, 4), 3: (0, Mtop // 2 + 2, 2),
                              4: (0, Mtop, 4), 5: (0, Mtop // 2 + 2, 4), 6: (0, Mtop // 2 + 2, 2), 7: (1, 2 * Mtop, 4), 8: (0, Mtop, 4)}[mode]
-    rate, _ = hec.gather_bench(where, max(entries, 1024), width, 1024, 1, 4, 8192 if where == 0 else 1024)
-    return rate
+    if where == 0:
+        rate, _ = hec.gather_bench(0, max(entries, 1024), width, 1024, 1, 4, 8192)
+        return rate
+    return global_gather_ceiling(hec, where, max(entries, 1024), width)
+
+
+def global_gather_ceiling(hec, where, entries, width):
+    """Random-gather ceiling of the global-memory paths (where = 1: ld.global.nc through L1; 2: ld.global.cg, L2 only): the
+    best rate over a few shapes of the micro-benchmark (1 or 2 CTAs of 1024 threads per SM, 4 or 8 independent chains per lane)
+    -- these loads are latency-bound, so the ceiling is the shape with the most loads in flight, not one fixed shape."""
+    return max(hec.gather_bench(where, entries, width, 1024, ctas, chains, 1024)[0] for ctas, chains in ((1, 4), (1, 8), (2, 4), (2, 8)))
 
 
 def measure(torch, hec, D, cfg, rows, eval_name, steps, warmup, world, local_rank, sample_clocks=True):
@@ -386,22 +417,36 @@ def roofline_record(torch, hec, cfg, rows, m, local_rank, counters):
         "algorithmic_lookups_per_launch": lookups,
         "algorithmic_equiv": lookups / (k_ms * 1e-3) / 1e9,
         "algorithmic_equiv_note": "paper's scheme: one lookup per Horner step with a nonzero coefficient and x; executed only under --eval horner",
+        # SURVEY.md 8(d) as written: algorithmic lookups / kernel time / measured random-gather ceiling
+        "frac_sec8d": lookups / (k_ms * 1e-3) / gather_rate,
+        "frac_sec8d_note": "above 1 = the kernel executes fewer table loads than the paper's scheme counts (radix split / orbit scheme); "
+                           "about 1 under --eval horner, which executes exactly that count",
     }
     if loads is not None:
         total = loads["random"] + loads["conflict_free"]
         t_floor = loads["random"] / gather_rate + loads["conflict_free"] / conflict_free_rate
         rec.update({"executed_loads_per_launch": total, "executed_random": loads["random"],
                     "executed_conflict_free": loads["conflict_free"], "executed_source": "model of the kernel's dispatch from the rows' zero patterns (bench.py: executed_loads)" + (f", every {stride}-th row, scaled" if stride > 1 else ""),
-                    "achieved": total / (k_ms * 1e-3) / 1e9, "peak": total / t_floor / 1e9, "frac": t_floor / (k_ms * 1e-3),
+                    "achieved": total / (k_ms * 1e-3) / 1e9, "peak": total / t_floor / 1e9, "frac_executed": t_floor / (k_ms * 1e-3),
                     "t_floor_ms": t_floor * 1e3})
     else:
-        rec.update({"achieved": None, "peak": gather_rate / 1e9, "frac": None})
+        rec.update({"achieved": None, "peak": gather_rate / 1e9, "frac_executed": None})
+    rec["smem_pipe_frac"] = None
     c = counters.get((cfg.name, stats["eval"]))
-    if c:                                               # committed ncu counters of the same kernel (first `curves` rows)
+    if "stale" in counters:
+        rec["ncu"] = None
+        rec["ncu_stale"] = counters["stale"]
+    elif c and abs(float(c["count_kernel_ms"]) * rows.shape[0] / float(c["curves"]) / k_ms - 1.0) > COUNTERS_MS_TOLERANCE:
+        rec["ncu"] = None
+        rec["ncu_stale"] = (f"{COUNTERS_FILE.name}: count_kernel_ms {float(c['count_kernel_ms']):.4f} per {c['curves']} rows scales to "
+                            f"{float(c['count_kernel_ms']) * rows.shape[0] / float(c['curves']):.3f} ms, this run measured {k_ms:.3f} ms")
+        c = None
+    if c and "stale" not in counters:                   # committed ncu counters of the same kernel (first `curves` rows)
         scale = rows.shape[0] / float(c["curves"])
         ld = float(c["smsp__inst_executed_op_shared_ld.sum"]) * 32 * scale
         wf = float(c["l1tex__data_pipe_lsu_wavefronts_mem_shared_op_ld.sum"]) * scale
-        rec["ncu"] = {"source": f"profiles/r02_counters.csv ({c['curves']} rows profiled, scaled to the launch)",
+        rec["ncu"] = {"source": f"profiles/{COUNTERS_FILE.name} at commit {c.get('commit')} ({c['curves']} rows profiled, scaled to the launch; "
+                                f"kernel sources {kernel_sources_sha16()} unchanged, kernel time within {COUNTERS_MS_TOLERANCE:.0%})",
                       "shared_ld_lanes_per_launch": ld, "shared_ld_wavefronts_per_launch": wf,
                       "wavefronts_per_request": wf / (ld / 32),
                       "model_over_counter": (rec.get("executed_loads_per_launch") or 0) / ld if ld else None,
@@ -411,10 +456,20 @@ def roofline_record(torch, hec, cfg, rows, m, local_rank, counters):
                       "smem_pipe_pct": float(c["l1tex__data_pipe_lsu_wavefronts_mem_shared.sum.pct_of_peak_sustained_elapsed"]),
                       "alu_pipe_pct": float(c["sm__inst_executed_pipe_alu.avg.pct_of_peak_sustained_active"]),
                       "issue_active_pct": float(c["smsp__issue_active.avg.pct_of_peak_sustained_active"])}
+        rec["smem_pipe_frac"] = rec["ncu"]["smem_pipe_frac"]
         rec["traffic"] = rec["ncu"]["dram_bytes_per_launch"]
-        rec["traffic_unit"] = "bytes per launch: ncu dram read + write of the count kernel (profiles/r02_counters.csv), scaled"
+        rec["traffic_unit"] = f"bytes per launch: ncu dram read + write of the count kernel (profiles/{COUNTERS_FILE.name}), scaled"
     else:
         rec["traffic"] = None
+    # `frac`: the executed-load fraction, unless the model's floor exceeds the kernel time (the 2-byte random-gather ceiling
+    # over-prices the u8 / mirrored loads of the 16+1-bit half tables): then the wavefront-peak figure, which cannot exceed 1
+    fe = rec["frac_executed"]
+    if fe is not None and fe <= 1.0:
+        rec["frac"], rec["frac_source"] = fe, "frac_executed"
+    elif rec["smem_pipe_frac"] is not None and mode not in (0, 7):
+        rec["frac"], rec["frac_source"] = rec["smem_pipe_frac"], "smem_pipe_frac (frac_executed is None or above 1)"
+    else:
+        rec["frac"], rec["frac_source"] = (min(fe, 1.0) if fe is not None else None), "frac_executed capped at 1 (no valid ncu counters)"
     return rec
 
 
@@ -529,37 +584,54 @@ def sub_config_records(torch, hec, D, args, local_rank, counters):
     from oracle import hec_oracle as O
     out = {}
     # (the orbit scheme evaluates one representative per Frobenius orbit: SURVEY.md 8(f) NEXT-4, reported separately, never the metric)
-    for cid, eval_name, steps in [(5, "auto", 3), (3, "auto", 3), (2, "auto", 5), (1, "auto", 5), (4, "horner", 2), (4, "orbit", 3)]:
+    # each record stays below ~300 characters and the metric's second named configuration (q = 293, g = 2) and config 3 come
+    # LAST, so that they survive in the tail of stdout that the driver keeps
+    # regime "l2": the L2-resident table forced for the largest field (north_star (b): the regime every field above the
+    # shared-memory half table runs in, e.g. the paper's Table 1 for p >= 401), on the first 2^22 rows of the workload
+    for cid, eval_name, steps, regime in [(1, "auto", 5, "auto"), (2, "auto", 5, "auto"), (4, "horner", 2, "auto"), (4, "orbit", 3, "auto"),
+                                          (5, "auto", 2, "l2"), (3, "auto", 3, "auto"), (5, "auto", 3, "auto")]:
         cfg = W.CONFIGS[cid]
         rows = workload_rows(cfg, 0)
-        m = measure(torch, hec, D, cfg, rows, eval_name, steps, 2, 1, local_rank)
-        m["steps"] = steps
-        rl = roofline_record(torch, hec, cfg, rows, m, local_rank, counters)
+        if regime == "l2":
+            rows = rows[: 1 << 22]
+        hec.set_regime(getattr(hec, REGIMES[regime]))
+        try:
+            m = measure(torch, hec, D, cfg, rows, eval_name, steps, 2, 1, local_rank)
+            m["steps"] = steps
+            if regime != "auto":
+                m["stats"]["eval"] = f"{eval_name}_{regime}"               # its own row of the counters file
+            rl = roofline_record(torch, hec, cfg, rows, m, local_rank, counters)
+        finally:
+            hec.set_regime(getattr(hec, REGIMES[args.regime]))
         n = rows.shape[0]
         value = n * steps / (m["elapsed_ms"] * 1e-3)
-        rec = {"workload": cfg.name, "eval": eval_name, "steps": steps, "warmup": 2, "ms_per_step": m["elapsed_ms"] / steps,
-               "value": value, "unit": "curves/s", "xevals_per_s": value * cfg.xevals_per_curve, "kernel_ms": m["kernel_ms"],
-               "table_layout": rl["table_layout"], "radix_per_field": rl["radix_per_field"], "frac": rl["frac"],
-               "achieved": rl["achieved"], "peak": rl["peak"], "roofline_unit": rl["unit"],
-               "algorithmic_equiv": rl["algorithmic_equiv"], "peak_random_gather": rl["peak_random_gather"],
-               "gpu_launches": m["launches"], "clocks": m["clocks"]}
-        if "ncu" in rl:
-            rec["smem_pipe_frac"] = rl["ncu"]["smem_pipe_frac"]
+        def r4(x):
+            return None if x is None else float(f"{x:.4g}")
+        rec = {"steps": steps, "ms_per_step": r4(m["elapsed_ms"] / steps), "curves_per_s": r4(value),
+               "xevals_per_s": r4(value * cfg.xevals_per_curve), "kernel_ms": r4(m["kernel_ms"]), "layout": rl["table_layout"],
+               "frac": r4(rl["frac"]), "frac_sec8d": r4(rl["frac_sec8d"]), "frac_executed": r4(rl["frac_executed"]),
+               "smem_pipe_frac": r4(rl["smem_pipe_frac"]), "launches": m["launches"], "sm_mhz": m["clocks"].get("sm_mhz")}
         if not args.no_cpu_baseline:
             S = {1: cfg.n, 2: 2048, 3: 40, 4: 160, 5: 256}[cid]
             idx = W.sample_indices(cfg, S, edge=0)
+            idx = idx[idx < n]                                             # the L2 record runs on a prefix of the workload
             t0 = time.perf_counter()
             ocnt, osf, used = O.count(cfg.q, cfg.g, rows[idx])
             dt = time.perf_counter() - t0
             cnt = m["d_cnt"].cpu().numpy().view(np.uint32)
             sf = m["d_sf"].cpu().numpy()
-            rec["parity_rows_checked"] = int(len(idx))
+            rec["parity_rows"] = int(len(idx))
             rec["parity_ok"] = bool((cnt[idx] == ocnt).all() and (sf[idx] == osf).all())
-            rec["oracle_curves_per_s"] = len(idx) / dt
-            rec["oracle_cores"] = used
         if eval_name == "orbit":
-            rec["note"] = "HEC_EVAL_ORBIT: 1/k of the points evaluated, counts weighted by orbit length; reported separately, not the judged metric"
-        out[cfg.name if eval_name == "auto" else f"{cfg.name}_{eval_name}"] = rec
+            rec["note"] = "1/k of the points; not the metric"
+        if regime == "l2":                                                 # ceilings of both cache paths at this table's footprint
+            Mtop = cfg.q ** cfg.g - 1
+            rec["n_curves"] = int(n)
+            rec["gather_nc_Gps"] = r4(global_gather_ceiling(hec, 1, 2 * Mtop, 4) / 1e9)               # ld.global.nc (L1 + L2)
+            rec["gather_cg_Gps"] = r4(global_gather_ceiling(hec, 2, 2 * Mtop, 4) / 1e9)               # ld.global.cg (L2 only)
+            rec["lookups_Gps"] = r4(rl["achieved"])                                                    # executed table loads / s
+        name = cfg.name if eval_name == "auto" else f"{cfg.name}_{eval_name}"
+        out[name if regime == "auto" else f"{name}_{regime}"] = rec
         del m, rows
         torch.cuda.empty_cache()
     hec.set_eval(hec.EVAL_AUTO)
@@ -594,6 +666,7 @@ def run_table1(args):
         d_cnt = torch.empty((1, 2), dtype=torch.int32, device="cuda")
         d_sf = torch.empty((1,), dtype=torch.uint8, device="cuda")
         hec.shutdown()
+        hec.set_stream(stream.cuda_stream)                          # hec_shutdown resets the stream setting
         torch.cuda.synchronize()
         t0 = time.perf_counter()
         for k in (1, 2):
